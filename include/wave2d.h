@@ -1,0 +1,154 @@
+/*
+ * wave2d.h -- C ABI of libwave2d.so: B200-native (sm_100a) ADI time stepping for the 2D acoustic
+ * wave equation
+ *
+ *     u_tt - c(t) (u_xx + u_yy) = f(t,x,y)  on [0,T] x [0,l]^2,   u(0) = phi, u_t(0) = psi,
+ *     u = 0 on the boundary                                     (eqs (2.1)-(2.5))
+ *
+ * discretised on the grid t_k = k tau, x_i = i h1, y_j = j h2, h_d = l/N_d ((2.6)-(2.7))
+ * by the split implicit scheme (2.11)-(2.12) and stepped by Algorithm 1
+ * (PAPER.md:99-118): per time step one batched family of tridiagonal solves along x (one per grid
+ * row), one along y (one per grid column), and a rotation of the time levels.  Every step of that
+ * path runs in hand-written CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions (all entry points):
+ *   - extern "C"; every function returns an int status (WAVE2D_OK == 0, errors < 0) and never throws
+ *     or aborts.  wave2d_strerror() names a status, wave2d_last_error() gives detail (CUDA error text).
+ *   - N1, N2 >= 2 are the paper's INTERVAL counts; a line along x has n1 = N1-1 unknowns, along y
+ *     n2 = N2-1.  Boundary nodes are never stored, read or written: (2.10) fixes them to 0.
+ *   - Field arrays (phi, psi, s, u_out) are INTERIOR arrays of n2 rows x n1 columns: node (i,j),
+ *     1 <= i <= n1, 1 <= j <= n2, lives at [(j-1)*ld + (i-1)], ld >= n1 in ELEMENTS.  The element type
+ *     is the handle's dtype (double for WAVE2D_F64, float for WAVE2D_F32).
+ *   - Field pointers may be HOST or DEVICE pointers (detected with cudaPointerGetAttributes; a torch
+ *     tensor passes .data_ptr()).  Inputs are copied during the call: the caller keeps ownership and may
+ *     free them on return.  Time-sample arrays (c_half, g_half) are HOST double arrays for both dtypes.
+ *   - Half-level index n = 0,1,2,...: t = n tau/2; the half-step n -> n+1 is implicit in x for even n and
+ *     in y for odd n.  c_half[n] = c(n tau/2), g_half[n] = g(n tau/2).
+ *   - The handle owns all device memory it allocates (three pitched field buffers, the optional source
+ *     field, a per-half-step scalar table) and frees it in wave2d_destroy().
+ *   - One handle is single-threaded; distinct handles are independent.  Work is asynchronous on the
+ *     handle's stream unless stated otherwise.
+ *
+ * State machine: create -> (set_* in any order; set_initial required) -> run* -> get.
+ *   run before set_initial                      -> WAVE2D_ERR_STATE
+ *   cumulative steps > M                        -> WAVE2D_ERR_RANGE
+ *   set_speed / set_source / set_option after the first run -> WAVE2D_ERR_STATE
+ *   set_initial at any time resets the step count k to 0.
+ */
+#ifndef WAVE2D_H
+#define WAVE2D_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wave2d_s wave2d_t; /* opaque */
+
+enum { WAVE2D_F64 = 0, WAVE2D_F32 = 1 };
+
+enum {
+    WAVE2D_OK = 0,
+    WAVE2D_ERR_ARG = -1,         /* NULL / out-of-range argument                                  */
+    WAVE2D_ERR_STATE = -2,       /* call not allowed in the handle's current state                */
+    WAVE2D_ERR_ALLOC = -3,       /* host or device allocation failed                              */
+    WAVE2D_ERR_CUDA = -4,        /* a CUDA call failed; see wave2d_last_error()                   */
+    WAVE2D_ERR_UNSUPPORTED = -5, /* no solver path can handle this size / option on this device   */
+    WAVE2D_ERR_RANGE = -6        /* more than M steps requested                                   */
+};
+
+/* Solver selection for wave2d_set_option(h, "solver", v). */
+enum {
+    WAVE2D_SOLVER_AUTO = 0,     /* streamed/windowed kernels where the decay bound allows, else CR     */
+    WAVE2D_SOLVER_CR = 1,       /* exact whole-line cyclic reduction in shared memory (any tau/h)      */
+    WAVE2D_SOLVER_STREAM = 2    /* force the streamed kernels; ERR_UNSUPPORTED if the bound fails      */
+};
+
+/*
+ * Create a solver for the grid of (2.6)-(2.7): N1 x N2 intervals on [0,l]^2, time step tau, at most M
+ * steps (T = M tau), dtype WAVE2D_F64 or WAVE2D_F32.  Defaults: c == 1, no source, gamma = 2,
+ * kappa = 1/2 (see wave2d_set_option).  Uses the current CUDA device and the legacy default stream.
+ * Errors: ERR_ARG (N < 2, l <= 0, tau <= 0, M < 0, bad dtype, out == NULL), ERR_ALLOC, ERR_CUDA
+ * (no device, or not an sm_100 device), ERR_UNSUPPORTED (a line too long for every solver path).
+ */
+int wave2d_create(wave2d_t **out, int N1, int N2, double l, double tau, int M, int dtype);
+
+/* Free the handle and everything it owns.  NULL-safe.  Synchronises the handle's stream first. */
+void wave2d_destroy(wave2d_t *h);
+
+/* Use `cuda_stream` (a cudaStream_t; NULL = legacy default stream) for all later work. */
+int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
+
+/*
+ * Options (before the first run only):
+ *   "gamma"  time-quotient constant, > 0.  Default 2.   | gamma = 2, kappa = 1/2 is the consistent
+ *   "kappa"  source weight.              Default 0.5.   | locally-one-dimensional form of (2.11)-(2.12);
+ *                                                       | gamma = kappa = 1 is the scheme as printed
+ *                                                       |, which solves u_tt = 2c Lap u + 4f.
+ *   "solver" one of WAVE2D_SOLVER_*.     Default AUTO.
+ *   "graph"  1 (default): the step loop is replayed as a CUDA Graph; 0: plain launches.
+ * Errors: ERR_ARG (unknown name / bad value), ERR_STATE.
+ */
+int wave2d_set_option(wave2d_t *h, const char *name, double value);
+
+/*
+ * Initial data (2.2)-(2.3), discretised as in (2.9) adapted to half-levels:
+ *   u^0 = phi,  u^{-1/2} = phi - (tau/2) psi     (psi == NULL means psi = 0, i.e. Algorithm 1's "u = U0").
+ * Resets the step count to 0.  Synchronous for host pointers.
+ */
+int wave2d_set_initial(wave2d_t *h, const void *phi, const void *psi, long ld);
+
+/*
+ * Speed samples c_half[n] = c(n tau/2), n = 0..2M (count == 2M+1), or one constant (count == 1).
+ * Every value must be > 0 ("positive speed function"), else ERR_ARG.  c_{-1} := c_0.
+ */
+int wave2d_set_speed(wave2d_t *h, const double *c_half, int count);
+
+/*
+ * Source f(t,x,y) = g(t) s(x,y).  s: interior array (NULL clears the source);
+ * g_half[n] = g(n tau/2), n = 0..2M-1 (count >= 2M), or NULL for g == 1 (a time-independent full-grid
+ * source).  Half-step n uses g_half[n]: f^k in (2.11), f^{k+1/2} in (2.12).
+ */
+int wave2d_set_source(wave2d_t *h, const void *s, long ld, const double *g_half, int count);
+
+/*
+ * Advance `steps` time steps (Algorithm 1's loop body: x-sweep (2.11), y-sweep (2.12), rotate levels).
+ * Asynchronous on the handle's stream.  Errors: ERR_STATE, ERR_RANGE, ERR_UNSUPPORTED, ERR_CUDA.
+ */
+int wave2d_run(wave2d_t *h, int steps);
+
+/* Copy u^k (k = steps done so far) / u^{k-1/2} to u_out (host or device).  Synchronises the stream. */
+int wave2d_get(wave2d_t *h, void *u_out, long ld);
+int wave2d_get_prev(wave2d_t *h, void *u_out, long ld);
+
+/* Number of completed time steps k. */
+int wave2d_steps_done(const wave2d_t *h, int *k);
+
+/* Block until all work queued on the handle's stream has finished. */
+int wave2d_sync(wave2d_t *h);
+
+/*
+ * Introspection for benchmarks and tests.  name:
+ *   "solver_x", "solver_y"   solver path in use per direction (WAVE2D_SOLVER_CR / _STREAM), after planning
+ *   "halo_x", "halo_y"       window halo H (points) derived from the decay bound rho^H <= 1e-18
+ *   "rho_x", "rho_y"         largest off-diagonal decay ratio rho over all half-steps
+ *   "launches"               kernels launched by this handle so far (graph nodes count individually)
+ *   "pitch"                  internal row pitch in elements
+ *   "device_bytes"           device memory owned by the handle
+ * The plan is (re)computed by this call if needed.  Errors: ERR_ARG.
+ */
+int wave2d_get_info(wave2d_t *h, const char *name, double *value);
+
+/*
+ * Time the two sweeps separately: runs `steps` time steps with plain launches and CUDA events around
+ * every kernel on the handle's stream, returning the mean milliseconds per launch of the x-sweep and
+ * y-sweep kernels.  Synchronous.  Counts toward the step total like wave2d_run.
+ */
+int wave2d_profile_sweeps(wave2d_t *h, int steps, double *ms_x, double *ms_y);
+
+const char *wave2d_strerror(int status);
+const char *wave2d_last_error(const wave2d_t *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WAVE2D_H */
