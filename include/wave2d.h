@@ -58,15 +58,16 @@ enum {
 
 /* Solver selection for wave2d_set_option(h, "solver", v). */
 enum {
-    WAVE2D_SOLVER_AUTO = 0,     /* streamed/windowed kernels where the decay bound allows, else CR     */
-    WAVE2D_SOLVER_CR = 1,       /* exact whole-line cyclic reduction in shared memory (any tau/h)      */
-    WAVE2D_SOLVER_STREAM = 2    /* force the streamed kernels; ERR_UNSUPPORTED if the bound fails      */
+    WAVE2D_SOLVER_AUTO = 0,     /* streamed kernels where the decay bound rho^H <= tol allows, else EXACT */
+    WAVE2D_SOLVER_EXACT = 1,    /* untruncated two-pass elimination through HBM (any tau/h)              */
+    WAVE2D_SOLVER_STREAM = 2    /* force the streamed kernels; ERR_UNSUPPORTED if the bound fails        */
 };
 
 /*
  * Create a solver for the grid of (2.6)-(2.7): N1 x N2 intervals on [0,l]^2, time step tau, at most M
  * steps (T = M tau), dtype WAVE2D_F64 or WAVE2D_F32.  Defaults: c == 1, no source, gamma = 2,
- * kappa = 1/2 (see wave2d_set_option).  Uses the current CUDA device and the legacy default stream.
+ * kappa = 1/2 (see wave2d_set_option).  Uses the current CUDA device and a non-blocking stream of its own
+ * (CUDA Graph capture is not possible on the legacy default stream).
  * Errors: ERR_ARG (N < 2, l <= 0, tau <= 0, M < 0, bad dtype, out == NULL), ERR_ALLOC, ERR_CUDA
  * (no device, or not an sm_100 device), ERR_UNSUPPORTED (a line too long for every solver path).
  */
@@ -75,7 +76,8 @@ int wave2d_create(wave2d_t **out, int N1, int N2, double l, double tau, int M, i
 /* Free the handle and everything it owns.  NULL-safe.  Synchronises the handle's stream first. */
 void wave2d_destroy(wave2d_t *h);
 
-/* Use `cuda_stream` (a cudaStream_t; NULL = legacy default stream) for all later work. */
+/* Use `cuda_stream` (a cudaStream_t) for all later work; NULL returns to the handle's own stream.  On the
+ * legacy default stream the step loop falls back from graph replay to plain launches. */
 int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
 
 /*
@@ -86,6 +88,9 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *                                                       |, which solves u_tt = 2c Lap u + 4f.
  *   "solver" one of WAVE2D_SOLVER_*.     Default AUTO.
  *   "graph"  1 (default): the step loop is replayed as a CUDA Graph; 0: plain launches.
+ *   "graph_steps"  time steps per graph replay (multiple of 3, the period of the buffer ring).  Default 12.
+ *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (consumer warps / units per stage / stages).
+ *   "chunks_x", "chunks_y" tuning: number of chunks a line is cut into (0 = planned from the SM count).
  * Errors: ERR_ARG (unknown name / bad value), ERR_STATE.
  */
 int wave2d_set_option(wave2d_t *h, const char *name, double value);
@@ -128,9 +133,11 @@ int wave2d_sync(wave2d_t *h);
 
 /*
  * Introspection for benchmarks and tests.  name:
- *   "solver_x", "solver_y"   solver path in use per direction (WAVE2D_SOLVER_CR / _STREAM), after planning
- *   "halo_x", "halo_y"       window halo H (points) derived from the decay bound rho^H <= 1e-18
- *   "rho_x", "rho_y"         largest off-diagonal decay ratio rho over all half-steps
+ *   "solver_x", "solver_y"   solver path in use per direction (WAVE2D_SOLVER_EXACT / _STREAM), after planning
+ *   "halo_x", "halo_y"       look-ahead H (points) with rho^H <= 1e-17 (fp64) / 1e-8 (fp32)
+ *   "rho_x", "rho_y"         largest decay ratio rho over all half-steps
+ *   "chunks_*", "grid_*", "ctas_per_sm_*", "smem_*", "threads_*", "unit_*", "upc_*"   launch geometry
+ *   "source_window"          points kept of the source field (its non-zero bounding box)
  *   "launches"               kernels launched by this handle so far (graph nodes count individually)
  *   "pitch"                  internal row pitch in elements
  *   "device_bytes"           device memory owned by the handle

@@ -1,0 +1,786 @@
+// wave2d.cu -- C ABI of libwave2d.so (include/wave2d.h): host-side planning, the per-half-step scalar
+// table (A0), TMA descriptors, the CUDA-Graph step loop (A6/A7) and the launches of kernels.cuh.
+#include "../../include/wave2d.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace w2d;
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// Kernel variants: (NW consumer warps, XB units per stage, NSTAGE) per direction, per look-ahead NB.
+// ------------------------------------------------------------------------------------------------
+struct Variant {
+    int dir, nb, nw, xb, nstage, smem, threads, elem;   // elem = sizeof(T)
+    const void* fn;
+};
+
+template <typename T, int DIR, int NB, int NW, int XB, int NSTAGE>
+Variant make_variant()
+{
+    using K = StreamCfg<T, DIR, NB, NW, XB, NSTAGE>;
+    return Variant{DIR, NB, NW, XB, NSTAGE, K::SMEM_BYTES, K::THREADS, (int)sizeof(T),
+                   reinterpret_cast<const void*>(&wave2d_sweep_stream<T, DIR, NB, NW, XB, NSTAGE>)};
+}
+
+constexpr int NVAR = 4;   // shape variants per (dtype, dir, NB); index 0 is the default
+template <typename T, int DIR, int NB>
+void add_shapes(std::vector<Variant>& v)
+{
+    if (DIR == 0) {
+        v.push_back(make_variant<T, DIR, NB, 1, 2, 4>());
+        v.push_back(make_variant<T, DIR, NB, 1, 1, 6>());
+        v.push_back(make_variant<T, DIR, NB, 2, 2, 3>());
+        v.push_back(make_variant<T, DIR, NB, 1, 4, 3>());
+    } else {
+        v.push_back(make_variant<T, DIR, NB, 2, 1, 4>());
+        v.push_back(make_variant<T, DIR, NB, 1, 1, 6>());
+        v.push_back(make_variant<T, DIR, NB, 4, 1, 3>());
+        v.push_back(make_variant<T, DIR, NB, 2, 2, 3>());
+    }
+}
+constexpr int NB_MAX_F64 = 3, NB_MAX_F32 = 2;
+
+const std::vector<Variant>& variants()
+{
+    static std::vector<Variant> v = [] {
+        std::vector<Variant> w;
+        add_shapes<double, 0, 1>(w); add_shapes<double, 0, 2>(w); add_shapes<double, 0, 3>(w);
+        add_shapes<double, 1, 1>(w); add_shapes<double, 1, 2>(w); add_shapes<double, 1, 3>(w);
+        add_shapes<float, 0, 1>(w);  add_shapes<float, 0, 2>(w);
+        add_shapes<float, 1, 1>(w);  add_shapes<float, 1, 2>(w);
+        return w;
+    }();
+    return v;
+}
+
+const Variant* find_variant(int elem, int dir, int nb, int shape)
+{
+    int seen = 0;
+    for (const Variant& v : variants())
+        if (v.elem == elem && v.dir == dir && v.nb == nb) {
+            if (seen == shape) return &v;
+            ++seen;
+        }
+    return nullptr;
+}
+
+// ------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled()
+{
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) != cudaSuccess) p = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+
+struct DirPlan {
+    int solver = WAVE2D_SOLVER_STREAM;   // STREAM or EXACT after planning
+    int nb = 1, halo = 0, shape = 0;
+    double rho = 0.0;
+    const Variant* var = nullptr;
+    int n = 0, nlines = 0, ntiles = 0, upc = 0, nchunks = 0, total_units = 0, grid = 0, ctas_per_sm = 0;
+};
+
+}  // namespace
+
+struct wave2d_s {
+    int N1, N2, n1, n2, M, dtype, elem;
+    double l, tau, gamma = 2.0, kappa = 0.5;
+    int opt_solver = WAVE2D_SOLVER_AUTO, opt_graph = 1, opt_graph_steps = 12, opt_shape[2] = {0, 0};
+    int opt_chunks[2] = {0, 0};
+    cudaStream_t own_stream = nullptr, stream = nullptr;
+    int num_sms = 0;
+
+    long long pitch = 0;                 // elements
+    void* buf[3] = {nullptr, nullptr, nullptr};
+    std::vector<double> c_half, g_half;  // g_half empty: g == 1
+    bool have_src = false;
+    void* src_dev[2] = {nullptr, nullptr};    // [0]: x sweep (transposed window), [1]: y sweep (natural window)
+    int win_i0 = 0, win_j0 = 0, win_w = 0, win_h = 0;
+
+    std::vector<double> table;           // host copy
+    double* d_table = nullptr;
+    int* d_k = nullptr;
+    double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
+    bool plan_ok = false;
+    DirPlan plan[2];
+    CUtensorMap tm_load[2][3], tm_store[3];   // [dir][buffer]
+    cudaGraphExec_t gexec = nullptr;
+    int gexec_steps = 0;
+
+    bool have_initial = false, ran = false;
+    int k = 0;                           // completed steps
+    long long launches = 0;
+    size_t device_bytes = 0;
+    std::string err;
+};
+
+namespace {
+
+#define W2D_CUDA(h, call)                                                                      \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            (h)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                     \
+            (void)cudaGetLastError();                                                          \
+            return WAVE2D_ERR_CUDA;                                                            \
+        }                                                                                      \
+    } while (0)
+
+int dev_alloc(wave2d_t* h, void** p, size_t bytes)
+{
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        h->err = std::string("cudaMalloc: ") + cudaGetErrorString(e);
+        (void)cudaGetLastError();
+        *p = nullptr;
+        return WAVE2D_ERR_ALLOC;
+    }
+    h->device_bytes += bytes;
+    return WAVE2D_OK;
+}
+
+void drop_graph(wave2d_t* h)
+{
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    h->gexec = nullptr;
+    h->gexec_steps = 0;
+}
+
+void invalidate_plan(wave2d_t* h)
+{
+    h->plan_ok = false;
+    drop_graph(h);
+}
+
+// ---- A0: per-half-step scalars, fp64 on the host -----------------------------------------
+void build_table(wave2d_t* h)
+{
+    const int nhalf = 2 * h->M;
+    h->table.assign(static_cast<size_t>(std::max(nhalf, 1)) * ROW_DOUBLES, 0.0);
+    const double t2 = h->tau * h->tau;
+    for (int n = 0; n < nhalf; ++n) {
+        double* row = &h->table[static_cast<size_t>(n) * ROW_DOUBLES];
+        const double hd = h->l / ((n & 1) == 0 ? h->N1 : h->N2);                  // reading A3
+        const double ap = t2 * h->c_half[n + 1] / (2.0 * hd * hd);
+        const double am = t2 * h->c_half[n > 0 ? n - 1 : 0] / (2.0 * hd * hd);      // reading A5: c_{-1} := c_0
+        const double g = h->g_half.empty() ? 1.0 : h->g_half[n];                   // reading A8
+        const double beta = h->gamma + 2.0 * ap;
+        const double rho = 2.0 * ap / (beta + std::sqrt(beta * beta - 4.0 * ap * ap));
+        row[ROW_AM] = am;
+        row[ROW_Q] = h->have_src ? h->kappa * t2 * g : 0.0;
+        row[ROW_RHO] = rho;
+        row[ROW_INV] = 1.0 / (beta - ap * rho);
+        row[ROW_C1] = -(h->gamma + 2.0 * am);
+        row[ROW_AP] = ap;
+        row[ROW_BETA] = beta;
+        double cp = 0.0;
+        for (int p = 0; p < KMAX; ++p) {
+            const double iv = 1.0 / (beta - ap * cp);
+            cp = ap * iv;
+            row[ROW_CP + p] = cp;
+            row[ROW_INVP + p] = iv;
+        }
+    }
+}
+
+int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, bool swizzle)
+{
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) {
+        h->err = "cuTensorMapEncodeTiled entry point not available";
+        return WAVE2D_ERR_CUDA;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)h->n1, (cuuint64_t)h->n2};
+    const cuuint64_t strides[1] = {(cuuint64_t)h->pitch * h->elem};
+    const cuuint32_t box[2] = {(cuuint32_t)box0, (cuuint32_t)box1};
+    const cuuint32_t es[2] = {1, 1};
+    CUresult r = enc(tm, h->dtype == WAVE2D_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                     base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char msg[160];
+        snprintf(msg, sizeof msg, "cuTensorMapEncodeTiled failed (%d) box=%dx%d n=%dx%d pitch=%lld", (int)r, box0, box1,
+                 h->n1, h->n2, h->pitch);
+        h->err = msg;
+        return WAVE2D_ERR_CUDA;
+    }
+    return WAVE2D_OK;
+}
+
+int plan_dir(wave2d_t* h, int d)
+{
+    DirPlan& P = h->plan[d];
+    P = DirPlan();
+    P.n = d == 0 ? h->n1 : h->n2;
+    P.nlines = d == 0 ? h->n2 : h->n1;
+    double rho = 0.0;
+    for (int n = d; n < 2 * h->M; n += 2) rho = std::max(rho, h->table[static_cast<size_t>(n) * ROW_DOUBLES + ROW_RHO]);
+    P.rho = rho;
+    const int U = 128 / h->elem;
+    const double tol = h->dtype == WAVE2D_F64 ? 1e-17 : 1e-8;   // rho^H <= tol: below half an ulp of T
+    int H = 1;
+    if (rho > 0.0) H = std::max(1, (int)std::ceil(std::log(tol) / std::log(rho)));
+    P.halo = H;
+    const int nbmax = h->dtype == WAVE2D_F64 ? NB_MAX_F64 : NB_MAX_F32;
+    const int nb = (H + U - 1) / U;
+    if (h->opt_solver == WAVE2D_SOLVER_EXACT || (h->opt_solver == WAVE2D_SOLVER_AUTO && nb > nbmax)) {
+        P.solver = WAVE2D_SOLVER_EXACT;
+        return WAVE2D_OK;
+    }
+    if (nb > nbmax) {
+        h->err = "streamed solver: decay bound rho^H <= tol needs more look-ahead than supported";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    P.solver = WAVE2D_SOLVER_STREAM;
+    P.nb = nb;
+    P.halo = nb * U;
+    P.shape = h->opt_shape[d];
+    P.var = find_variant(h->elem, d, nb, P.shape);
+    if (!P.var) {
+        h->err = "no kernel variant for this shape index";
+        return WAVE2D_ERR_ARG;
+    }
+    const Variant& V = *P.var;
+    W2D_CUDA(h, cudaFuncSetAttribute(V.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, V.smem));
+    int per_sm = 0;
+    W2D_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, V.fn, V.threads, V.smem));
+    if (per_sm < 1) {
+        h->err = "streamed kernel does not fit on an SM";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    P.ctas_per_sm = per_sm;
+    const int TL = 32 * V.nw;
+    P.ntiles = (P.nlines + TL - 1) / TL;
+    P.total_units = (P.n + U - 1) / U;
+    // One wave: as many chunks per line tile as resident CTA slots allow, but keep the halo (2 NB units of
+    // re-read per chunk) under ~25% of the chunk.
+    const int slots = per_sm * h->num_sms;
+    int q = std::max(1, slots / P.ntiles);
+    q = std::min(q, std::max(1, P.total_units / (8 * nb)));
+    if (h->opt_chunks[d] > 0) q = std::min(h->opt_chunks[d], std::max(1, P.total_units));
+    int upc = (P.total_units + q - 1) / q;
+    upc = (upc + V.xb - 1) / V.xb * V.xb;
+    P.upc = upc;
+    P.nchunks = (P.total_units + upc - 1) / upc;
+    P.grid = P.ntiles * P.nchunks;
+    return WAVE2D_OK;
+}
+
+int ensure_plan(wave2d_t* h)
+{
+    if (h->plan_ok) return WAVE2D_OK;
+    drop_graph(h);
+    build_table(h);
+    if (h->d_table) {
+        cudaFree(h->d_table);
+        h->device_bytes -= 0;   // accounted once below
+        h->d_table = nullptr;
+    }
+    const size_t tbytes = h->table.size() * sizeof(double);
+    if (tbytes > (size_t)1 << 30) {
+        h->err = "per-half-step table would exceed 1 GiB (M too large)";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    int st = dev_alloc(h, reinterpret_cast<void**>(&h->d_table), tbytes);
+    if (st) return st;
+    W2D_CUDA(h, cudaMemcpyAsync(h->d_table, h->table.data(), tbytes, cudaMemcpyHostToDevice, h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    for (int d = 0; d < 2; ++d) {
+        st = plan_dir(h, d);
+        if (st) return st;
+    }
+    const int U = 128 / h->elem;
+    for (int b = 0; b < 3; ++b) {
+        for (int d = 0; d < 2; ++d) {
+            if (h->plan[d].solver != WAVE2D_SOLVER_STREAM) continue;
+            const Variant& V = *h->plan[d].var;
+            const int TL = 32 * V.nw;
+            st = d == 0 ? make_tmap(h, &h->tm_load[0][b], h->buf[b], U, TL, true)
+                        : make_tmap(h, &h->tm_load[1][b], h->buf[b], TL, U * V.xb, false);
+            if (st) return st;
+        }
+        if (h->plan[0].solver == WAVE2D_SOLVER_STREAM) {
+            st = make_tmap(h, &h->tm_store[b], h->buf[b], U, 32, true);
+            if (st) return st;
+        }
+    }
+    if ((h->plan[0].solver == WAVE2D_SOLVER_EXACT || h->plan[1].solver == WAVE2D_SOLVER_EXACT) && !h->d_piv) {
+        st = dev_alloc(h, reinterpret_cast<void**>(&h->d_piv), sizeof(double) * 2 * (size_t)std::max(h->n1, h->n2));
+        if (st) return st;
+    }
+    h->plan_ok = true;
+    return WAVE2D_OK;
+}
+
+// One half-step n -> n+1.  With use_counter the kernels read the step count from d_k (graph replay) and
+// n_off is relative to it; otherwise n_off is the absolute half-step index.
+int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
+{
+    const int d = n_abs & 1;
+    const DirPlan& P = h->plan[d];
+    void* prev = h->buf[n_abs % 3];
+    void* cur = h->buf[(n_abs + 1) % 3];
+    void* out = h->buf[(n_abs + 2) % 3];
+    const int* dk = use_counter ? h->d_k : nullptr;
+    const void* src = h->have_src ? h->src_dev[d] : nullptr;
+    const int sl0 = d == 0 ? h->win_j0 : h->win_i0, snl = d == 0 ? h->win_h : h->win_w;
+    const int sp0 = d == 0 ? h->win_i0 : h->win_j0, snp = d == 0 ? h->win_w : h->win_h;
+    if (P.solver == WAVE2D_SOLVER_STREAM) {
+        SweepArgs a;
+        a.table = h->d_table; a.d_k = dk; a.n_off = n_off;
+        a.n = P.n; a.nlines = P.nlines; a.ntiles = P.ntiles; a.upc = P.upc; a.total_units = P.total_units;
+        a.out = out; a.pitch = h->pitch;
+        a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
+        a.g2 = 2.0 * h->gamma;
+        CUtensorMap* tp = &h->tm_load[d][n_abs % 3];
+        CUtensorMap* tc = &h->tm_load[d][(n_abs + 1) % 3];
+        CUtensorMap* to = &h->tm_store[(n_abs + 2) % 3];   // unused by the y sweep
+        void* args[4] = {tp, tc, to, &a};
+        W2D_CUDA(h, cudaLaunchKernel(P.var->fn, dim3(P.grid), dim3(P.var->threads), args, P.var->smem, h->stream));
+        h->launches += 1;
+        return WAVE2D_OK;
+    }
+    // exact two-pass Thomas
+    double* cpv = h->d_piv;
+    double* ivv = h->d_piv + std::max(h->n1, h->n2);
+    wave2d_exact_pivots<<<1, 256, 0, h->stream>>>(h->d_table, dk, n_off, P.n, cpv, ivv);
+    const int tb = 128, gb = (P.nlines + tb - 1) / tb;
+    const double g2 = 2.0 * h->gamma;
+#define W2D_EXACT(T, D)                                                                                               \
+    do {                                                                                                              \
+        wave2d_exact_forward<T, D><<<gb, tb, 0, h->stream>>>((const T*)prev, (const T*)cur, (T*)out, h->d_table, dk,  \
+                                                             n_off, P.n, P.nlines, h->pitch, cpv, ivv, (const T*)src, \
+                                                             sl0, snl, sp0, snp, g2);                                 \
+        wave2d_exact_backward<T, D><<<gb, tb, 0, h->stream>>>((T*)out, P.n, P.nlines, h->pitch, cpv);                 \
+    } while (0)
+    if (h->dtype == WAVE2D_F64) {
+        if (d == 0) W2D_EXACT(double, 0); else W2D_EXACT(double, 1);
+    } else {
+        if (d == 0) W2D_EXACT(float, 0); else W2D_EXACT(float, 1);
+    }
+#undef W2D_EXACT
+    W2D_CUDA(h, cudaGetLastError());
+    h->launches += 3;
+    return WAVE2D_OK;
+}
+
+int build_graph(wave2d_t* h, int steps)
+{
+    drop_graph(h);
+    cudaGraph_t g = nullptr;
+    W2D_CUDA(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+    const long long l0 = h->launches;
+    int st = WAVE2D_OK;
+    for (int s = 0; s < steps && st == WAVE2D_OK; ++s) {
+        st = launch_half_step(h, 2 * s, 2 * s, true);
+        if (st == WAVE2D_OK) st = launch_half_step(h, 2 * s + 1, 2 * s + 1, true);
+    }
+    if (st == WAVE2D_OK) wave2d_bump_counter<<<1, 1, 0, h->stream>>>(h->d_k, steps);
+    h->launches = l0;   // capture is not execution
+    cudaError_t e = cudaStreamEndCapture(h->stream, &g);
+    if (st != WAVE2D_OK) {
+        if (g) cudaGraphDestroy(g);
+        return st;
+    }
+    if (e != cudaSuccess) {
+        h->err = std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e);
+        (void)cudaGetLastError();
+        return WAVE2D_ERR_CUDA;
+    }
+    e = cudaGraphInstantiate(&h->gexec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) {
+        h->gexec = nullptr;
+        h->err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e);
+        (void)cudaGetLastError();
+        return WAVE2D_ERR_CUDA;
+    }
+    h->gexec_steps = steps;
+    return WAVE2D_OK;
+}
+
+long long launches_per_step(const wave2d_t* h)
+{
+    long long n = 0;
+    for (int d = 0; d < 2; ++d) n += h->plan[d].solver == WAVE2D_SOLVER_STREAM ? 1 : 3;
+    return n;
+}
+
+bool is_device_ptr(const void* p)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int copy_in(wave2d_t* h, void* dst, const void* src, long ld)
+{
+    W2D_CUDA(h, cudaMemcpy2DAsync(dst, (size_t)h->pitch * h->elem, src, (size_t)ld * h->elem, (size_t)h->n1 * h->elem,
+                                  h->n2, cudaMemcpyDefault, h->stream));
+    return WAVE2D_OK;
+}
+
+int copy_out(wave2d_t* h, void* dst, long ld, const void* src)
+{
+    if (!h || !dst || ld < h->n1) return WAVE2D_ERR_ARG;
+    if (!h->have_initial) return WAVE2D_ERR_STATE;
+    W2D_CUDA(h, cudaMemcpy2DAsync(dst, (size_t)ld * h->elem, src, (size_t)h->pitch * h->elem, (size_t)h->n1 * h->elem,
+                                  h->n2, cudaMemcpyDefault, h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WAVE2D_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" {
+
+int wave2d_create(wave2d_t** out, int N1, int N2, double l, double tau, int M, int dtype)
+{
+    if (!out) return WAVE2D_ERR_ARG;
+    *out = nullptr;
+    if (N1 < 2 || N2 < 2 || !(l > 0.0) || !(tau > 0.0) || M < 0 || (dtype != WAVE2D_F64 && dtype != WAVE2D_F32))
+        return WAVE2D_ERR_ARG;
+    wave2d_t* h = new (std::nothrow) wave2d_t();
+    if (!h) return WAVE2D_ERR_ALLOC;
+    h->N1 = N1; h->N2 = N2; h->n1 = N1 - 1; h->n2 = N2 - 1; h->M = M; h->dtype = dtype;
+    h->elem = dtype == WAVE2D_F64 ? 8 : 4;
+    h->l = l; h->tau = tau;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess || prop.major != 10) {
+        (void)cudaGetLastError();
+        delete h;
+        return WAVE2D_ERR_CUDA;   // no device, or not an sm_100-class device: there is no other code path
+    }
+    h->num_sms = prop.multiProcessorCount;
+    if (cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        (void)cudaGetLastError();
+        delete h;
+        return WAVE2D_ERR_CUDA;
+    }
+    h->stream = h->own_stream;
+    const int per128 = 128 / h->elem;
+    h->pitch = ((long long)h->n1 + per128 - 1) / per128 * per128;     // rows start 128-byte aligned (H5)
+    const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
+    int st = WAVE2D_OK;
+    for (int b = 0; b < 3 && st == WAVE2D_OK; ++b) st = dev_alloc(h, &h->buf[b], fbytes);
+    if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_k), sizeof(int));
+    if (st == WAVE2D_OK) {
+        for (int b = 0; b < 3; ++b) cudaMemsetAsync(h->buf[b], 0, fbytes, h->stream);
+        cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream);
+        if (cudaStreamSynchronize(h->stream) != cudaSuccess) st = WAVE2D_ERR_CUDA;
+    }
+    if (st != WAVE2D_OK) {
+        (void)cudaGetLastError();
+        wave2d_destroy(h);
+        return st;
+    }
+    h->c_half.assign((size_t)2 * M + 1, 1.0);
+    *out = h;
+    return WAVE2D_OK;
+}
+
+void wave2d_destroy(wave2d_t* h)
+{
+    if (!h) return;
+    if (h->stream) cudaStreamSynchronize(h->stream);
+    drop_graph(h);
+    for (int b = 0; b < 3; ++b) cudaFree(h->buf[b]);
+    cudaFree(h->src_dev[0]);
+    cudaFree(h->src_dev[1]);
+    cudaFree(h->d_table);
+    cudaFree(h->d_k);
+    cudaFree(h->d_piv);
+    if (h->own_stream) cudaStreamDestroy(h->own_stream);
+    (void)cudaGetLastError();
+    delete h;
+}
+
+int wave2d_set_stream(wave2d_t* h, void* cuda_stream)
+{
+    if (!h) return WAVE2D_ERR_ARG;
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->stream = cuda_stream ? static_cast<cudaStream_t>(cuda_stream) : h->own_stream;
+    drop_graph(h);
+    return WAVE2D_OK;
+}
+
+int wave2d_set_option(wave2d_t* h, const char* name, double value)
+{
+    if (!h || !name) return WAVE2D_ERR_ARG;
+    if (h->ran) return WAVE2D_ERR_STATE;
+    const int iv = (int)value;
+    if (!strcmp(name, "gamma")) { if (!(value > 0.0)) return WAVE2D_ERR_ARG; h->gamma = value; }
+    else if (!strcmp(name, "kappa")) h->kappa = value;
+    else if (!strcmp(name, "solver")) { if (iv < 0 || iv > 2) return WAVE2D_ERR_ARG; h->opt_solver = iv; }
+    else if (!strcmp(name, "graph")) h->opt_graph = iv != 0;
+    else if (!strcmp(name, "graph_steps")) { if (iv < 3 || iv % 3) return WAVE2D_ERR_ARG; h->opt_graph_steps = iv; }
+    else if (!strcmp(name, "shape_x")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[0] = iv; }
+    else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
+    else if (!strcmp(name, "chunks_x")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_chunks[0] = iv; }
+    else if (!strcmp(name, "chunks_y")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_chunks[1] = iv; }
+    else return WAVE2D_ERR_ARG;
+    invalidate_plan(h);
+    return WAVE2D_OK;
+}
+
+int wave2d_set_initial(wave2d_t* h, const void* phi, const void* psi, long ld)
+{
+    if (!h || !phi || ld < h->n1) return WAVE2D_ERR_ARG;
+    // w_0 = phi -> buf[1]; psi staged in buf[2]; w_{-1} = phi - (tau/2) psi -> buf[0]   (roles of half-step 0)
+    int st = copy_in(h, h->buf[1], phi, ld);
+    if (st) return st;
+    if (psi) {
+        st = copy_in(h, h->buf[2], psi, ld);
+        if (st) return st;
+    }
+    const dim3 blk(128), grd((h->n1 + 127) / 128, h->n2);
+    if (h->dtype == WAVE2D_F64)
+        wave2d_init_prev<double><<<grd, blk, 0, h->stream>>>((double*)h->buf[0], (const double*)h->buf[1],
+                                                             psi ? (const double*)h->buf[2] : nullptr, h->n1, h->n2,
+                                                             h->pitch, 0.5 * h->tau);
+    else
+        wave2d_init_prev<float><<<grd, blk, 0, h->stream>>>((float*)h->buf[0], (const float*)h->buf[1],
+                                                            psi ? (const float*)h->buf[2] : nullptr, h->n1, h->n2,
+                                                            h->pitch, 0.5 * h->tau);
+    W2D_CUDA(h, cudaGetLastError());
+    W2D_CUDA(h, cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->have_initial = true;
+    h->k = 0;
+    h->ran = false;
+    return WAVE2D_OK;
+}
+
+int wave2d_set_speed(wave2d_t* h, const double* c_half, int count)
+{
+    if (!h || !c_half || (count != 1 && count != 2 * h->M + 1)) return WAVE2D_ERR_ARG;
+    if (h->ran) return WAVE2D_ERR_STATE;
+    for (int n = 0; n < count; ++n)
+        if (!(c_half[n] > 0.0)) return WAVE2D_ERR_ARG;   // PAPER.md:31, "positive speed function"
+    for (int n = 0; n <= 2 * h->M; ++n) h->c_half[n] = count == 1 ? c_half[0] : c_half[n];
+    invalidate_plan(h);
+    return WAVE2D_OK;
+}
+
+int wave2d_set_source(wave2d_t* h, const void* s, long ld, const double* g_half, int count)
+{
+    if (!h) return WAVE2D_ERR_ARG;
+    if (h->ran) return WAVE2D_ERR_STATE;
+    if (s && (ld < h->n1 || (g_half && count < 2 * h->M))) return WAVE2D_ERR_ARG;
+    for (int d = 0; d < 2; ++d) {
+        cudaFree(h->src_dev[d]);
+        h->src_dev[d] = nullptr;
+    }
+    h->have_src = false;
+    h->g_half.clear();
+    invalidate_plan(h);
+    if (!s) return WAVE2D_OK;
+    // Bring s to the host once, find the window of non-zero values (config 3's sigma = 2h Gaussian underflows to
+    // exactly 0 outside ~155^2 points) and keep only that window on the device, in both orientations.
+    const size_t e = h->elem, n1 = h->n1, n2 = h->n2;
+    std::vector<unsigned char> host(n1 * n2 * e);
+    W2D_CUDA(h, cudaMemcpy2D(host.data(), n1 * e, s, (size_t)ld * e, n1 * e, n2, cudaMemcpyDefault));
+    auto nz = [&](size_t j, size_t i) {
+        return h->dtype == WAVE2D_F64 ? reinterpret_cast<const double*>(host.data())[j * n1 + i] != 0.0
+                                      : reinterpret_cast<const float*>(host.data())[j * n1 + i] != 0.0f;
+    };
+    long i0 = n1, i1 = -1, j0 = n2, j1 = -1;
+    for (size_t j = 0; j < n2; ++j)
+        for (size_t i = 0; i < n1; ++i)
+            if (nz(j, i)) {
+                i0 = std::min<long>(i0, i); i1 = std::max<long>(i1, i);
+                j0 = std::min<long>(j0, j); j1 = std::max<long>(j1, j);
+            }
+    if (i1 < 0) return WAVE2D_OK;   // identically zero: no source
+    const size_t w = i1 - i0 + 1, hh = j1 - j0 + 1;
+    std::vector<unsigned char> nat(w * hh * e), tr(w * hh * e);
+    for (size_t j = 0; j < hh; ++j)
+        for (size_t i = 0; i < w; ++i) {
+            const unsigned char* src = host.data() + ((j0 + j) * n1 + (i0 + i)) * e;
+            memcpy(nat.data() + (j * w + i) * e, src, e);
+            memcpy(tr.data() + (i * hh + j) * e, src, e);
+        }
+    int st = dev_alloc(h, &h->src_dev[0], w * hh * e);
+    if (st == WAVE2D_OK) st = dev_alloc(h, &h->src_dev[1], w * hh * e);
+    if (st) return st;
+    W2D_CUDA(h, cudaMemcpy(h->src_dev[0], tr.data(), w * hh * e, cudaMemcpyHostToDevice));
+    W2D_CUDA(h, cudaMemcpy(h->src_dev[1], nat.data(), w * hh * e, cudaMemcpyHostToDevice));
+    h->win_i0 = (int)i0; h->win_j0 = (int)j0; h->win_w = (int)w; h->win_h = (int)hh;
+    h->have_src = true;
+    if (g_half) h->g_half.assign(g_half, g_half + 2 * h->M);
+    return WAVE2D_OK;
+}
+
+int wave2d_run(wave2d_t* h, int steps)
+{
+    if (!h || steps < 0) return WAVE2D_ERR_ARG;
+    if (!h->have_initial) return WAVE2D_ERR_STATE;
+    if ((long long)h->k + steps > h->M) return WAVE2D_ERR_RANGE;
+    int st = ensure_plan(h);
+    if (st) return st;
+    if (steps > 0) h->ran = true;
+    const bool can_graph = h->opt_graph && h->stream != nullptr && h->stream != cudaStreamLegacy &&
+                           h->stream != cudaStreamPerThread;
+    int left = steps;
+    bool counter_set = false;
+    while (left > 0) {
+        const int gs = h->opt_graph_steps;
+        if (can_graph && h->k % 3 == 0 && left >= gs) {
+            if (!h->gexec || h->gexec_steps != gs) {
+                st = build_graph(h, gs);
+                if (st) return st;
+            }
+            if (!counter_set) {
+                W2D_CUDA(h, cudaMemcpyAsync(h->d_k, &h->k, sizeof(int), cudaMemcpyHostToDevice, h->stream));
+                counter_set = true;
+            }
+            W2D_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
+            h->launches += launches_per_step(h) * gs + 1;
+            h->k += gs;
+            left -= gs;
+        } else {
+            st = launch_half_step(h, 2 * h->k, 2 * h->k, false);
+            if (st == WAVE2D_OK) st = launch_half_step(h, 2 * h->k + 1, 2 * h->k + 1, false);
+            if (st) return st;
+            h->k += 1;
+            left -= 1;
+            counter_set = false;
+        }
+    }
+    return WAVE2D_OK;
+}
+
+int wave2d_get(wave2d_t* h, void* u_out, long ld)
+{
+    if (!h) return WAVE2D_ERR_ARG;
+    return copy_out(h, u_out, ld, h->buf[(2 * h->k + 1) % 3]);
+}
+
+int wave2d_get_prev(wave2d_t* h, void* u_out, long ld)
+{
+    if (!h) return WAVE2D_ERR_ARG;
+    return copy_out(h, u_out, ld, h->buf[(2 * h->k) % 3]);
+}
+
+int wave2d_steps_done(const wave2d_t* h, int* k)
+{
+    if (!h || !k) return WAVE2D_ERR_ARG;
+    *k = h->k;
+    return WAVE2D_OK;
+}
+
+int wave2d_sync(wave2d_t* h)
+{
+    if (!h) return WAVE2D_ERR_ARG;
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WAVE2D_OK;
+}
+
+int wave2d_get_info(wave2d_t* h, const char* name, double* value)
+{
+    if (!h || !name || !value) return WAVE2D_ERR_ARG;
+    if (!strcmp(name, "pitch")) { *value = (double)h->pitch; return WAVE2D_OK; }
+    if (!strcmp(name, "device_bytes")) { *value = (double)h->device_bytes; return WAVE2D_OK; }
+    if (!strcmp(name, "launches")) { *value = (double)h->launches; return WAVE2D_OK; }
+    if (!strcmp(name, "source_window")) { *value = h->have_src ? (double)h->win_w * h->win_h : 0.0; return WAVE2D_OK; }
+    int st = ensure_plan(h);
+    if (st) return st;
+    const size_t len = strlen(name);
+    if (len < 3 || name[len - 2] != '_' || (name[len - 1] != 'x' && name[len - 1] != 'y')) return WAVE2D_ERR_ARG;
+    const DirPlan& P = h->plan[name[len - 1] == 'y'];
+    const std::string key(name, len - 2);
+    const bool stream = P.solver == WAVE2D_SOLVER_STREAM;
+    if (key == "solver") *value = P.solver;
+    else if (key == "halo") *value = P.halo;
+    else if (key == "rho") *value = P.rho;
+    else if (key == "chunks") *value = stream ? P.nchunks : 1;
+    else if (key == "grid") *value = stream ? P.grid : (P.nlines + 127) / 128;
+    else if (key == "ctas_per_sm") *value = stream ? P.ctas_per_sm : 0;
+    else if (key == "smem") *value = stream ? P.var->smem : 0;
+    else if (key == "threads") *value = stream ? P.var->threads : 128;
+    else if (key == "unit") *value = 128 / h->elem;
+    else if (key == "upc") *value = stream ? P.upc : 0;
+    else return WAVE2D_ERR_ARG;
+    return WAVE2D_OK;
+}
+
+int wave2d_profile_sweeps(wave2d_t* h, int steps, double* ms_x, double* ms_y)
+{
+    if (!h || steps < 1 || !ms_x || !ms_y) return WAVE2D_ERR_ARG;
+    if (!h->have_initial) return WAVE2D_ERR_STATE;
+    if ((long long)h->k + steps > h->M) return WAVE2D_ERR_RANGE;
+    int st = ensure_plan(h);
+    if (st) return st;
+    h->ran = true;
+    std::vector<cudaEvent_t> ev((size_t)3 * steps);
+    for (auto& e : ev) W2D_CUDA(h, cudaEventCreate(&e));
+    for (int s = 0; s < steps; ++s) {
+        W2D_CUDA(h, cudaEventRecord(ev[3 * s], h->stream));
+        st = launch_half_step(h, 2 * h->k, 2 * h->k, false);
+        if (st) return st;
+        W2D_CUDA(h, cudaEventRecord(ev[3 * s + 1], h->stream));
+        st = launch_half_step(h, 2 * h->k + 1, 2 * h->k + 1, false);
+        if (st) return st;
+        W2D_CUDA(h, cudaEventRecord(ev[3 * s + 2], h->stream));
+        h->k += 1;
+    }
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    double sx = 0.0, sy = 0.0;
+    for (int s = 0; s < steps; ++s) {
+        float a = 0.f, b = 0.f;
+        W2D_CUDA(h, cudaEventElapsedTime(&a, ev[3 * s], ev[3 * s + 1]));
+        W2D_CUDA(h, cudaEventElapsedTime(&b, ev[3 * s + 1], ev[3 * s + 2]));
+        sx += a;
+        sy += b;
+    }
+    for (auto& e : ev) cudaEventDestroy(e);
+    *ms_x = sx / steps;
+    *ms_y = sy / steps;
+    return WAVE2D_OK;
+}
+
+const char* wave2d_strerror(int status)
+{
+    switch (status) {
+        case WAVE2D_OK: return "ok";
+        case WAVE2D_ERR_ARG: return "invalid argument";
+        case WAVE2D_ERR_STATE: return "call not allowed in this state";
+        case WAVE2D_ERR_ALLOC: return "allocation failed";
+        case WAVE2D_ERR_CUDA: return "CUDA error";
+        case WAVE2D_ERR_UNSUPPORTED: return "unsupported size or option";
+        case WAVE2D_ERR_RANGE: return "more than M steps requested";
+        default: return "unknown status";
+    }
+}
+
+const char* wave2d_last_error(const wave2d_t* h) { return h ? h->err.c_str() : ""; }
+
+}  // extern "C"
