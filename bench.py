@@ -1,0 +1,417 @@
+#!/usr/bin/env python
+"""bench.py -- ADI step throughput of the wave2d hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|cfg4_f64|cfg4_f32|cfg5|cfg1]
+                    [--impl ours|reference] [--no-cpu-baseline]
+
+A "step" is one ADI time step of the whole hot path (fused RHS + x-sweep solve,
+fused RHS + y-sweep solve, level rotation) over the whole grid of the workload.  The default workload is
+config 3 of BASELINE.json (fp64 4096^2, the one the north_star's roofline target is quoted on); it fits
+one GPU (0.4 GB).  Its three fields (403 MB) exceed the 126 MB L2, and every sweep streams 2 fields in
+and 1 out, so successive timed steps cannot reuse L2 contents ("inputs larger than L2").
+
+Prints ONE JSON line (rank 0).  Keys follow the graft bench contract; `roofline` is the dominant kernel
+(the slower of the two sweep kernels) timed live with CUDA events on the launching stream through
+wave2d_profile_sweeps; `cpu_baseline` is the oracle as it stands on the host cores on a bounded sample;
+`e2e` is the same metric through the public API with HOST buffers (H2D of phi and D2H of u inside the
+timed region, every iteration).
+
+Multi-GPU: the path does not shard without an exchange: "replicas only".  Under torchrun
+every rank runs an independent replica of the workload on its own GPU; value = total point-updates of all
+ranks / max-over-ranks device time; no data-path collective.
+
+--impl reference: the reference arm of this tier is the CPU oracle (oracle/), timed as it stands on the
+host cores on a bounded sample of the same workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ADI step throughput (Gpoint-updates/s) fp64; achieved HBM GB/s vs peak"
+UNIT = "Gpoint-updates/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=960)
+    ap.add_argument("--warmup", type=int, default=24)
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="steps per end-to-end iteration (default: --steps)")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc, self.ok = index, [], None, True
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i",
+                 str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.t = threading.Thread(target=self._read, daemon=True)
+        self.t.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self, t0=None, t1=None):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.t.join(timeout=2)
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def load_workload(name: str, steps_needed: int):
+    from paper_2006_10142_b200 import workloads as W
+    w = W.by_name(name)
+    if steps_needed > w.M:   # more timed steps than the config's M: extend the time axis with the same recipe
+        w = W.by_name(name, M=steps_needed)
+    return w
+
+
+class NvmlSampler:
+    """SM clock + throttle reasons sampled every 5 ms through NVML while the timed region runs."""
+
+    def __init__(self, torch_index: int):
+        self.rows, self.stop_flag, self.ok = [], False, False
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            uuid = str(torch.cuda.get_device_properties(torch_index).uuid)
+            if not uuid.startswith("GPU-"):
+                uuid = "GPU-" + uuid
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(torch_index)
+            self.nv = pynvml
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:   # noqa: BLE001
+            self.err = repr(e)
+
+    def start(self):
+        if not self.ok:
+            return
+        self.t = threading.Thread(target=self._loop, daemon=True)
+        self.t.start()
+
+    def _loop(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                self.rows.append((time.perf_counter(), float(mhz), int(rs), pw))
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def stop(self, t0=None, t1=None):
+        if not self.ok:
+            return None
+        self.stop_flag = True
+        self.t.join(timeout=2)
+        nv = self.nv
+        rows = [r for r in self.rows if (t0 is None or r[0] >= t0) and (t1 is None or r[0] <= t1)] or self.rows
+        bits = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        reasons = sorted(n for n, b in bits.items() if any(r[2] & b for r in rows))
+        return {"sm_mhz": float(np.median([r[1] for r in rows])) if rows else None, "sm_max_mhz": self.max_mhz,
+                "power_w_max": max((r[3] for r in rows), default=None), "samples": len(rows), "reasons": reasons}
+
+
+def field_bytes(w):
+    return w.points * (8 if w.dtype == "f64" else 4)
+
+
+def time_oracle(w, budget_s: float, min_steps: int = 2):
+    """The oracle as it stands on the host cores: first `steps` time steps of workload w (full grid)."""
+    from oracle import oracle
+    o = oracle.Wave2DOracle(w.N1, w.N2, w.l, w.tau, w.M)
+    try:
+        o.set_speed(w.c_half)
+        if w.s is not None:
+            o.set_source(w.s, w.g_half)
+        o.set_initial(w.phi, w.psi)
+        t0 = time.perf_counter()
+        o.run(1)
+        t1 = time.perf_counter() - t0
+        steps = int(max(min_steps, min(w.M - 1, budget_s / max(t1, 1e-6))))
+        t0 = time.perf_counter()
+        o.run(steps)
+        dt = time.perf_counter() - t0
+    finally:
+        o.close()
+    return {"value": w.points * steps / dt / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{steps} time steps of {w.name} on the full {w.n1}x{w.n2} grid after 1 untimed step "
+                      f"({dt:.1f} s, oracle/wave2d_oracle.c: Thomas per line, OpenMP over lines, fp64)",
+            "seconds": dt, "steps": steps}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def run_reference(args):
+    """Reference arm of this tier: the CPU oracle, K timed steps after W warm-up steps, rank 0 only."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    from oracle import oracle
+    oracle.build()
+    K, Wm = args.steps, args.warmup
+    w = load_workload(args.workload, K + Wm + 1)
+    # bounded sample: one calibration step on the full grid; if W+K full-grid steps would take more than
+    # ~150 s, the sample is the same recipe on a grid with fewer rows (N2 reduced), stated in `sample`.
+    o = oracle.Wave2DOracle(w.N1, w.N2, w.l, w.tau, w.M)
+    o.set_speed(w.c_half)
+    if w.s is not None:
+        o.set_source(w.s, w.g_half)
+    o.set_initial(w.phi, w.psi)
+    t0 = time.perf_counter(); o.run(1); t1 = time.perf_counter() - t0
+    o.close()
+    N2 = w.N2
+    est = t1 * (K + Wm)
+    if est > 150.0:
+        N2 = max(64, int(w.N2 * 150.0 / est) // 64 * 64)
+    rows = N2 - 1
+    phi = np.ascontiguousarray(w.phi[:rows])
+    s = None if w.s is None else np.ascontiguousarray(w.s[:rows])
+    o = oracle.Wave2DOracle(w.N1, N2, w.l * 1.0, w.tau, w.M)
+    # keep h2 = l/N2 of the full workload: the strip is [0,l] x [0, l*N2/N2_full]; the oracle takes one l,
+    # so the strip uses its own h2 -- only the arithmetic cost per point matters for this timing.
+    o.set_speed(w.c_half)
+    if s is not None:
+        o.set_source(s, w.g_half)
+    o.set_initial(phi, None)
+    o.run(Wm)
+    t0 = time.perf_counter()
+    o.run(K)
+    dt = time.perf_counter() - t0
+    o.close()
+    pts = (w.N1 - 1) * rows
+    value = pts * K / dt / 1e9
+    sample = (f"{K} timed steps (after {Wm}) of {w.name} on " +
+              (f"the full {w.n1}x{w.n2} grid" if N2 == w.N2 else
+               f"a {w.n1}x{rows} strip of its {w.n1}x{w.n2} grid (full grid would take ~{est:.0f} s)"))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+            "warmup": Wm, "ms_per_step": dt / K * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N1": w.N1, "N2": w.N2, "tau": w.tau, "sample_points": pts},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path is CUDA only, there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    from paper_2006_10142_b200 import binding as B
+    K, Wm = args.steps, args.warmup
+    PROF = 12                                             # per-kernel timing pass (plain launches + events)
+    w = load_workload(args.workload, Wm + K + PROF)
+    npdt = np.float64 if w.dtype == "f64" else np.float32
+    esz = 8 if w.dtype == "f64" else 4
+    fbytes = field_bytes(w)
+
+    # pinned host buffers (the e2e leg copies from / to these every iteration)
+    phi_pin = torch.empty((w.n2, w.n1), dtype=torch.float64 if esz == 8 else torch.float32).pin_memory()
+    phi_pin.numpy()[...] = w.phi.astype(npdt, copy=False)
+    out_pin = torch.empty_like(phi_pin).pin_memory()
+
+    stream = torch.cuda.Stream()
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+    h.set_stream(stream)
+    h.set_speed(w.c_half)
+    if w.s is not None:
+        h.set_source(w.s.astype(npdt, copy=False), w.g_half)
+    h.set_initial(phi_pin)
+
+    sampler = NvmlSampler(local)
+    if not sampler.ok:
+        sampler = ClockSampler(local)   # nvidia-smi fallback (coarser: 100 ms)
+    sampler.start()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between two events on the stream
+    h.run(Wm)
+    h.sync()
+    l0 = h.info("launches")
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    tw0 = time.perf_counter()
+    ev0.record(stream)
+    h.run(K)
+    ev1.record(stream)
+    h.sync()
+    barrier()
+    tw1 = time.perf_counter()
+    ms = max_over_ranks(float(ev0.elapsed_time(ev1)))
+    launches = int(h.info("launches") - l0)
+    clocks = sampler.stop(tw0, tw1) or {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable"]}
+
+    # ---- per-kernel timing of the two sweep kernels, live, CUDA events on the same stream
+    ms_x, ms_y = h.profile_sweeps(PROF)
+    geom = {k: h.info(k) for k in ("solver_x", "solver_y", "halo_x", "halo_y", "chunks_x", "chunks_y", "grid_x",
+                                   "grid_y", "ctas_per_sm_x", "ctas_per_sm_y", "threads_x", "threads_y",
+                                   "smem_x", "smem_y")}
+
+    # ---- end to end through the public API with HOST buffers: H2D(phi) + K steps + D2H(u) per iteration
+    Ke = args.e2e_steps or K
+    e2e_iters = 3
+    h.set_initial(phi_pin); h.run(min(Ke, 12)); h.get(out_pin)          # warm the path once
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_iters):
+        h.set_initial(phi_pin)        # pinned host -> device (u^0 and u^{-1/2})
+        h.run(Ke)
+        h.get(out_pin)                # device -> pinned host, synchronises
+    barrier()
+    e2e_s = max_over_ranks((time.perf_counter() - t0) / e2e_iters)
+    h.close()
+
+    peak, peak_src = measured_peaks()
+    pts = w.points
+    value = world * pts * K / (ms * 1e-3) / 1e9
+    dom = "x" if ms_x >= ms_y else "y"
+    ms_dom = max(ms_x, ms_y)
+    sweep_bytes = 3 * fbytes                                           # read 2 fields, write 1
+    achieved = sweep_bytes / (ms_dom * 1e-3) / 1e9
+    step_s = ms * 1e-3 / K
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": w.dtype, "data": "synthetic",
+        "config": {"workload": w.name, "N1": w.N1, "N2": w.N2, "unknowns": [w.n1, w.n2], "tau": w.tau, "M": w.M,
+                   "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
+                   "l2": (f"working set {3 * fbytes / 1e6:.0f} MB (3 fields) "
+                          + ("> 126 MB L2: inputs larger than L2, no flush needed" if 3 * fbytes > 126e6 * 1.5
+                             else "fits the 126 MB L2: L2-resident, HBM fraction not meaningful")),
+                   "geometry": geom},
+        "clocks": clocks,
+        "gpu_launches": launches,
+        "e2e": {"value": world * pts * Ke / e2e_s / 1e9, "unit": UNIT,
+                "h2d_bytes_per_step": fbytes / Ke, "d2h_bytes_per_step": fbytes / Ke,
+                "steps_per_call": Ke, "seconds_per_call": e2e_s,
+                "what": "wave2d_set_initial(pinned host phi) + wave2d_run(steps_per_call) + wave2d_get(pinned host u), "
+                        "wall clock incl. both copies; bytes are per call / steps_per_call"},
+        "roofline": {"bound": "hbm", "kernel": f"wave2d_sweep_stream<{w.dtype}, dir={dom}>", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "bytes_per_launch": sweep_bytes,
+                     "ms_per_launch": ms_dom, "ms_x": ms_x, "ms_y": ms_y,
+                     "gbs_x": sweep_bytes / ms_x / 1e6, "gbs_y": sweep_bytes / ms_y / 1e6,
+                     "frac_x": sweep_bytes / ms_x / 1e6 / peak, "frac_y": sweep_bytes / ms_y / 1e6 / peak,
+                     "step_frac6": 6 * fbytes / step_s / 1e9 / peak, "step_frac5": 5 * fbytes / step_s / 1e9 / peak},
+    }
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):   # dram bytes per launch from the committed ncu --set full capture
+        try:
+            t = json.load(open(traffic_file)).get(f"{w.name}:{dom}")
+            if t:
+                line["roofline"]["traffic"] = t
+        except Exception:
+            pass
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            from oracle import oracle
+            oracle.build()
+            line["cpu_baseline"] = time_oracle(w, budget_s=15.0)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

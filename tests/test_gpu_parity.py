@@ -1,0 +1,262 @@
+"""Parity of the CUDA path (through the C ABI, include/wave2d.h) against the CPU oracle -- `-m gpu`.
+
+Tolerances are BASELINE.json's north_star: max|u_gpu - u_oracle| <= 1e-10 * max|u_oracle| after all M
+steps in fp64, 1e-4 in the fp32 variant.  Every input is seeded and synthetic
+(paper_2006_10142_b200/workloads.py); the same bytes go to both sides.  Nothing here reads /root/reference.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle
+from paper_2006_10142_b200 import binding as B
+from paper_2006_10142_b200 import workloads as W
+from tests.modal import modal_amplitudes
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-10, "f32": 1e-4}
+
+
+def ref(w, steps=None, gamma=None, kappa=None):
+    return oracle.solve(w.N1, w.N2, w.l, w.tau, w.M, w.phi, w.psi, c_half=w.c_half, s=w.s, g_half=w.g_half,
+                        steps=steps, gamma=gamma, kappa=kappa)
+
+
+def gpu(w, steps=None, **opts):
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+    try:
+        for k, v in opts.items():
+            h.set_option(k, v)
+        npdt = np.float64 if w.dtype == "f64" else np.float32
+        h.set_speed(w.c_half)
+        if w.s is not None:
+            h.set_source(w.s.astype(npdt), w.g_half)
+        h.set_initial(w.phi.astype(npdt), None if w.psi is None else w.psi.astype(npdt))
+        h.run(w.M if steps is None else steps)
+        u = h.get()
+        info = {k: h.info(k) for k in ("solver_x", "solver_y", "launches", "chunks_x", "chunks_y")}
+    finally:
+        h.close()
+    return u, info
+
+
+def relerr(u, r):
+    return float(np.abs(u.astype(np.float64) - r).max() / max(np.abs(r).max(), 1e-300))
+
+
+def small_cases():
+    return [
+        ("cfg1", W.cfg1()),
+        ("cfg2_N96", W.cfg2(N=96, M=40)),
+        ("cfg2_N700", W.cfg2(N=700, M=50)),            # several line tiles, ragged tail in both directions
+        ("cfg3_N128", W.cfg3(N=128, M=60)),
+        ("cfg3_N1000", W.cfg3(N=1000, M=260)),         # source switched on (Ricker centre at step ~245)
+        ("cfg4_160x40", W.cfg4(N1=160, N2=40, M=30)),
+        ("cfg4_1030x270", W.cfg4(N1=1030, N2=270, M=24)),
+        ("cfg4_160x40_f32", W.cfg4(N1=160, N2=40, M=30, dtype="f32")),
+        ("cfg4_1030x270_f32", W.cfg4(N1=1030, N2=270, M=200, dtype="f32")),
+        ("cfg5_N192", W.cfg5(N=192, M=20)),
+    ]
+
+
+@pytest.mark.parametrize("name,w", small_cases(), ids=[c[0] for c in small_cases()])
+@pytest.mark.parametrize("opts", [{}, {"solver": B.SOLVER_EXACT}, {"graph": 0}, {"chunks_x": 3, "chunks_y": 2},
+                                  {"shape_x": 2, "shape_y": 3}],
+                         ids=["default", "exact", "nograph", "chunks", "shapes"])
+def test_small_workloads_match_oracle(name, w, opts):
+    r = ref(w)
+    u, info = gpu(w, **opts)
+    assert np.isfinite(u).all()
+    assert relerr(u, r) <= TOL[w.dtype]
+    assert info["launches"] >= 2 * w.M          # the CUDA kernels ran: >= 2 sweeps per step
+    if opts.get("solver") == B.SOLVER_EXACT:
+        assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
+    elif "solver" not in opts:
+        assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
+
+
+@pytest.mark.parametrize("N1,N2", [(2, 2), (2, 9), (9, 2), (3, 3), (4, 5), (16, 17), (17, 16), (18, 33), (33, 18),
+                                   (127, 129), (129, 127), (128, 128), (130, 66), (257, 40)])
+def test_tiny_and_ragged_sizes(N1, N2):
+    """n = 1, 2, 3 unknowns per line, sizes straddling one 16-point unit / one 32-line tile."""
+    rng = np.random.default_rng(1000 * N1 + N2)
+    M = 7
+    tau = 0.9 / max(N1, N2)
+    phi = rng.uniform(-1, 1, (N2 - 1, N1 - 1))
+    psi = rng.uniform(-1, 1, (N2 - 1, N1 - 1))
+    s = rng.uniform(-1, 1, (N2 - 1, N1 - 1))
+    c = rng.uniform(0.5, 1.5, 2 * M + 1)
+    g = rng.uniform(-1, 1, 2 * M)
+    w = W.Workload("rand", N1, N2, 1.0, tau, M, "f64", phi, psi, c, s=s, g_half=g)
+    r = ref(w)
+    for opts in ({}, {"solver": B.SOLVER_EXACT}):
+        u, _ = gpu(w, **opts)
+        assert relerr(u, r) <= 1e-12, (opts, relerr(u, r))
+
+
+def test_literal_constants_gamma1_kappa1():
+    """The scheme exactly as printed: gamma = kappa = 1 (reading A2)."""
+    w = W.cfg3(N=200, M=30)
+    w.phi = W.cfg2(N=200, M=30).phi
+    w.g_half = np.cos(np.arange(2 * w.M) * 0.3)
+    r = ref(w, gamma=1.0, kappa=1.0)
+    u, _ = gpu(w, gamma=1.0, kappa=1.0)
+    assert relerr(u, r) <= 1e-10
+    assert relerr(u, ref(w)) > 1e-3   # and it differs from the default reading
+
+
+def test_large_tau_falls_back_to_exact_solver():
+    """tau = 16 h: rho = 0.88, the decay bound needs ~300 points of look-ahead -> AUTO picks EXACT."""
+    N, M = 160, 12
+    w = W.cfg2(N=N, M=M)
+    w.tau = 16.0 / N
+    r = ref(w)
+    u, info = gpu(w)
+    assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
+    assert relerr(u, r) <= 1e-10
+    with pytest.raises(B.Wave2DError) as e:
+        gpu(w, solver=B.SOLVER_STREAM)
+    assert e.value.status == -5
+
+
+def test_moderate_tau_uses_wider_lookahead():
+    """tau = 2.5 h (alpha ~ 3): halo of 48 points in fp64 -- the NB = 3 kernels."""
+    N, M = 300, 10
+    w = W.cfg2(N=N, M=M)
+    w.tau = 2.5 / N
+    w.c_half = np.ones(2 * M + 1)
+    r = ref(w)
+    u, info = gpu(w)
+    assert info["solver_x"] == B.SOLVER_STREAM
+    assert relerr(u, r) <= 1e-10
+
+
+def test_run_in_pieces_equals_one_run_and_reset_is_reproducible():
+    w = W.cfg2(N=260, M=40)
+    h = B.from_workload(w)
+    try:
+        h.run(w.M)
+        a = h.get()
+        h.set_initial(w.phi)            # resets k to 0
+        assert h.steps_done() == 0
+        for part in (1, 12, 2, 24, 1):   # plain launches, graph replays, tails
+            h.run(part)
+        assert h.steps_done() == w.M
+        b = h.get()
+        prev = h.get_prev()
+    finally:
+        h.close()
+    assert np.array_equal(a, b)         # bit-reproducible regardless of how the steps are batched
+    o = oracle.Wave2DOracle(w.N1, w.N2, w.l, w.tau, w.M)
+    o.set_speed(w.c_half)
+    o.set_initial(w.phi)
+    o.run(w.M)
+    assert relerr(prev, o.get_prev()) <= 1e-10
+    o.close()
+
+
+def test_device_pointers_strided_inputs_and_user_stream():
+    import torch
+    w = W.cfg4(N1=200, N2=120, M=15)
+    r = ref(w)
+    dev = torch.device("cuda:0")
+    ld = w.n1 + 5
+    big = torch.zeros((w.n2, ld), dtype=torch.float64, device=dev)
+    big[:, :w.n1] = torch.from_numpy(w.phi).to(dev)
+    st = torch.cuda.Stream()
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, "f64")
+    try:
+        h.set_stream(st)
+        h.set_speed(w.c_half)
+        h.set_initial(big[:, :w.n1])     # device pointer, ld > n1
+        h.run(w.M)
+        out = torch.full((w.n2, ld), 7.0, dtype=torch.float64, device=dev)
+        h.get(out[:, :w.n1])
+    finally:
+        h.close()
+    assert relerr(out[:, :w.n1].cpu().numpy(), r) <= 1e-10
+    assert bool((out[:, w.n1:] == 7.0).all())   # padding columns of the caller's buffer untouched
+
+
+def test_state_machine_and_argument_errors():
+    with pytest.raises(B.Wave2DError) as e:
+        B.Wave2D(1, 8, 1.0, 0.1, 4)
+    assert e.value.status == -1
+    h = B.Wave2D(32, 32, 1.0, 0.01, 4)
+    try:
+        with pytest.raises(B.Wave2DError) as e:
+            h.run(1)
+        assert e.value.status == -2                       # run before set_initial
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_speed(np.array([1.0, -1.0, 1.0, 1.0, 1.0, 1.0, 1.0, 1.0, 1.0]))
+        assert e.value.status == -1                       # c must be positive
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_speed(np.ones(5))
+        assert e.value.status == -1                       # count must be 1 or 2M+1
+        h.set_initial(np.zeros((31, 31)))
+        h.run(3)
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_speed(np.ones(1))
+        assert e.value.status == -2                       # set_* after the first run
+        with pytest.raises(B.Wave2DError) as e:
+            h.run(2)
+        assert e.value.status == -6                       # more than M steps
+        assert np.array_equal(h.get(), np.zeros((31, 31)))   # zero in, exactly zero out
+    finally:
+        h.close()
+
+
+# ---- full-size grids in the launch configuration bench.py times --------------------------------------------
+def test_cfg1_full_modal_closed_form():
+    w = W.cfg1()
+    u, _ = gpu(w)
+    a = modal_amplitudes(w.N1, w.N2, w.l, w.tau, 1, 1, 1.0, 0.0, w.c_half, 2 * w.M)[-1]
+    assert np.abs(u - a * w.phi).max() <= 1e-12
+    assert relerr(u, ref(w)) <= 1e-10
+
+
+def test_cfg2_full_size_full_M():
+    w = W.cfg2()
+    r = ref(w)
+    u, info = gpu(w)
+    assert relerr(u, r) <= 1e-10
+    assert np.abs(u - u[::-1, :]).max() <= 1e-12 and np.abs(u - u[:, ::-1]).max() <= 1e-12   # quadrant symmetry
+
+
+def test_cfg3_full_grid_source_on():
+    """4095^2 grid in bench.py's launch configuration; 24 steps with the Ricker wavelet shifted so that the
+    source is at its peak inside the window (the full M = 1000 oracle run is opt-in, see below)."""
+    M = 24
+    w = W.cfg3(N=4096, M=M)
+    w.g_half = W.ricker(W.half_times(w.tau, 2 * M) + 0.058)
+    r = ref(w)
+    u, info = gpu(w)
+    assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
+    assert np.abs(r).max() > 1e-6
+    assert relerr(u, r) <= 1e-10
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_cfg4_full_grid(dtype):
+    w = W.cfg4(M=16, dtype=dtype)
+    r = ref(w)
+    u, info = gpu(w)
+    assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
+    assert relerr(u, r) <= TOL[dtype]
+
+
+def test_cfg5_full_size_full_M_against_modal_closed_form():
+    """16383^2, M = 200: every mode's amplitude follows the exact scalar recurrence (tests/modal.py), so the
+    result is known at every point without running the oracle at this size.  Compared on 64 sampled rows."""
+    w = W.cfg5()
+    u, info = gpu(w)
+    assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
+    x, y = W.grid(w.N1, w.N2)
+    rows = np.unique(np.r_[0, 1, w.n2 - 1, np.random.default_rng(5).integers(0, w.n2, 61)])
+    expect = np.zeros((rows.size, w.n1))
+    for m, n, A in w.modes:
+        a = modal_amplitudes(w.N1, w.N2, w.l, w.tau, m, n, A, 0.0, w.c_half, 2 * w.M)[-1]
+        expect += a * np.outer(np.sin(n * np.pi * y[rows]), np.sin(m * np.pi * x))
+    scale = max(abs(A) for _, _, A in w.modes)
+    assert np.abs(u[rows] - expect).max() <= 1e-10 * scale
+    assert np.isfinite(u).all()
