@@ -120,10 +120,11 @@ def test_large_tau_falls_back_to_exact_solver():
 
 
 def test_moderate_tau_uses_wider_lookahead():
-    """tau = 2.5 h (alpha ~ 3): halo of 48 points in fp64 -- the NB = 3 kernels."""
+    """tau = 2.3 h (alpha = 2.645, rho = 0.430): rho^H <= 1e-17 needs H = 47 points in fp64 -- the NB = 3
+    kernels (48 points of look-ahead).  tau = 2.5 h would need H = 51 and fall to the exact solver."""
     N, M = 300, 10
     w = W.cfg2(N=N, M=M)
-    w.tau = 2.5 / N
+    w.tau = 2.3 / N
     w.c_half = np.ones(2 * M + 1)
     r = ref(w)
     u, info = gpu(w)
