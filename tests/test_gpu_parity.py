@@ -212,7 +212,10 @@ def test_cfg1_full_modal_closed_form():
     w = W.cfg1()
     u, _ = gpu(w)
     a = modal_amplitudes(w.N1, w.N2, w.l, w.tau, 1, 1, 1.0, 0.0, w.c_half, 2 * w.M)[-1]
-    assert np.abs(u - a * w.phi).max() <= 1e-12
+    # rounding noise eps per half-step enters the marginally stable three-term recurrence and grows like
+    # n per injection, so ~ n^2 eps / 2 = 200^2 * 1.1e-16 / 2 = 2e-12 in the worst case (the oracle itself sits
+    # 1.3e-12 from the closed form, tests/test_oracle_pins.py): 1e-11 absolute on an O(0.17) field.
+    assert np.abs(u - a * w.phi).max() <= 1e-11
     assert relerr(u, ref(w)) <= 1e-10
 
 
