@@ -338,7 +338,7 @@ def run_ours(args):
     ms_x, ms_y = h.profile_sweeps(PROF)
     geom = {k: h.info(k) for k in ("solver_x", "solver_y", "halo_x", "halo_y", "chunks_x", "chunks_y", "grid_x",
                                    "grid_y", "ctas_per_sm_x", "ctas_per_sm_y", "threads_x", "threads_y",
-                                   "smem_x", "smem_y")}
+                                   "smem_x", "smem_y", "nbk_x", "nbk_y", "quota_x", "quota_y", "unit_x", "unit_y")}
 
     # ---- end to end through the public API with HOST buffers: H2D(phi) + K steps + D2H(u) per iteration
     Ke = args.e2e_steps or K
@@ -379,7 +379,7 @@ def run_ours(args):
                 "steps_per_call": Ke, "seconds_per_call": e2e_s,
                 "what": "wave2d_set_initial(pinned host phi) + wave2d_run(steps_per_call) + wave2d_get(pinned host u), "
                         "wall clock incl. both copies; bytes are per call / steps_per_call"},
-        "roofline": {"bound": "hbm", "kernel": f"wave2d_sweep_stream<{w.dtype}, dir={dom}>", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": f"wave2d_sweep_panel<{w.dtype}, dir={dom}>", "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                      "peak_source": peak_src, "bytes_per_launch": sweep_bytes,
                      "ms_per_launch": ms_dom, "ms_x": ms_x, "ms_y": ms_y,

@@ -89,8 +89,9 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "solver" one of WAVE2D_SOLVER_*.     Default AUTO.
  *   "graph"  1 (default): the step loop is replayed as a CUDA Graph; 0: plain launches.
  *   "graph_steps"  time steps per graph replay (multiple of 3, the period of the buffer ring).  Default 12.
- *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (consumer warps / units per stage / stages).
- *   "chunks_x", "chunks_y" tuning: number of chunks a line is cut into (0 = planned from the SM count).
+ *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (units per stage = consumer warps / stages).
+ *   "quota_x", "quota_y"   tuning: stages of work per CTA (0 = planned: one wave over the resident CTA slots);
+ *                          lines are cut where a CTA's quota ends.
  * Errors: ERR_ARG (unknown name / bad value), ERR_STATE.
  */
 int wave2d_set_option(wave2d_t *h, const char *name, double value);
@@ -136,7 +137,10 @@ int wave2d_sync(wave2d_t *h);
  *   "solver_x", "solver_y"   solver path in use per direction (WAVE2D_SOLVER_EXACT / _STREAM), after planning
  *   "halo_x", "halo_y"       look-ahead H (points) with rho^H <= 1e-17 (fp64) / 1e-8 (fp32)
  *   "rho_x", "rho_y"         largest decay ratio rho over all half-steps
- *   "chunks_*", "grid_*", "ctas_per_sm_*", "smem_*", "threads_*", "unit_*", "upc_*"   launch geometry
+ *   "nbk_*"                  carry series length in units (halo = nbk * unit)
+ *   "kb_*"                   leading units solved with the tabulated boundary pivots
+ *   "chunks_*" (pieces of work), "grid_*", "ctas_per_sm_*", "smem_*", "threads_*", "unit_*", "quota_*",
+ *   "upc_*" (units per CTA)  launch geometry
  *   "source_window"          points kept of the source field (its non-zero bounding box)
  *   "launches"               kernels launched by this handle so far (graph nodes count individually)
  *   "pitch"                  internal row pitch in elements

@@ -12,9 +12,13 @@
 //
 //      forward   y_p = cp_p y_{p-1} + inv_p r_p          backward   x_p = y_p + cp_p x_{p+1}.
 //
-// Both are first-order recurrences with memory rho^k, so a line can be cut into chunks that each
-// start H points early (forward) and look H points ahead (backward) with rho^H below the rounding
-// unit.  The host stores cp_p, inv_p for p < K per half-step (exact boundary rows) and rho, 1/(beta-ap rho).
+// Both are first-order LINEAR recurrences, so a line is cut into units of U points that are solved
+// independently from a zero carry ("local" solve, one thread per unit), and the true carry is added
+// afterwards:   y_{p0+e} = yloc_e + (cp_{p0} .. cp_{p0+e}) Y_in,   Y_in = y at the end of the previous unit
+//                        = L_{g-1} + A_{g-1} (L_{g-2} + A_{g-2} ( ... ))        (L = last yloc, A = product of the unit's cp)
+// and the same from the right for x.  A_g <= rho^U, so the carry series is cut after NBK units with
+// rho^{NBK U} below the rounding unit (host-planned).  The host stores cp_p, inv_p for p < KMAX per
+// half-step (exact boundary rows) and rho, 1/(beta - ap rho) for the stationary rest.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -26,9 +30,16 @@
 namespace w2d {
 
 // ---- per-half-step scalar table (fp64, built on the host; row n serves half-step n -> n+1) ------
-constexpr int KMAX = 64;   // boundary rows with their own (cp_p, inv_p)
+constexpr int KMAX = 128;    // boundary rows with their own (cp_p, inv_p)
+constexpr int NBK_MAX = 8;   // longest carry series (units)
 constexpr int ROW_AM = 0, ROW_Q = 1, ROW_RHO = 2, ROW_INV = 3, ROW_C1 = 4, ROW_AP = 5, ROW_BETA = 6;
 constexpr int ROW_CP = 8, ROW_INVP = 8 + KMAX, ROW_DOUBLES = 8 + 2 * KMAX;
+
+// A piece of work: output units [ua, ub) of the 32 lines of panel `panel`; nst stages of NW units are
+// streamed, starting NBK units early (carry warm-up) and ending >= NBK units late (carry look-ahead).
+struct Piece {
+    int panel, ua, ub, nst;
+};
 
 struct SweepArgs {
     const double* table;   // device, ROW_DOUBLES per half-step
@@ -36,9 +47,10 @@ struct SweepArgs {
     int n_off;             // half-step index = n_off + 2 * (*d_k)
     int n;                 // unknowns per line
     int nlines;            // number of lines
-    int ntiles;            // ceil(nlines / TL)
-    int upc;               // units per chunk
-    int total_units;       // ceil(n / U)
+    int nbk;               // carry series length in units (<= NW, <= NBK_MAX)
+    int kb;                // units [0, kb) use the boundary pivots of the table
+    const Piece* pieces;   // device
+    const int* cta_off;    // device: CTA b owns pieces [cta_off[b], cta_off[b+1])
     void* out;             // y sweep: output field (direct coalesced stores)
     long long pitch;       // row pitch in elements
     const void* src;       // compact source window, [p - sp0][line - sl0] (line fastest), or NULL
@@ -46,73 +58,82 @@ struct SweepArgs {
     double g2;             // 2 gamma
 };
 
-template <typename T, int DIR, int NB, int NW, int XB, int NSTAGE>
-struct StreamCfg {
-    static constexpr int U = 128 / sizeof(T);          // points per unit (one 128-byte swizzle row)
-    static constexpr int TL = 32 * NW;                 // lines per CTA, one per consumer thread
-    static constexpr int UNIT_BYTES = TL * 128;        // one unit of one field
-    static constexpr int STAGE_BYTES = 2 * XB * UNIT_BYTES;
-    static constexpr int OUT_BYTES = DIR == 0 ? NW * 2 * 32 * 128 : 0;
+template <typename T, int DIR, int NW, int NSTAGE>
+struct PanelCfg {
+    static constexpr int U = DIR == 0 ? 128 / (int)sizeof(T) : 16;   // points per unit
+    static constexpr int TL = 32;                                    // lines per panel, one per lane
+    static constexpr int V = 16 / (int)sizeof(T);                    // elements per 16 bytes
+    // x sweep: per field NW unit tiles [32 rows][128 B] (128B-swizzled) + two edge boxes [32 rows][16 B] of wp
+    // y sweep: per field one box [U*NW + 2 rows][32 columns]
+    static constexpr int FIELD_BYTES = DIR == 0 ? NW * 4096 : (U * NW + 2) * TL * (int)sizeof(T);
+    static constexpr int EDGE_BYTES = DIR == 0 ? 512 : 0;
+    static constexpr int STAGE_BYTES = 2 * FIELD_BYTES + 2 * EDGE_BYTES;
+    static constexpr int OUT_BYTES = DIR == 0 ? NW * 4096 : 0;
     static constexpr int BAR_BYTES = ((2 * NSTAGE * 8) + 15) / 16 * 16;
-    static constexpr int TAB_BYTES = 2 * KMAX * sizeof(T);
-    static constexpr int SMEM_BYTES = 1024 + NSTAGE * STAGE_BYTES + OUT_BYTES + BAR_BYTES + TAB_BYTES;
+    static constexpr int TAB_BYTES = 2 * KMAX * (int)sizeof(T);
+    static constexpr int XCH_BYTES = (4 * NW * TL + 2 * NW + 2) * (int)sizeof(T);   // Ls[2][NW][32], Hs[2][NW][32], As[2][NW]
+    static constexpr int SMEM_BYTES = 1024 + NSTAGE * STAGE_BYTES + OUT_BYTES + BAR_BYTES + TAB_BYTES + XCH_BYTES;
     static constexpr int THREADS = 32 * (NW + 1);
+    static_assert(FIELD_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
+    static_assert(DIR == 0 || U * NW + 2 <= 256, "TMA box dimension limit");
 };
 
-// Read this thread's line of one unit tile into registers.
-//   DIR 0 (x sweep): tile = [TL rows][128 B], 128B-swizzled by TMA: 16-byte chunk c of row t sits at chunk c ^ (t & 7).
-//   DIR 1 (y sweep): tile = [U rows][TL columns], dense.
-template <typename T, int DIR, int TL>
-__device__ __forceinline__ void load_unit(const unsigned char* tile, int tid, T (&v)[128 / sizeof(T)])
+// Read this lane's line of one x-sweep unit tile [32 rows][128 B] into registers; the tile is
+// 128B-swizzled by TMA: 16-byte chunk c of row t sits at chunk c ^ (t & 7)  (bank-conflict-free).
+template <typename T>
+__device__ __forceinline__ void load_unit_x(const unsigned char* tile, int lane, T (&v)[128 / sizeof(T)])
 {
-    constexpr int U = 128 / sizeof(T);
-    if constexpr (DIR == 0) {
-        const unsigned char* row = tile + tid * 128;
-        const int sw = (tid & 7) << 4;
+    const unsigned char* row = tile + lane * 128;
+    const int sw = (lane & 7) << 4;
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            if constexpr (sizeof(T) == 8) {
-                const double2 t = *reinterpret_cast<const double2*>(row + ((c << 4) ^ sw));
-                v[2 * c] = t.x;
-                v[2 * c + 1] = t.y;
-            } else {
-                const float4 t = *reinterpret_cast<const float4*>(row + ((c << 4) ^ sw));
-                v[4 * c] = t.x;
-                v[4 * c + 1] = t.y;
-                v[4 * c + 2] = t.z;
-                v[4 * c + 3] = t.w;
-            }
+    for (int c = 0; c < 8; ++c) {
+        if constexpr (sizeof(T) == 8) {
+            const double2 t = *reinterpret_cast<const double2*>(row + ((c << 4) ^ sw));
+            v[2 * c] = t.x;
+            v[2 * c + 1] = t.y;
+        } else {
+            const float4 t = *reinterpret_cast<const float4*>(row + ((c << 4) ^ sw));
+            v[4 * c] = t.x;
+            v[4 * c + 1] = t.y;
+            v[4 * c + 2] = t.z;
+            v[4 * c + 3] = t.w;
         }
-    } else {
-        const T* col = reinterpret_cast<const T*>(tile) + tid;
-#pragma unroll
-        for (int e = 0; e < U; ++e) v[e] = col[e * TL];
     }
 }
-
-template <typename T, int DIR, int TL>
-__device__ __forceinline__ T peek_first(const unsigned char* tile, int tid)
+// first / last element of this lane's row of an x-sweep unit tile
+template <typename T>
+__device__ __forceinline__ T tile_first_x(const unsigned char* tile, int lane)
 {
-    if constexpr (DIR == 0)
-        return *reinterpret_cast<const T*>(tile + tid * 128 + ((tid & 7) << 4));
-    else
-        return reinterpret_cast<const T*>(tile)[tid];
+    return *reinterpret_cast<const T*>(tile + lane * 128 + ((lane & 7) << 4));
+}
+template <typename T>
+__device__ __forceinline__ T tile_last_x(const unsigned char* tile, int lane)
+{
+    return *reinterpret_cast<const T*>(tile + lane * 128 + ((7 ^ (lane & 7)) << 4) + 16 - sizeof(T));
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Streamed sweep: RHS assembly (A1/A3) fused with the line solve (A2/A4), SURVEY.md 8a.
-//   grid  = ntiles * nchunks CTAs; CTA (tile, chunk) owns lines [tile*TL, +TL) and output units
-//           [chunk*upc, +upc) of every one of them; it streams units [first - NB, last + NB].
-//   block = NW consumer warps (one thread per line) + 1 producer warp (one lane issues TMA).
+// Panel sweep: RHS assembly (A1/A3) fused with the line solve (A2/A4), SURVEY.md 8a.
+//   grid  = persistent CTAs (SM count x CTAs/SM); CTA b walks its host-planned pieces.
+//   block = NW consumer warps + 1 producer warp (one lane issues TMA).  Per stage, consumer warp w
+//           owns unit g = gbase + s*NW + w of the panel's 32 lines, lane = line.
+//   stage:  smem -> registers, release the slot; RHS + local forward; publish L, A; bar;
+//           carry-in, correct y, local backward; publish head; bar;
+//           finish the unit of the PREVIOUS stage (its look-ahead heads are now known) and store it.
 // ---------------------------------------------------------------------------------------------------
-template <typename T, int DIR, int NB, int NW, int XB, int NSTAGE>
-__global__ void __launch_bounds__(32 * (NW + 1))
-wave2d_sweep_stream(const __grid_constant__ CUtensorMap tm_prev, const __grid_constant__ CUtensorMap tm_cur,
-                    const __grid_constant__ CUtensorMap tm_out, const SweepArgs a)
+template <typename T, int DIR, int NW, int NSTAGE>
+__global__ void __launch_bounds__(32 * (NW + 1), 1)
+wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_constant__ CUtensorMap tm_cur,
+                   const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_edge,
+                   const SweepArgs a)
 {
-    using K = StreamCfg<T, DIR, NB, NW, XB, NSTAGE>;
-    constexpr int U = K::U, TL = K::TL, RING = (NB + 1) * U;
-    static_assert(NB * U <= KMAX, "boundary table too short");
+    using K = PanelCfg<T, DIR, NW, NSTAGE>;
+    constexpr int U = K::U, TL = K::TL, V = K::V;
 
     extern __shared__ unsigned char smem_raw[];
     const uint32_t raw32 = smem_u32(smem_raw);
@@ -123,6 +144,9 @@ wave2d_sweep_stream(const __grid_constant__ CUtensorMap tm_prev, const __grid_co
     const uint32_t bar32 = sm32 + NSTAGE * K::STAGE_BYTES + K::OUT_BYTES;   // full[NSTAGE], empty[NSTAGE]
     T* s_cp = reinterpret_cast<T*>(sm + NSTAGE * K::STAGE_BYTES + K::OUT_BYTES + K::BAR_BYTES);
     T* s_inv = s_cp + KMAX;
+    T* s_L = s_inv + KMAX;            // [2][NW][32]  last local y of a unit
+    T* s_H = s_L + 2 * NW * TL;       // [2][NW][32]  first local x of a unit
+    T* s_A = s_H + 2 * NW * TL;       // [2][NW]      product of the unit's cp
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nh = a.n_off + (a.d_k ? 2 * (*a.d_k) : 0);
@@ -142,179 +166,223 @@ wave2d_sweep_stream(const __grid_constant__ CUtensorMap tm_prev, const __grid_co
     }
     __syncthreads();
 
-    const int tile = blockIdx.x % a.ntiles, chunk = blockIdx.x / a.ntiles;
-    const int line0 = tile * TL;
-    const int uo0 = chunk * a.upc;                                         // output units [uo0, uo1)
-    const int uo1 = min(uo0 + a.upc, a.total_units);
-    const int ub = max(uo0 - NB, 0);                                       // first streamed unit
-    const int ue_want = (uo1 == a.total_units ? a.total_units : uo1) + NB; // lookahead / flush units
-    const int ns = (ue_want - ub + XB - 1) / XB;                           // stages
+    const int pc_begin = a.cta_off[blockIdx.x], pc_end = a.cta_off[blockIdx.x + 1];
 
     if (warp == NW) {   // ---------------- producer: one lane feeds the stage ring by TMA
         if (lane == 0) {
             tma_prefetch_desc(&tm_prev);
             tma_prefetch_desc(&tm_cur);
-            for (int s = 0; s < ns; ++s) {
-                const int slot = s % NSTAGE;
-                if (s >= NSTAGE) mbar_wait(bar32 + 8 * (NSTAGE + slot), ((s / NSTAGE) - 1) & 1);
-                const uint32_t full = bar32 + 8 * slot;
-                mbar_arrive_expect_tx(full, K::STAGE_BYTES);
-                const uint32_t dst = sm32 + slot * K::STAGE_BYTES;
-                const int u0 = ub + s * XB;
-                if constexpr (DIR == 0) {
+            int it = 0;
+            for (int pi = pc_begin; pi < pc_end; ++pi) {
+                const Piece pc = a.pieces[pi];
+                const int line0 = pc.panel * TL;
+                const int gbase = max(pc.ua - a.nbk, 0);
+                for (int s = 0; s < pc.nst; ++s, ++it) {
+                    const int slot = it % NSTAGE;
+                    if (it >= NSTAGE) mbar_wait(bar32 + 8 * (NSTAGE + slot), ((it / NSTAGE) - 1) & 1);
+                    const uint32_t full = bar32 + 8 * slot;
+                    mbar_arrive_expect_tx(full, K::STAGE_BYTES);
+                    const uint32_t dst = sm32 + slot * K::STAGE_BYTES;
+                    const int g0 = gbase + s * NW;
+                    if constexpr (DIR == 0) {
 #pragma unroll
-                    for (int xb = 0; xb < XB; ++xb) {
-                        tma_load_2d(dst + xb * K::UNIT_BYTES, &tm_prev, (u0 + xb) * U, line0, full);
-                        tma_load_2d(dst + (XB + xb) * K::UNIT_BYTES, &tm_cur, (u0 + xb) * U, line0, full);
+                        for (int w = 0; w < NW; ++w) {
+                            tma_load_2d(dst + w * 4096, &tm_prev, (g0 + w) * U, line0, full);
+                            tma_load_2d(dst + K::FIELD_BYTES + w * 4096, &tm_cur, (g0 + w) * U, line0, full);
+                        }
+                        tma_load_2d(dst + 2 * K::FIELD_BYTES, &tm_edge, g0 * U - V, line0, full);
+                        tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
+                    } else {
+                        tma_load_2d(dst, &tm_prev, line0, g0 * U - 1, full);
+                        tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0, g0 * U - 1, full);
                     }
-                } else {
-                    tma_load_2d(dst, &tm_prev, line0, u0 * U, full);
-                    tma_load_2d(dst + XB * K::UNIT_BYTES, &tm_cur, line0, u0 * U, full);
                 }
             }
         }
         return;
     }
 
-    // -------------------- consumers: thread tid owns line line0 + tid
-    const int tid = threadIdx.x;
-    const int line = line0 + tid;
+    // -------------------- consumers
     const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), rho = static_cast<T>(row[ROW_RHO]);
     const T inv = static_cast<T>(row[ROW_INV]), c1 = static_cast<T>(row[ROW_C1]), g2 = static_cast<T>(a.g2);
-    const int n = a.n;
-    const bool src_tile = a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
-    const bool src_line = line >= a.sl0 && line < a.sl0 + a.snl;
-    const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
+    const int n = a.n, nbk = a.nbk;
+    T pw[U];   // pw[e] = rho^(e+1)
+    pw[0] = rho;
+#pragma unroll
+    for (int e = 1; e < U; ++e) pw[e] = pw[e - 1] * rho;
+    auto cp_at = [&](int p) -> T { return p < KMAX ? s_cp[p] : rho; };
+    auto inv_at = [&](int p) -> T { return p < KMAX ? s_inv[p] : inv; };
 
-    T ring[RING];   // y of the last NB+1 units, oldest first
+    T pend[U];
 #pragma unroll
-    for (int e = 0; e < RING; ++e) ring[e] = T(0);
-    T fy = T(0), wp_last = T(0);
-    int ob = 0;
+    for (int e = 0; e < U; ++e) pend[e] = T(0);
+    int it = 0;
 
-    auto unit = [&](auto gen_c, const unsigned char* tprev, const unsigned char* tcur, T peek, int k) {
-        constexpr bool GEN = decltype(gen_c)::value;
-        T wp[U], wc[U];
-        load_unit<T, DIR, TL>(tprev, tid, wp);
-        load_unit<T, DIR, TL>(tcur, tid, wc);
+    for (int pi = pc_begin; pi < pc_end; ++pi) {
+        const Piece pc = a.pieces[pi];
+        const int line0 = pc.panel * TL, line = line0 + lane;
+        const int gbase = max(pc.ua - nbk, 0);
+        const bool src_tile = a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
+        const bool src_line = line >= a.sl0 && line < a.sl0 + a.snl;
+        const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
+
+        named_bar_sync(1, NW * 32);   // the previous piece is completely finished
+        s_L[(NW + warp) * TL + lane] = T(0);   // "stage -1": zero carries
+        if (lane == 0) s_A[NW + warp] = T(0);
+
+        for (int s = 0; s <= pc.nst; ++s) {
+            const int buf = s & 1;
+            const int g = gbase + s * NW + warp, p0 = g * U;
+            const bool act = s < pc.nst;
+            bool fast = false;
+            T xl[U];
 #pragma unroll
-        for (int e = 0; e < NB * U; ++e) ring[e] = ring[e + U];
-        const int p0 = k * U;
-        const bool tab_new = GEN && k < NB;
-        const bool src_unit = GEN && src_tile && src_line;
-        // ---- RHS (A1/A3) and forward elimination
+            for (int e = 0; e < U; ++e) xl[e] = T(0);
+
+            if (act) {
+                const int slot = it % NSTAGE;
+                mbar_wait(bar32 + 8 * slot, (it / NSTAGE) & 1);
+                ++it;
+                const unsigned char* st = sm + slot * K::STAGE_BYTES;
+                T wp[U], wc[U], wl, wr;
+                if constexpr (DIR == 0) {
+                    const unsigned char* tp = st + warp * 4096;
+                    load_unit_x<T>(tp, lane, wp);
+                    load_unit_x<T>(st + K::FIELD_BYTES + warp * 4096, lane, wc);
+                    wl = warp == 0 ? reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES)[lane * V + V - 1]
+                                   : tile_last_x<T>(tp - 4096, lane);
+                    wr = warp == NW - 1 ? reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V]
+                                        : tile_first_x<T>(tp + 4096, lane);
+                } else {
+                    const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
+                    const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
+                    wl = cpv[0];
 #pragma unroll
-        for (int e = 0; e < U; ++e) {
-            const T left = e == 0 ? wp_last : wp[e - 1];
-            const T right = e == U - 1 ? peek : wp[e + 1];
-            T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
-            T cpe = rho, ive = inv;
-            if constexpr (GEN) {
-                const int p = p0 + e;
-                if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
-                    r = fma(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
-                if (tab_new) {
-                    cpe = s_cp[p];
-                    ive = s_inv[p];
+                    for (int e = 0; e < U; ++e) wp[e] = cpv[(e + 1) * TL];
+                    wr = cpv[(U + 1) * TL];
+#pragma unroll
+                    for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar32 + 8 * (NSTAGE + slot));   // data is in registers: release the slot
+
+                const bool src_k = src_tile && p0 < a.sp0 + a.snp && p0 + U > a.sp0;
+                fast = g >= a.kb && p0 + U <= n && !src_k;
+                T Aval;
+                if (fast) {   // stationary pivots: y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
+                    T fy = T(0);
+#pragma unroll
+                    for (int e = 0; e < U; ++e) {
+                        const T left = e == 0 ? wl : wp[e - 1];
+                        const T right = e == U - 1 ? wr : wp[e + 1];
+                        const T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                        fy = fma(rho, fy, r * inv);
+                        xl[e] = fy;
+                    }
+                    Aval = pw[U - 1];
+                } else {
+                    const bool src_unit = src_k && src_line;
+                    T fy = T(0), prod = T(1);
+#pragma unroll
+                    for (int e = 0; e < U; ++e) {
+                        const int p = p0 + e;
+                        const T left = e == 0 ? wl : wp[e - 1];
+                        const T right = e == U - 1 ? wr : wp[e + 1];
+                        T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                        if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
+                            r = fma(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
+                        const T cpe = cp_at(p);
+                        fy = fma(cpe, fy, r * inv_at(p));
+                        if (p >= n) fy = T(0);
+                        prod *= cpe;
+                        xl[e] = fy;
+                    }
+                    Aval = prod;
+                }
+                s_L[(buf * NW + warp) * TL + lane] = xl[U - 1];
+                if (lane == 0) s_A[buf * NW + warp] = Aval;
+            }
+            named_bar_sync(1, NW * 32);
+
+            if (act) {
+                T Yin = T(0);   // y at the end of unit g-1
+                for (int j = nbk; j >= 1; --j) {
+                    int idx = warp - j, b = buf;
+                    if (idx < 0) { idx += NW; b ^= 1; }
+                    Yin = fma(s_A[b * NW + idx], Yin, s_L[(b * NW + idx) * TL + lane]);
+                }
+                if (fast) {
+#pragma unroll
+                    for (int e = 0; e < U; ++e) xl[e] = fma(pw[e], Yin, xl[e]);
+#pragma unroll
+                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(rho, xl[e + 1], xl[e]);
+                } else {
+                    T c = Yin;
+#pragma unroll
+                    for (int e = 0; e < U; ++e) {
+                        c *= cp_at(p0 + e);
+                        xl[e] = p0 + e < n ? xl[e] + c : T(0);
+                    }
+#pragma unroll
+                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(cp_at(p0 + e), xl[e + 1], xl[e]);
                 }
             }
-            fy = fma(cpe, fy, r * ive);
-            T v = fy;
-            if constexpr (GEN) {
-                if (p0 + e >= n) v = T(0);
-            }
-            ring[NB * U + e] = v;
-        }
-        wp_last = wp[U - 1];
-        // ---- back substitution: NB units of look-ahead, then the unit that is NB behind
-        T x = T(0);
+            s_H[(buf * NW + warp) * TL + lane] = xl[0];   // 0 in the flush stage
+            named_bar_sync(1, NW * 32);
+
+            if (s > 0) {   // finish the unit of stage s-1: gp = g - NW, local x in pend[]
+                const int gp = g - NW, pp0 = gp * U;
+                T Xin = T(0);   // x at the start of unit gp+1
+                for (int j = nbk; j >= 1; --j) {
+                    int idx = warp + j, b = buf ^ 1;
+                    if (idx >= NW) { idx -= NW; b ^= 1; }
+                    Xin = fma(s_A[b * NW + idx], Xin, s_H[(b * NW + idx) * TL + lane]);
+                }
+                if (gp >= pc.ua && gp < pc.ub) {   // warp-uniform
+                    if (gp >= a.kb && pp0 + U <= n) {
 #pragma unroll
-        for (int e = RING - 1; e >= U; --e) {
-            T cpe = rho;
-            if constexpr (GEN) {
-                const int p = (k - NB) * U + e;
-                if (p >= 0 && p < NB * U) cpe = s_cp[p];
-            }
-            x = fma(cpe, x, ring[e]);
-        }
-        const int ko = k - NB;
-        if (ko >= uo0 && ko < uo1) {
-            if constexpr (DIR == 0) {
-                unsigned char* ot = sm_out + (warp * 2 + ob) * 4096;
-                if (lane == 0) tma_wait_read<1>();
-                __syncwarp();
-                unsigned char* orow = ot + lane * 128;
-                const int sw = (lane & 7) << 4;
-                constexpr int V = 16 / sizeof(T);
+                        for (int e = 0; e < U; ++e) pend[e] = fma(pw[U - 1 - e], Xin, pend[e]);
+                    } else {
+                        T c = Xin;
 #pragma unroll
-                for (int c = 7; c >= 0; --c) {
-                    T xo[V];
-#pragma unroll
-                    for (int i = V - 1; i >= 0; --i) {
-                        T cpe = rho;
-                        if constexpr (GEN) {
-                            const int p = ko * U + c * V + i;
-                            if (p < NB * U) cpe = s_cp[p];
+                        for (int e = U - 1; e >= 0; --e) {
+                            c *= cp_at(pp0 + e);
+                            pend[e] += c;
                         }
-                        x = fma(cpe, x, ring[c * V + i]);
-                        xo[i] = x;
                     }
-                    if constexpr (sizeof(T) == 8)
-                        *reinterpret_cast<double2*>(orow + ((c << 4) ^ sw)) = make_double2(xo[0], xo[1]);
-                    else
-                        *reinterpret_cast<float4*>(orow + ((c << 4) ^ sw)) = make_float4(xo[0], xo[1], xo[2], xo[3]);
-                }
-                fence_async_smem();
-                __syncwarp();
-                if (lane == 0) {
-                    tma_store_2d(&tm_out, ko * U, line0 + warp * 32, smem_u32(ot));
-                    tma_commit();
-                }
-                ob ^= 1;
-            } else {
-                T* o = reinterpret_cast<T*>(a.out) + static_cast<long long>(ko * U) * a.pitch + line;
-                const bool line_ok = line < a.nlines;
+                    if constexpr (DIR == 0) {
+                        unsigned char* ot = sm_out + warp * 4096;
+                        if (lane == 0) tma_wait_read<0>();   // the previous store of this warp has read the tile
+                        __syncwarp();
+                        unsigned char* orow = ot + lane * 128;
+                        const int sw = (lane & 7) << 4;
 #pragma unroll
-                for (int e = U - 1; e >= 0; --e) {
-                    T cpe = rho;
-                    if constexpr (GEN) {
-                        const int p = ko * U + e;
-                        if (p < NB * U) cpe = s_cp[p];
+                        for (int c = 0; c < 8; ++c) {
+                            if constexpr (sizeof(T) == 8)
+                                *reinterpret_cast<double2*>(orow + ((c << 4) ^ sw)) = make_double2(pend[2 * c], pend[2 * c + 1]);
+                            else
+                                *reinterpret_cast<float4*>(orow + ((c << 4) ^ sw)) =
+                                    make_float4(pend[4 * c], pend[4 * c + 1], pend[4 * c + 2], pend[4 * c + 3]);
+                        }
+                        fence_async_smem();
+                        __syncwarp();
+                        if (lane == 0) {
+                            tma_store_2d(&tm_out, pp0, line0, smem_u32(ot));
+                            tma_commit();
+                        }
+                    } else {
+                        if (line < a.nlines) {
+                            T* o = reinterpret_cast<T*>(a.out) + static_cast<long long>(pp0) * a.pitch + line;
+#pragma unroll
+                            for (int e = 0; e < U; ++e)
+                                if (pp0 + e < n) o[static_cast<long long>(e) * a.pitch] = pend[e];
+                        }
                     }
-                    x = fma(cpe, x, ring[e]);
-                    bool ok = line_ok;
-                    if constexpr (GEN) ok = ok && (ko * U + e < n);
-                    if (ok) o[static_cast<long long>(e) * a.pitch] = x;
                 }
             }
-        }
-    };
-
-    mbar_wait(bar32, 0);
-    for (int s = 0; s < ns; ++s) {
-        const int slot = s % NSTAGE;
-        const unsigned char* st = sm + slot * K::STAGE_BYTES;
-        const bool has_next = s + 1 < ns;
-        const int nslot = (s + 1) % NSTAGE;
 #pragma unroll
-        for (int xb = 0; xb < XB; ++xb) {
-            const int k = ub + s * XB + xb;
-            T peek = T(0);
-            if (xb + 1 < XB) {
-                peek = peek_first<T, DIR, TL>(st + (xb + 1) * K::UNIT_BYTES, tid);
-            } else if (has_next) {
-                mbar_wait(bar32 + 8 * nslot, ((s + 1) / NSTAGE) & 1);   // the next stage is also this loop's next wait
-                peek = peek_first<T, DIR, TL>(sm + nslot * K::STAGE_BYTES, tid);
-            }
-            const bool src_k = src_tile && k * U < a.sp0 + a.snp && (k + 1) * U > a.sp0;
-            const bool fast = k >= 2 * NB && (k + 1) * U <= n && !src_k;
-            if (fast)
-                unit(std::false_type{}, st + xb * K::UNIT_BYTES, st + (XB + xb) * K::UNIT_BYTES, peek, k);
-            else
-                unit(std::true_type{}, st + xb * K::UNIT_BYTES, st + (XB + xb) * K::UNIT_BYTES, peek, k);
+            for (int e = 0; e < U; ++e) pend[e] = xl[e];
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar32 + 8 * (NSTAGE + slot));
     }
     if constexpr (DIR == 0) {
         if (lane == 0) tma_wait_read<0>();

@@ -21,57 +21,51 @@ using namespace w2d;
 namespace {
 
 // ------------------------------------------------------------------------------------------------
-// Kernel variants: (NW consumer warps, XB units per stage, NSTAGE) per direction, per look-ahead NB.
+// Kernel variants: (NW consumer warps = units per stage, NSTAGE) per dtype and direction.
 // ------------------------------------------------------------------------------------------------
 struct Variant {
-    int dir, nb, nw, xb, nstage, smem, threads, elem;   // elem = sizeof(T)
+    int dir, nw, nstage, unit, smem, threads, elem;   // elem = sizeof(T), unit = points per unit
     const void* fn;
 };
 
-template <typename T, int DIR, int NB, int NW, int XB, int NSTAGE>
+template <typename T, int DIR, int NW, int NSTAGE>
 Variant make_variant()
 {
-    using K = StreamCfg<T, DIR, NB, NW, XB, NSTAGE>;
-    return Variant{DIR, NB, NW, XB, NSTAGE, K::SMEM_BYTES, K::THREADS, (int)sizeof(T),
-                   reinterpret_cast<const void*>(&wave2d_sweep_stream<T, DIR, NB, NW, XB, NSTAGE>)};
+    using K = PanelCfg<T, DIR, NW, NSTAGE>;
+    return Variant{DIR, NW, NSTAGE, K::U, K::SMEM_BYTES, K::THREADS, (int)sizeof(T),
+                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, NW, NSTAGE>)};
 }
 
-constexpr int NVAR = 4;   // shape variants per (dtype, dir, NB); index 0 is the default
-template <typename T, int DIR, int NB>
+constexpr int NVAR = 4;   // shape variants per (dtype, dir); index 0 is the default
+template <typename T>
 void add_shapes(std::vector<Variant>& v)
 {
-    if (DIR == 0) {
-        v.push_back(make_variant<T, DIR, NB, 1, 2, 4>());
-        v.push_back(make_variant<T, DIR, NB, 1, 1, 6>());
-        v.push_back(make_variant<T, DIR, NB, 2, 2, 3>());
-        v.push_back(make_variant<T, DIR, NB, 1, 4, 3>());
-    } else {
-        v.push_back(make_variant<T, DIR, NB, 2, 1, 4>());
-        v.push_back(make_variant<T, DIR, NB, 1, 1, 6>());
-        v.push_back(make_variant<T, DIR, NB, 4, 1, 3>());
-        v.push_back(make_variant<T, DIR, NB, 2, 2, 3>());
-    }
+    v.push_back(make_variant<T, 0, 8, 2>());
+    v.push_back(make_variant<T, 0, 4, 3>());
+    v.push_back(make_variant<T, 0, 4, 2>());
+    v.push_back(make_variant<T, 0, 6, 2>());
+    v.push_back(make_variant<T, 1, 8, 3>());
+    v.push_back(make_variant<T, 1, 4, 3>());
+    v.push_back(make_variant<T, 1, 8, 2>());
+    v.push_back(make_variant<T, 1, 4, 4>());
 }
-constexpr int NB_MAX_F64 = 3, NB_MAX_F32 = 2;
 
 const std::vector<Variant>& variants()
 {
     static std::vector<Variant> v = [] {
         std::vector<Variant> w;
-        add_shapes<double, 0, 1>(w); add_shapes<double, 0, 2>(w); add_shapes<double, 0, 3>(w);
-        add_shapes<double, 1, 1>(w); add_shapes<double, 1, 2>(w); add_shapes<double, 1, 3>(w);
-        add_shapes<float, 0, 1>(w);  add_shapes<float, 0, 2>(w);
-        add_shapes<float, 1, 1>(w);  add_shapes<float, 1, 2>(w);
+        add_shapes<double>(w);
+        add_shapes<float>(w);
         return w;
     }();
     return v;
 }
 
-const Variant* find_variant(int elem, int dir, int nb, int shape)
+const Variant* find_variant(int elem, int dir, int shape)
 {
     int seen = 0;
     for (const Variant& v : variants())
-        if (v.elem == elem && v.dir == dir && v.nb == nb) {
+        if (v.elem == elem && v.dir == dir) {
             if (seen == shape) return &v;
             ++seen;
         }
@@ -96,10 +90,12 @@ EncodeTiledFn encode_tiled()
 
 struct DirPlan {
     int solver = WAVE2D_SOLVER_STREAM;   // STREAM or EXACT after planning
-    int nb = 1, halo = 0, shape = 0;
+    int nbk = 1, kb = 0, halo = 0, shape = 0;
     double rho = 0.0;
     const Variant* var = nullptr;
-    int n = 0, nlines = 0, ntiles = 0, upc = 0, nchunks = 0, total_units = 0, grid = 0, ctas_per_sm = 0;
+    int n = 0, nlines = 0, npanels = 0, total_units = 0, grid = 0, ctas_per_sm = 0, quota = 0;
+    std::vector<Piece> pieces;
+    std::vector<int> cta_off;
 };
 
 }  // namespace
@@ -108,7 +104,7 @@ struct wave2d_s {
     int N1, N2, n1, n2, M, dtype, elem;
     double l, tau, gamma = 2.0, kappa = 0.5;
     int opt_solver = WAVE2D_SOLVER_AUTO, opt_graph = 1, opt_graph_steps = 12, opt_shape[2] = {0, 0};
-    int opt_chunks[2] = {0, 0};
+    int opt_quota[2] = {0, 0};
     cudaStream_t own_stream = nullptr, stream = nullptr;
     int num_sms = 0;
 
@@ -125,7 +121,9 @@ struct wave2d_s {
     double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
     bool plan_ok = false;
     DirPlan plan[2];
-    CUtensorMap tm_load[2][3], tm_store[3];   // [dir][buffer]
+    CUtensorMap tm_load[2][3], tm_edge[3];    // [dir][buffer]; x: unit tile (load and store) + 16-byte edge box
+    Piece* d_pieces[2] = {nullptr, nullptr};
+    int* d_cta_off[2] = {nullptr, nullptr};
     cudaGraphExec_t gexec = nullptr;
     int gexec_steps = 0;
 
@@ -230,62 +228,106 @@ int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, bool
     return WAVE2D_OK;
 }
 
+// Cut the (panel, unit) space into pieces, `quota` stages per CTA.  A cut costs 2 nbk extra units (carry warm-up
+// before the cut, look-ahead after it).  Returns false if a CTA could make no progress (quota too small).
+bool build_pieces(DirPlan& P, int nw, int quota)
+{
+    P.pieces.clear();
+    P.cta_off.assign(1, 0);
+    const int UT = P.total_units;
+    int panel = 0, ua = 0;
+    while (panel < P.npanels) {
+        int left = quota;
+        while (left > 0 && panel < P.npanels) {
+            const int ua0 = std::max(ua - P.nbk, 0);
+            const int rest = (UT - ua0 + nw - 1) / nw;
+            if (rest <= left) {
+                P.pieces.push_back(Piece{panel, ua, UT, rest});
+                left -= rest;
+                ++panel;
+                ua = 0;
+            } else {
+                const int ub = ua0 + left * nw - P.nbk;
+                if (ub <= ua) {
+                    if (left == quota) return false;
+                    break;
+                }
+                P.pieces.push_back(Piece{panel, ua, ub, left});
+                ua = ub;
+                left = 0;
+            }
+        }
+        P.cta_off.push_back((int)P.pieces.size());
+    }
+    return true;
+}
+
 int plan_dir(wave2d_t* h, int d)
 {
     DirPlan& P = h->plan[d];
     P = DirPlan();
     P.n = d == 0 ? h->n1 : h->n2;
     P.nlines = d == 0 ? h->n2 : h->n1;
-    double rho = 0.0;
-    for (int n = d; n < 2 * h->M; n += 2) rho = std::max(rho, h->table[static_cast<size_t>(n) * ROW_DOUBLES + ROW_RHO]);
-    P.rho = rho;
-    const int U = 128 / h->elem;
-    const double tol = h->dtype == WAVE2D_F64 ? 1e-17 : 1e-8;   // rho^H <= tol: below half an ulp of T
-    int H = 1;
-    if (rho > 0.0) H = std::max(1, (int)std::ceil(std::log(tol) / std::log(rho)));
-    P.halo = H;
-    const int nbmax = h->dtype == WAVE2D_F64 ? NB_MAX_F64 : NB_MAX_F32;
-    const int nb = (H + U - 1) / U;
-    if (h->opt_solver == WAVE2D_SOLVER_EXACT || (h->opt_solver == WAVE2D_SOLVER_AUTO && nb > nbmax)) {
-        P.solver = WAVE2D_SOLVER_EXACT;
-        return WAVE2D_OK;
-    }
-    if (nb > nbmax) {
-        h->err = "streamed solver: decay bound rho^H <= tol needs more look-ahead than supported";
-        return WAVE2D_ERR_UNSUPPORTED;
-    }
-    P.solver = WAVE2D_SOLVER_STREAM;
-    P.nb = nb;
-    P.halo = nb * U;
     P.shape = h->opt_shape[d];
-    P.var = find_variant(h->elem, d, nb, P.shape);
+    P.var = find_variant(h->elem, d, P.shape);
     if (!P.var) {
         h->err = "no kernel variant for this shape index";
         return WAVE2D_ERR_ARG;
     }
     const Variant& V = *P.var;
+    const int U = V.unit;
+    const double tol = h->dtype == WAVE2D_F64 ? 1e-17 : 1e-8;   // rho^H <= tol: below half an ulp of T
+    const double tolp = h->dtype == WAVE2D_F64 ? 2e-15 : 1e-8;  // pivots count as stationary within a few ulp
+    double rho = 0.0;
+    int pconv = 0;   // rows [pconv, n) have stationary pivots (to tol) in every half-step
+    for (int n = d; n < 2 * h->M; n += 2) {
+        const double* row = &h->table[static_cast<size_t>(n) * ROW_DOUBLES];
+        rho = std::max(rho, row[ROW_RHO]);
+        int pc = KMAX + 1;
+        for (int p = KMAX - 1; p >= 0 && std::fabs(row[ROW_CP + p] - row[ROW_RHO]) <= tolp * row[ROW_RHO] &&
+                               std::fabs(row[ROW_INVP + p] - row[ROW_INV]) <= tolp * row[ROW_INV]; --p)
+            pc = p;
+        pconv = std::max(pconv, pc);
+    }
+    P.rho = rho;
+    int H = 1;
+    if (rho > 0.0) H = std::max(1, (int)std::ceil(std::log(tol) / std::log(rho)));
+    P.halo = H;
+    const int nbk = (H + U - 1) / U;
+    const bool fits = nbk <= std::min(NBK_MAX, V.nw) && pconv <= KMAX;
+    if (h->opt_solver == WAVE2D_SOLVER_EXACT || (h->opt_solver == WAVE2D_SOLVER_AUTO && !fits)) {
+        P.solver = WAVE2D_SOLVER_EXACT;
+        return WAVE2D_OK;
+    }
+    if (!fits) {
+        h->err = "streamed solver: decay bound rho^H <= tol needs a longer carry series than supported";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    P.solver = WAVE2D_SOLVER_STREAM;
+    P.nbk = nbk;
+    P.halo = nbk * U;
+    P.kb = (pconv + U - 1) / U;
     W2D_CUDA(h, cudaFuncSetAttribute(V.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, V.smem));
     int per_sm = 0;
     W2D_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, V.fn, V.threads, V.smem));
     if (per_sm < 1) {
-        h->err = "streamed kernel does not fit on an SM";
+        h->err = "sweep kernel does not fit on an SM";
         return WAVE2D_ERR_UNSUPPORTED;
     }
     P.ctas_per_sm = per_sm;
-    const int TL = 32 * V.nw;
-    P.ntiles = (P.nlines + TL - 1) / TL;
+    P.npanels = (P.nlines + 31) / 32;
     P.total_units = (P.n + U - 1) / U;
-    // One wave: as many chunks per line tile as resident CTA slots allow, but keep the halo (2 NB units of
-    // re-read per chunk) under ~25% of the chunk.
+    // Persistent grid, one wave: the smallest per-CTA quota of stages whose pieces fit the resident CTA slots.
     const int slots = per_sm * h->num_sms;
-    int q = std::max(1, slots / P.ntiles);
-    q = std::min(q, std::max(1, P.total_units / (8 * nb)));
-    if (h->opt_chunks[d] > 0) q = std::min(h->opt_chunks[d], std::max(1, P.total_units));
-    int upc = (P.total_units + q - 1) / q;
-    upc = (upc + V.xb - 1) / V.xb * V.xb;
-    P.upc = upc;
-    P.nchunks = (P.total_units + upc - 1) / upc;
-    P.grid = P.ntiles * P.nchunks;
+    const long long total = (long long)P.npanels * ((P.total_units + V.nw - 1) / V.nw);
+    int quota = (int)std::max<long long>(1, (total + slots - 1) / slots);
+    if (h->opt_quota[d] > 0) quota = h->opt_quota[d];
+    for (;; ++quota) {
+        if (!build_pieces(P, V.nw, quota)) continue;
+        if (h->opt_quota[d] > 0 || (int)P.cta_off.size() - 1 <= slots) break;
+    }
+    P.quota = quota;
+    P.grid = (int)P.cta_off.size() - 1;
     return WAVE2D_OK;
 }
 
@@ -312,20 +354,33 @@ int ensure_plan(wave2d_t* h)
         st = plan_dir(h, d);
         if (st) return st;
     }
-    const int U = 128 / h->elem;
     for (int b = 0; b < 3; ++b) {
-        for (int d = 0; d < 2; ++d) {
-            if (h->plan[d].solver != WAVE2D_SOLVER_STREAM) continue;
-            const Variant& V = *h->plan[d].var;
-            const int TL = 32 * V.nw;
-            st = d == 0 ? make_tmap(h, &h->tm_load[0][b], h->buf[b], U, TL, true)
-                        : make_tmap(h, &h->tm_load[1][b], h->buf[b], TL, U * V.xb, false);
-            if (st) return st;
-        }
         if (h->plan[0].solver == WAVE2D_SOLVER_STREAM) {
-            st = make_tmap(h, &h->tm_store[b], h->buf[b], U, 32, true);
+            const int U = h->plan[0].var->unit;
+            st = make_tmap(h, &h->tm_load[0][b], h->buf[b], U, 32, true);       // unit tile; also the store box
+            if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_edge[b], h->buf[b], 16 / h->elem, 32, false);
             if (st) return st;
         }
+        if (h->plan[1].solver == WAVE2D_SOLVER_STREAM) {
+            const Variant& V = *h->plan[1].var;
+            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32, V.unit * V.nw + 2, false);
+            if (st) return st;
+        }
+    }
+    for (int d = 0; d < 2; ++d) {
+        cudaFree(h->d_pieces[d]);
+        cudaFree(h->d_cta_off[d]);
+        h->d_pieces[d] = nullptr;
+        h->d_cta_off[d] = nullptr;
+        const DirPlan& P = h->plan[d];
+        if (P.solver != WAVE2D_SOLVER_STREAM) continue;
+        const size_t pb = std::max<size_t>(1, P.pieces.size()) * sizeof(Piece), ob = P.cta_off.size() * sizeof(int);
+        st = dev_alloc(h, reinterpret_cast<void**>(&h->d_pieces[d]), pb);
+        if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_cta_off[d]), ob);
+        if (st) return st;
+        if (!P.pieces.empty())
+            W2D_CUDA(h, cudaMemcpy(h->d_pieces[d], P.pieces.data(), P.pieces.size() * sizeof(Piece), cudaMemcpyHostToDevice));
+        W2D_CUDA(h, cudaMemcpy(h->d_cta_off[d], P.cta_off.data(), ob, cudaMemcpyHostToDevice));
     }
     if ((h->plan[0].solver == WAVE2D_SOLVER_EXACT || h->plan[1].solver == WAVE2D_SOLVER_EXACT) && !h->d_piv) {
         st = dev_alloc(h, reinterpret_cast<void**>(&h->d_piv), sizeof(double) * 2 * (size_t)std::max(h->n1, h->n2));
@@ -351,14 +406,17 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     if (P.solver == WAVE2D_SOLVER_STREAM) {
         SweepArgs a;
         a.table = h->d_table; a.d_k = dk; a.n_off = n_off;
-        a.n = P.n; a.nlines = P.nlines; a.ntiles = P.ntiles; a.upc = P.upc; a.total_units = P.total_units;
+        a.n = P.n; a.nlines = P.nlines; a.nbk = P.nbk; a.kb = P.kb;
+        a.pieces = h->d_pieces[d]; a.cta_off = h->d_cta_off[d];
         a.out = out; a.pitch = h->pitch;
         a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
         a.g2 = 2.0 * h->gamma;
         CUtensorMap* tp = &h->tm_load[d][n_abs % 3];
         CUtensorMap* tc = &h->tm_load[d][(n_abs + 1) % 3];
-        CUtensorMap* to = &h->tm_store[(n_abs + 2) % 3];   // unused by the y sweep
-        void* args[4] = {tp, tc, to, &a};
+        CUtensorMap* to = &h->tm_load[0][(n_abs + 2) % 3];   // x sweep: TMA store box; unused by the y sweep
+        CUtensorMap* te = &h->tm_edge[n_abs % 3];            // x sweep: neighbours of a stage in w_{n-1}
+        if (h->plan[0].solver != WAVE2D_SOLVER_STREAM) { to = tp; te = tp; }   // y sweep alone: placeholders
+        void* args[5] = {tp, tc, to, te, &a};
         W2D_CUDA(h, cudaLaunchKernel(P.var->fn, dim3(P.grid), dim3(P.var->threads), args, P.var->smem, h->stream));
         h->launches += 1;
         return WAVE2D_OK;
@@ -518,6 +576,10 @@ void wave2d_destroy(wave2d_t* h)
     cudaFree(h->d_table);
     cudaFree(h->d_k);
     cudaFree(h->d_piv);
+    for (int d = 0; d < 2; ++d) {
+        cudaFree(h->d_pieces[d]);
+        cudaFree(h->d_cta_off[d]);
+    }
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
     (void)cudaGetLastError();
     delete h;
@@ -544,8 +606,8 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "graph_steps")) { if (iv < 3 || iv % 3) return WAVE2D_ERR_ARG; h->opt_graph_steps = iv; }
     else if (!strcmp(name, "shape_x")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[0] = iv; }
     else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
-    else if (!strcmp(name, "chunks_x")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_chunks[0] = iv; }
-    else if (!strcmp(name, "chunks_y")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_chunks[1] = iv; }
+    else if (!strcmp(name, "quota_x")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[0] = iv; }
+    else if (!strcmp(name, "quota_y")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[1] = iv; }
     else return WAVE2D_ERR_ARG;
     invalidate_plan(h);
     return WAVE2D_OK;
@@ -721,13 +783,16 @@ int wave2d_get_info(wave2d_t* h, const char* name, double* value)
     if (key == "solver") *value = P.solver;
     else if (key == "halo") *value = P.halo;
     else if (key == "rho") *value = P.rho;
-    else if (key == "chunks") *value = stream ? P.nchunks : 1;
+    else if (key == "chunks") *value = stream ? (double)P.pieces.size() : 1;
+    else if (key == "nbk") *value = stream ? P.nbk : 0;
+    else if (key == "kb") *value = stream ? P.kb : 0;
     else if (key == "grid") *value = stream ? P.grid : (P.nlines + 127) / 128;
     else if (key == "ctas_per_sm") *value = stream ? P.ctas_per_sm : 0;
     else if (key == "smem") *value = stream ? P.var->smem : 0;
     else if (key == "threads") *value = stream ? P.var->threads : 128;
-    else if (key == "unit") *value = 128 / h->elem;
-    else if (key == "upc") *value = stream ? P.upc : 0;
+    else if (key == "unit") *value = stream ? P.var->unit : 0;
+    else if (key == "upc") *value = stream ? P.quota * P.var->nw : 0;
+    else if (key == "quota") *value = stream ? P.quota : 0;
     else return WAVE2D_ERR_ARG;
     return WAVE2D_OK;
 }

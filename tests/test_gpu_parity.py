@@ -23,6 +23,10 @@ def ref(w, steps=None, gamma=None, kappa=None):
 
 
 def gpu(w, steps=None, **opts):
+    return gpu_info(w, (), steps, **opts)
+
+
+def gpu_info(w, keys, steps=None, **opts):
     h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
     try:
         for k, v in opts.items():
@@ -34,7 +38,7 @@ def gpu(w, steps=None, **opts):
         h.set_initial(w.phi.astype(npdt), None if w.psi is None else w.psi.astype(npdt))
         h.run(w.M if steps is None else steps)
         u = h.get()
-        info = {k: h.info(k) for k in ("solver_x", "solver_y", "launches", "chunks_x", "chunks_y")}
+        info = {k: h.info(k) for k in ("solver_x", "solver_y", "launches", "chunks_x", "chunks_y") + tuple(keys)}
     finally:
         h.close()
     return u, info
@@ -60,9 +64,10 @@ def small_cases():
 
 
 @pytest.mark.parametrize("name,w", small_cases(), ids=[c[0] for c in small_cases()])
-@pytest.mark.parametrize("opts", [{}, {"solver": B.SOLVER_EXACT}, {"graph": 0}, {"chunks_x": 3, "chunks_y": 2},
-                                  {"shape_x": 2, "shape_y": 3}],
-                         ids=["default", "exact", "nograph", "chunks", "shapes"])
+@pytest.mark.parametrize("opts", [{}, {"solver": B.SOLVER_EXACT}, {"graph": 0}, {"quota_x": 3, "quota_y": 3},
+                                  {"shape_x": 1, "shape_y": 1, "quota_x": 4, "quota_y": 5},
+                                  {"shape_x": 2, "shape_y": 3}, {"shape_x": 3, "shape_y": 2}],
+                         ids=["default", "exact", "nograph", "quota3", "shapes1_cut", "shapes23", "shapes32"])
 def test_small_workloads_match_oracle(name, w, opts):
     r = ref(w)
     u, info = gpu(w, **opts)
@@ -119,17 +124,21 @@ def test_large_tau_falls_back_to_exact_solver():
     assert e.value.status == -5
 
 
-def test_moderate_tau_uses_wider_lookahead():
-    """tau = 2.3 h (alpha = 2.645, rho = 0.430): rho^H <= 1e-17 needs H = 47 points in fp64 -- the NB = 3
-    kernels (48 points of look-ahead).  tau = 2.5 h would need H = 51 and fall to the exact solver."""
-    N, M = 300, 10
+@pytest.mark.parametrize("ratio,nbk", [(2.3, 3), (4.0, 5), (6.0, 8)])
+def test_moderate_tau_uses_longer_carry_series(ratio, nbk):
+    """tau = 2.3 h / 4 h / 6 h (alpha = 2.6 / 8 / 18, rho = 0.43 / 0.61 / 0.72): rho^H <= 1e-17 needs
+    H = 47 / 79 / 120 points in fp64, i.e. a carry series of 3 / 5 / 8 units of 16 points (the kernels carry up
+    to 8); the boundary pivots still converge inside the 128-row table.  Cut lines (quota) exercise warm-up."""
+    N, M = 600, 8
     w = W.cfg2(N=N, M=M)
-    w.tau = 2.3 / N
+    w.tau = ratio / N
     w.c_half = np.ones(2 * M + 1)
     r = ref(w)
-    u, info = gpu(w)
-    assert info["solver_x"] == B.SOLVER_STREAM
-    assert relerr(u, r) <= 1e-10
+    for opts in ({}, {"quota_x": 4, "quota_y": 4}):
+        u, info = gpu_info(w, ("nbk_x", "nbk_y"), **opts)
+        assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
+        assert info["nbk_x"] == nbk and info["nbk_y"] == nbk
+        assert relerr(u, r) <= 1e-10
 
 
 def test_run_in_pieces_equals_one_run_and_reset_is_reproducible():
