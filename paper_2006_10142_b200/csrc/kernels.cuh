@@ -58,41 +58,57 @@ struct SweepArgs {
     double g2;             // 2 gamma
 };
 
-template <typename T, int DIR, int NW, int NSTAGE>
+// UT = points per thread ("unit"), NW = consumer warps = units per stage, NSTAGE = TMA stages in flight.
+template <typename T, int DIR, int UT, int NW, int NSTAGE>
 struct PanelCfg {
-    static constexpr int U = DIR == 0 ? 128 / (int)sizeof(T) : 16;   // points per unit
-    static constexpr int TL = 32;                                    // lines per panel, one per lane
-    static constexpr int V = 16 / (int)sizeof(T);                    // elements per 16 bytes
-    // x sweep: per field NW unit tiles [32 rows][128 B] (128B-swizzled) + two edge boxes [32 rows][16 B] of wp
+    static constexpr int U = UT;                                      // points per unit
+    static constexpr int TL = 32;                                     // lines per panel, one per lane
+    static constexpr int V = 16 / (int)sizeof(T);                     // elements per 16 bytes
+    static constexpr int TU = 128 / (int)sizeof(T);                   // x sweep: points per 128-byte load tile row
+    static constexpr int SUB = DIR == 0 ? TU / UT : 1;                // x sweep: units (warps) sharing a load tile
+    static constexpr int NT = NW / SUB;                               // x sweep: load tiles per stage and field
+    static constexpr int RB = UT * (int)sizeof(T);                    // x sweep: bytes per row of a warp's store tile
+    // x sweep: per field NT tiles [32 rows][128 B] (128B-swizzled) + two edge boxes [32 rows][16 B] of wp
     // y sweep: per field one box [U*NW + 2 rows][32 columns]
-    static constexpr int FIELD_BYTES = DIR == 0 ? NW * 4096 : (U * NW + 2) * TL * (int)sizeof(T);
+    static constexpr int FIELD_BYTES = DIR == 0 ? NT * 4096 : (U * NW + 2) * TL * (int)sizeof(T);
     static constexpr int EDGE_BYTES = DIR == 0 ? 512 : 0;
     static constexpr int STAGE_BYTES = 2 * FIELD_BYTES + 2 * EDGE_BYTES;
-    static constexpr int OUT_BYTES = DIR == 0 ? NW * 4096 : 0;
-    static constexpr int BAR_BYTES = ((2 * NSTAGE * 8) + 15) / 16 * 16;
+    static constexpr int OUT_BYTES = DIR == 0 ? NW * 32 * RB : 0;
+    static constexpr int BAR_BYTES = ((NSTAGE * 8) + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * KMAX * (int)sizeof(T);
-    static constexpr int XCH_BYTES = (4 * NW * TL + 2 * NW + 2) * (int)sizeof(T);   // Ls[2][NW][32], Hs[2][NW][32], As[2][NW]
+    static constexpr int XCH_BYTES = (4 * NW * TL + 2 * NW) * (int)sizeof(T);   // L[2NW][32], H[2NW][32], A[2NW]
     static constexpr int SMEM_BYTES = 1024 + NSTAGE * STAGE_BYTES + OUT_BYTES + BAR_BYTES + TAB_BYTES + XCH_BYTES;
-    static constexpr int THREADS = 32 * (NW + 1);
-    static_assert(FIELD_BYTES % 128 == 0, "TMA destinations must stay 128-byte aligned");
+    static constexpr int THREADS = 32 * NW;
+    static_assert((NW & (NW - 1)) == 0, "NW must be a power of two (ring indexing)");
+    static_assert(DIR == 1 || (TU % UT == 0 && NW % SUB == 0 && RB >= 32), "x sweep: units must tile the 128-byte row");
+    static_assert(FIELD_BYTES % 128 == 0 && (32 * RB) % 1024 == 0 || DIR == 1, "TMA smem alignment");
     static_assert(DIR == 0 || U * NW + 2 <= 256, "TMA box dimension limit");
 };
 
-// Read this lane's line of one x-sweep unit tile [32 rows][128 B] into registers; the tile is
-// 128B-swizzled by TMA: 16-byte chunk c of row t sits at chunk c ^ (t & 7)  (bank-conflict-free).
+// ---- x sweep shared-memory tiles ---------------------------------------------------------------------
+// Load tile [32 rows][128 B], 128B-swizzled by TMA: 16-byte chunk c of row t sits at chunk c ^ (t & 7).
 template <typename T>
-__device__ __forceinline__ void load_unit_x(const unsigned char* tile, int lane, T (&v)[128 / sizeof(T)])
+__device__ __forceinline__ T tile_elem_x(const unsigned char* tile, int lane, int idx)
 {
+    const int byte = idx * (int)sizeof(T);
+    return *reinterpret_cast<const T*>(tile + lane * 128 + ((((byte >> 4) ^ lane) & 7) << 4) + (byte & 15));
+}
+// this lane's UT points of sub-unit `sub` of its row
+template <typename T, int UT>
+__device__ __forceinline__ void load_unit_x(const unsigned char* tile, int lane, int sub, T (&v)[UT])
+{
+    constexpr int V = 16 / (int)sizeof(T), NC = UT / V;
     const unsigned char* row = tile + lane * 128;
-    const int sw = (lane & 7) << 4;
+    const int c0 = sub * NC;
 #pragma unroll
-    for (int c = 0; c < 8; ++c) {
+    for (int c = 0; c < NC; ++c) {
+        const unsigned char* p = row + ((((c0 + c) ^ lane) & 7) << 4);
         if constexpr (sizeof(T) == 8) {
-            const double2 t = *reinterpret_cast<const double2*>(row + ((c << 4) ^ sw));
+            const double2 t = *reinterpret_cast<const double2*>(p);
             v[2 * c] = t.x;
             v[2 * c + 1] = t.y;
         } else {
-            const float4 t = *reinterpret_cast<const float4*>(row + ((c << 4) ^ sw));
+            const float4 t = *reinterpret_cast<const float4*>(p);
             v[4 * c] = t.x;
             v[4 * c + 1] = t.y;
             v[4 * c + 2] = t.z;
@@ -100,16 +116,22 @@ __device__ __forceinline__ void load_unit_x(const unsigned char* tile, int lane,
         }
     }
 }
-// first / last element of this lane's row of an x-sweep unit tile
-template <typename T>
-__device__ __forceinline__ T tile_first_x(const unsigned char* tile, int lane)
+// Store tile of one warp, [32 rows][RB bytes], swizzled as TMA expects for a box of RB-byte rows
+// (128B / 64B / 32B mode: address bits [4,7) ^= bits [7,10), restricted to the row span).
+template <typename T, int UT>
+__device__ __forceinline__ void store_unit_x(unsigned char* tile, int lane, const T (&v)[UT])
 {
-    return *reinterpret_cast<const T*>(tile + lane * 128 + ((lane & 7) << 4));
-}
-template <typename T>
-__device__ __forceinline__ T tile_last_x(const unsigned char* tile, int lane)
-{
-    return *reinterpret_cast<const T*>(tile + lane * 128 + ((7 ^ (lane & 7)) << 4) + 16 - sizeof(T));
+    constexpr int V = 16 / (int)sizeof(T), NC = UT / V, RB = UT * (int)sizeof(T);
+    unsigned char* row = tile + lane * RB;
+    const int f = RB == 128 ? (lane & 7) : RB == 64 ? ((lane >> 1) & 3) : ((lane >> 2) & 1);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        unsigned char* p = row + ((c ^ f) << 4);
+        if constexpr (sizeof(T) == 8)
+            *reinterpret_cast<double2*>(p) = make_double2(v[2 * c], v[2 * c + 1]);
+        else
+            *reinterpret_cast<float4*>(p) = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+    }
 }
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
@@ -120,33 +142,33 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 // ---------------------------------------------------------------------------------------------------
 // Panel sweep: RHS assembly (A1/A3) fused with the line solve (A2/A4), SURVEY.md 8a.
 //   grid  = persistent CTAs (SM count x CTAs/SM); CTA b walks its host-planned pieces.
-//   block = NW consumer warps + 1 producer warp (one lane issues TMA).  Per stage, consumer warp w
-//           owns unit g = gbase + s*NW + w of the panel's 32 lines, lane = line.
-//   stage:  smem -> registers, release the slot; RHS + local forward; publish L, A; bar;
+//   block = NW warps.  Per stage, warp w owns unit g = gbase + s*NW + w (UT points) of the panel's 32
+//           lines, lane = line.  Thread 0 also feeds the ring of NSTAGE TMA stages.
+//   stage:  smem -> registers; RHS + local forward; publish L, A; bar (the slot is free: refill it);
 //           carry-in, correct y, local backward; publish head; bar;
-//           finish the unit of the PREVIOUS stage (its look-ahead heads are now known) and store it.
+//           warps whose look-ahead heads are all in this stage finish and store their unit now, the last
+//           few keep it one more stage ("deferred").
 // ---------------------------------------------------------------------------------------------------
-template <typename T, int DIR, int NW, int NSTAGE>
-__global__ void __launch_bounds__(32 * (NW + 1), 1)
+template <typename T, int DIR, int UT, int NW, int NSTAGE>
+__global__ void __launch_bounds__(32 * NW, 1)
 wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_constant__ CUtensorMap tm_cur,
                    const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_edge,
                    const SweepArgs a)
 {
-    using K = PanelCfg<T, DIR, NW, NSTAGE>;
-    constexpr int U = K::U, TL = K::TL, V = K::V;
+    using K = PanelCfg<T, DIR, UT, NW, NSTAGE>;
+    constexpr int U = UT, TL = K::TL, V = K::V, SUB = K::SUB, NT = K::NT, RING = 2 * NW;
 
     extern __shared__ unsigned char smem_raw[];
     const uint32_t raw32 = smem_u32(smem_raw);
     const uint32_t pad = ((raw32 + 1023u) & ~1023u) - raw32;
     unsigned char* sm = smem_raw + pad;   // 1024-byte aligned: the 128B-swizzle atom
     const uint32_t sm32 = raw32 + pad;
-    unsigned char* sm_out = sm + NSTAGE * K::STAGE_BYTES;
-    const uint32_t bar32 = sm32 + NSTAGE * K::STAGE_BYTES + K::OUT_BYTES;   // full[NSTAGE], empty[NSTAGE]
+    const uint32_t bar32 = sm32 + NSTAGE * K::STAGE_BYTES + K::OUT_BYTES;   // full[NSTAGE]
     T* s_cp = reinterpret_cast<T*>(sm + NSTAGE * K::STAGE_BYTES + K::OUT_BYTES + K::BAR_BYTES);
     T* s_inv = s_cp + KMAX;
-    T* s_L = s_inv + KMAX;            // [2][NW][32]  last local y of a unit
-    T* s_H = s_L + 2 * NW * TL;       // [2][NW][32]  first local x of a unit
-    T* s_A = s_H + 2 * NW * TL;       // [2][NW]      product of the unit's cp
+    T* s_L = s_inv + KMAX;           // [RING][32]  last local y of a unit
+    T* s_H = s_L + RING * TL;        // [RING][32]  first local x of a unit
+    T* s_A = s_H + RING * TL;        // [RING]      product of the unit's cp
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nh = a.n_off + (a.d_k ? 2 * (*a.d_k) : 0);
@@ -158,54 +180,53 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     }
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int s = 0; s < NSTAGE; ++s) {
-            mbar_init(bar32 + 8 * s, 1);
-            mbar_init(bar32 + 8 * (NSTAGE + s), NW);
-        }
+        for (int s = 0; s < NSTAGE; ++s) mbar_init(bar32 + 8 * s, 1);
         mbar_fence_init();
+        tma_prefetch_desc(&tm_prev);
+        tma_prefetch_desc(&tm_cur);
     }
     __syncthreads();
 
     const int pc_begin = a.cta_off[blockIdx.x], pc_end = a.cta_off[blockIdx.x + 1];
+    const int nbk = a.nbk, n = a.n;
 
-    if (warp == NW) {   // ---------------- producer: one lane feeds the stage ring by TMA
-        if (lane == 0) {
-            tma_prefetch_desc(&tm_prev);
-            tma_prefetch_desc(&tm_cur);
-            int it = 0;
-            for (int pi = pc_begin; pi < pc_end; ++pi) {
-                const Piece pc = a.pieces[pi];
-                const int line0 = pc.panel * TL;
-                const int gbase = max(pc.ua - a.nbk, 0);
-                for (int s = 0; s < pc.nst; ++s, ++it) {
-                    const int slot = it % NSTAGE;
-                    if (it >= NSTAGE) mbar_wait(bar32 + 8 * (NSTAGE + slot), ((it / NSTAGE) - 1) & 1);
-                    const uint32_t full = bar32 + 8 * slot;
-                    mbar_arrive_expect_tx(full, K::STAGE_BYTES);
-                    const uint32_t dst = sm32 + slot * K::STAGE_BYTES;
-                    const int g0 = gbase + s * NW;
-                    if constexpr (DIR == 0) {
+    // ---- producer cursor (thread 0 only): the next stage to request, NSTAGE ahead of the consumers
+    int q_pi = pc_begin, q_s = 0, q_slot = 0;
+    Piece q_pc = Piece{0, 0, 0, 0};
+    if (pc_begin < pc_end) q_pc = a.pieces[pc_begin];
+    auto produce = [&]() {   // thread 0: request the next stage into slot q_slot (which must be free)
+        if (q_pi >= pc_end) return;
+        const int line0 = q_pc.panel * TL;
+        const int g0 = (max(q_pc.ua - nbk, 0) & ~(SUB - 1)) + q_s * NW;
+        const uint32_t full = bar32 + 8 * q_slot;
+        const uint32_t dst = sm32 + q_slot * K::STAGE_BYTES;
+        mbar_arrive_expect_tx(full, K::STAGE_BYTES);
+        if constexpr (DIR == 0) {
 #pragma unroll
-                        for (int w = 0; w < NW; ++w) {
-                            tma_load_2d(dst + w * 4096, &tm_prev, (g0 + w) * U, line0, full);
-                            tma_load_2d(dst + K::FIELD_BYTES + w * 4096, &tm_cur, (g0 + w) * U, line0, full);
-                        }
-                        tma_load_2d(dst + 2 * K::FIELD_BYTES, &tm_edge, g0 * U - V, line0, full);
-                        tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
-                    } else {
-                        tma_load_2d(dst, &tm_prev, line0, g0 * U - 1, full);
-                        tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0, g0 * U - 1, full);
-                    }
-                }
+            for (int t = 0; t < NT; ++t) {
+                tma_load_2d(dst + t * 4096, &tm_prev, (g0 + t * SUB) * U, line0, full);
+                tma_load_2d(dst + K::FIELD_BYTES + t * 4096, &tm_cur, (g0 + t * SUB) * U, line0, full);
             }
+            tma_load_2d(dst + 2 * K::FIELD_BYTES, &tm_edge, g0 * U - V, line0, full);
+            tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
+        } else {
+            tma_load_2d(dst, &tm_prev, line0, g0 * U - 1, full);
+            tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0, g0 * U - 1, full);
         }
-        return;
+        q_slot = q_slot + 1 == NSTAGE ? 0 : q_slot + 1;
+        if (++q_s == q_pc.nst) {
+            q_s = 0;
+            if (++q_pi < pc_end) q_pc = a.pieces[q_pi];
+        }
+    };
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NSTAGE; ++s) produce();
     }
 
-    // -------------------- consumers
+    // ---- consumers (all warps)
     const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), rho = static_cast<T>(row[ROW_RHO]);
     const T inv = static_cast<T>(row[ROW_INV]), c1 = static_cast<T>(row[ROW_C1]), g2 = static_cast<T>(a.g2);
-    const int n = a.n, nbk = a.nbk;
     T pw[U];   // pw[e] = rho^(e+1)
     pw[0] = rho;
 #pragma unroll
@@ -213,176 +234,177 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     auto cp_at = [&](int p) -> T { return p < KMAX ? s_cp[p] : rho; };
     auto inv_at = [&](int p) -> T { return p < KMAX ? s_inv[p] : inv; };
 
+    // warps [0, wdef) finish their unit in the stage that computed it; warps [wdef, NW) one stage later
+    const int wdef = ((NW - nbk) / SUB) * SUB;
+    const bool deferred = warp >= wdef;
+    [[maybe_unused]] unsigned char* my_out = sm + NSTAGE * K::STAGE_BYTES + warp * (32 * K::RB);
+    [[maybe_unused]] const int sub = warp % SUB, tix = warp / SUB;
+
+    // finish unit gp (local x in v[]): add the carry from the right, store
+    auto finish = [&](T (&v)[U], int gp, int ring, const Piece& pc) {
+        T Xin = T(0);   // x at the start of unit gp+1
+        for (int j = nbk; j >= 1; --j) {
+            const int idx = (ring + j) & (RING - 1);
+            Xin = fma(s_A[idx], Xin, s_H[idx * TL + lane]);
+        }
+        if (gp < pc.ua || gp >= pc.ub) return;   // warp-uniform
+        const int pp0 = gp * U;
+        if (gp >= a.kb && pp0 + U <= n) {
+#pragma unroll
+            for (int e = 0; e < U; ++e) v[e] = fma(pw[U - 1 - e], Xin, v[e]);
+        } else {
+            T c = Xin;
+#pragma unroll
+            for (int e = U - 1; e >= 0; --e) {
+                c *= cp_at(pp0 + e);
+                v[e] += c;
+            }
+        }
+        const int line0 = pc.panel * TL;
+        if constexpr (DIR == 0) {
+            if (lane == 0) tma_wait_read<0>();   // the previous store of this warp has read the tile
+            __syncwarp();
+            store_unit_x<T, U>(my_out, lane, v);
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+                tma_store_2d(&tm_out, pp0, line0, smem_u32(my_out));
+                tma_commit();
+            }
+        } else {
+            const int line = line0 + lane;
+            if (line < a.nlines) {
+                T* o = reinterpret_cast<T*>(a.out) + static_cast<long long>(pp0) * a.pitch + line;
+#pragma unroll
+                for (int e = 0; e < U; ++e)
+                    if (pp0 + e < n) o[static_cast<long long>(e) * a.pitch] = v[e];
+            }
+        }
+    };
+
     T pend[U];
 #pragma unroll
     for (int e = 0; e < U; ++e) pend[e] = T(0);
-    int it = 0;
+    int slot = 0, phase = 0;
 
     for (int pi = pc_begin; pi < pc_end; ++pi) {
         const Piece pc = a.pieces[pi];
         const int line0 = pc.panel * TL, line = line0 + lane;
-        const int gbase = max(pc.ua - nbk, 0);
+        const int gbase = max(pc.ua - nbk, 0) & ~(SUB - 1);
         const bool src_tile = a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
         const bool src_line = line >= a.sl0 && line < a.sl0 + a.snl;
         const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
 
-        named_bar_sync(1, NW * 32);   // the previous piece is completely finished
+        __syncthreads();   // the previous piece is completely finished
         s_L[(NW + warp) * TL + lane] = T(0);   // "stage -1": zero carries
         if (lane == 0) s_A[NW + warp] = T(0);
 
-        for (int s = 0; s <= pc.nst; ++s) {
-            const int buf = s & 1;
+        for (int s = 0; s < pc.nst; ++s) {
+            const int ring = (s & 1) * NW + warp;
             const int g = gbase + s * NW + warp, p0 = g * U;
-            const bool act = s < pc.nst;
-            bool fast = false;
             T xl[U];
+            // ---- shared memory -> registers
+            mbar_wait(bar32 + 8 * slot, phase);
+            const unsigned char* st = sm + slot * K::STAGE_BYTES;
+            if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
+            T wp[U], wc[U], wl, wr;
+            if constexpr (DIR == 0) {
+                const unsigned char* tp = st + tix * 4096;
+                load_unit_x<T, U>(tp, lane, sub, wp);
+                load_unit_x<T, U>(tp + K::FIELD_BYTES, lane, sub, wc);
+                if (sub > 0) wl = tile_elem_x<T>(tp, lane, sub * U - 1);
+                else if (tix > 0) wl = tile_elem_x<T>(tp - 4096, lane, K::TU - 1);
+                else wl = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES)[lane * V + V - 1];
+                if (sub < SUB - 1) wr = tile_elem_x<T>(tp, lane, (sub + 1) * U);
+                else if (tix < NT - 1) wr = tile_elem_x<T>(tp + 4096, lane, 0);
+                else wr = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V];
+            } else {
+                const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
+                const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
+                wl = cpv[0];
 #pragma unroll
-            for (int e = 0; e < U; ++e) xl[e] = T(0);
-
-            if (act) {
-                const int slot = it % NSTAGE;
-                mbar_wait(bar32 + 8 * slot, (it / NSTAGE) & 1);
-                ++it;
-                const unsigned char* st = sm + slot * K::STAGE_BYTES;
-                T wp[U], wc[U], wl, wr;
-                if constexpr (DIR == 0) {
-                    const unsigned char* tp = st + warp * 4096;
-                    load_unit_x<T>(tp, lane, wp);
-                    load_unit_x<T>(st + K::FIELD_BYTES + warp * 4096, lane, wc);
-                    wl = warp == 0 ? reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES)[lane * V + V - 1]
-                                   : tile_last_x<T>(tp - 4096, lane);
-                    wr = warp == NW - 1 ? reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V]
-                                        : tile_first_x<T>(tp + 4096, lane);
-                } else {
-                    const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
-                    const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
-                    wl = cpv[0];
+                for (int e = 0; e < U; ++e) wp[e] = cpv[(e + 1) * TL];
+                wr = cpv[(U + 1) * TL];
 #pragma unroll
-                    for (int e = 0; e < U; ++e) wp[e] = cpv[(e + 1) * TL];
-                    wr = cpv[(U + 1) * TL];
-#pragma unroll
-                    for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar32 + 8 * (NSTAGE + slot));   // data is in registers: release the slot
-
-                const bool src_k = src_tile && p0 < a.sp0 + a.snp && p0 + U > a.sp0;
-                fast = g >= a.kb && p0 + U <= n && !src_k;
-                T Aval;
-                if (fast) {   // stationary pivots: y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
-                    T fy = T(0);
-#pragma unroll
-                    for (int e = 0; e < U; ++e) {
-                        const T left = e == 0 ? wl : wp[e - 1];
-                        const T right = e == U - 1 ? wr : wp[e + 1];
-                        const T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
-                        fy = fma(rho, fy, r * inv);
-                        xl[e] = fy;
-                    }
-                    Aval = pw[U - 1];
-                } else {
-                    const bool src_unit = src_k && src_line;
-                    T fy = T(0), prod = T(1);
-#pragma unroll
-                    for (int e = 0; e < U; ++e) {
-                        const int p = p0 + e;
-                        const T left = e == 0 ? wl : wp[e - 1];
-                        const T right = e == U - 1 ? wr : wp[e + 1];
-                        T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
-                        if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
-                            r = fma(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
-                        const T cpe = cp_at(p);
-                        fy = fma(cpe, fy, r * inv_at(p));
-                        if (p >= n) fy = T(0);
-                        prod *= cpe;
-                        xl[e] = fy;
-                    }
-                    Aval = prod;
-                }
-                s_L[(buf * NW + warp) * TL + lane] = xl[U - 1];
-                if (lane == 0) s_A[buf * NW + warp] = Aval;
+                for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
             }
+            // ---- RHS + local forward elimination
+            const bool src_k = src_tile && p0 < a.sp0 + a.snp && p0 + U > a.sp0;
+            const bool fast = g >= a.kb && p0 + U <= n && !src_k;
+            T Aval;
+            if (fast) {   // stationary pivots: y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
+                T fy = T(0);
+#pragma unroll
+                for (int e = 0; e < U; ++e) {
+                    const T left = e == 0 ? wl : wp[e - 1];
+                    const T right = e == U - 1 ? wr : wp[e + 1];
+                    const T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                    fy = fma(rho, fy, r * inv);
+                    xl[e] = fy;
+                }
+                Aval = pw[U - 1];
+            } else {
+                const bool src_unit = src_k && src_line;
+                T fy = T(0), prod = T(1);
+#pragma unroll
+                for (int e = 0; e < U; ++e) {
+                    const int p = p0 + e;
+                    const T left = e == 0 ? wl : wp[e - 1];
+                    const T right = e == U - 1 ? wr : wp[e + 1];
+                    T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                    if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
+                        r = fma(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
+                    const T cpe = cp_at(p);
+                    fy = fma(cpe, fy, r * inv_at(p));
+                    if (p >= n) fy = T(0);
+                    prod *= cpe;
+                    xl[e] = fy;
+                }
+                Aval = prod;
+            }
+            s_L[ring * TL + lane] = xl[U - 1];
+            if (lane == 0) s_A[ring] = Aval;
+            named_bar_sync(1, NW * 32);
+            if (threadIdx.x == 0) produce();   // every warp holds its stage data in registers: refill the slot
+
+            // ---- carry from the left, local back substitution
+            T Yin = T(0);   // y at the end of unit g-1
+            for (int j = nbk; j >= 1; --j) {
+                const int idx = (ring - j) & (RING - 1);
+                Yin = fma(s_A[idx], Yin, s_L[idx * TL + lane]);
+            }
+            if (fast) {
+#pragma unroll
+                for (int e = 0; e < U; ++e) xl[e] = fma(pw[e], Yin, xl[e]);
+#pragma unroll
+                for (int e = U - 2; e >= 0; --e) xl[e] = fma(rho, xl[e + 1], xl[e]);
+            } else {
+                T c = Yin;
+#pragma unroll
+                for (int e = 0; e < U; ++e) {
+                    c *= cp_at(p0 + e);
+                    xl[e] = p0 + e < n ? xl[e] + c : T(0);
+                }
+#pragma unroll
+                for (int e = U - 2; e >= 0; --e) xl[e] = fma(cp_at(p0 + e), xl[e + 1], xl[e]);
+            }
+            s_H[ring * TL + lane] = xl[0];
             named_bar_sync(1, NW * 32);
 
-            if (act) {
-                T Yin = T(0);   // y at the end of unit g-1
-                for (int j = nbk; j >= 1; --j) {
-                    int idx = warp - j, b = buf;
-                    if (idx < 0) { idx += NW; b ^= 1; }
-                    Yin = fma(s_A[b * NW + idx], Yin, s_L[(b * NW + idx) * TL + lane]);
-                }
-                if (fast) {
+            // ---- carry from the right, store
+            if (deferred) {
+                if (s > 0) finish(pend, g - NW, ring ^ NW, pc);
 #pragma unroll
-                    for (int e = 0; e < U; ++e) xl[e] = fma(pw[e], Yin, xl[e]);
-#pragma unroll
-                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(rho, xl[e + 1], xl[e]);
-                } else {
-                    T c = Yin;
-#pragma unroll
-                    for (int e = 0; e < U; ++e) {
-                        c *= cp_at(p0 + e);
-                        xl[e] = p0 + e < n ? xl[e] + c : T(0);
-                    }
-#pragma unroll
-                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(cp_at(p0 + e), xl[e + 1], xl[e]);
-                }
+                for (int e = 0; e < U; ++e) pend[e] = xl[e];
+            } else {
+                finish(xl, g, ring, pc);
             }
-            s_H[(buf * NW + warp) * TL + lane] = xl[0];   // 0 in the flush stage
-            named_bar_sync(1, NW * 32);
-
-            if (s > 0) {   // finish the unit of stage s-1: gp = g - NW, local x in pend[]
-                const int gp = g - NW, pp0 = gp * U;
-                T Xin = T(0);   // x at the start of unit gp+1
-                for (int j = nbk; j >= 1; --j) {
-                    int idx = warp + j, b = buf ^ 1;
-                    if (idx >= NW) { idx -= NW; b ^= 1; }
-                    Xin = fma(s_A[b * NW + idx], Xin, s_H[(b * NW + idx) * TL + lane]);
-                }
-                if (gp >= pc.ua && gp < pc.ub) {   // warp-uniform
-                    if (gp >= a.kb && pp0 + U <= n) {
-#pragma unroll
-                        for (int e = 0; e < U; ++e) pend[e] = fma(pw[U - 1 - e], Xin, pend[e]);
-                    } else {
-                        T c = Xin;
-#pragma unroll
-                        for (int e = U - 1; e >= 0; --e) {
-                            c *= cp_at(pp0 + e);
-                            pend[e] += c;
-                        }
-                    }
-                    if constexpr (DIR == 0) {
-                        unsigned char* ot = sm_out + warp * 4096;
-                        if (lane == 0) tma_wait_read<0>();   // the previous store of this warp has read the tile
-                        __syncwarp();
-                        unsigned char* orow = ot + lane * 128;
-                        const int sw = (lane & 7) << 4;
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) {
-                            if constexpr (sizeof(T) == 8)
-                                *reinterpret_cast<double2*>(orow + ((c << 4) ^ sw)) = make_double2(pend[2 * c], pend[2 * c + 1]);
-                            else
-                                *reinterpret_cast<float4*>(orow + ((c << 4) ^ sw)) =
-                                    make_float4(pend[4 * c], pend[4 * c + 1], pend[4 * c + 2], pend[4 * c + 3]);
-                        }
-                        fence_async_smem();
-                        __syncwarp();
-                        if (lane == 0) {
-                            tma_store_2d(&tm_out, pp0, line0, smem_u32(ot));
-                            tma_commit();
-                        }
-                    } else {
-                        if (line < a.nlines) {
-                            T* o = reinterpret_cast<T*>(a.out) + static_cast<long long>(pp0) * a.pitch + line;
-#pragma unroll
-                            for (int e = 0; e < U; ++e)
-                                if (pp0 + e < n) o[static_cast<long long>(e) * a.pitch] = pend[e];
-                        }
-                    }
-                }
-            }
-#pragma unroll
-            for (int e = 0; e < U; ++e) pend[e] = xl[e];
         }
+        // ---- flush: the deferred units of the last stage see zero heads beyond it
+        const int ringf = (pc.nst & 1) * NW + warp;
+        s_H[ringf * TL + lane] = T(0);
+        named_bar_sync(1, NW * 32);
+        if (deferred && pc.nst > 0) finish(pend, gbase + (pc.nst - 1) * NW + warp, ringf ^ NW, pc);
     }
     if constexpr (DIR == 0) {
         if (lane == 0) tma_wait_read<0>();

@@ -24,38 +24,48 @@ namespace {
 // Kernel variants: (NW consumer warps = units per stage, NSTAGE) per dtype and direction.
 // ------------------------------------------------------------------------------------------------
 struct Variant {
-    int dir, nw, nstage, unit, smem, threads, elem;   // elem = sizeof(T), unit = points per unit
+    int dir, nw, nstage, unit, sub, smem, threads, elem;   // elem = sizeof(T), unit = points per thread
     const void* fn;
 };
 
-template <typename T, int DIR, int NW, int NSTAGE>
+template <typename T, int DIR, int UT, int NW, int NSTAGE>
 Variant make_variant()
 {
-    using K = PanelCfg<T, DIR, NW, NSTAGE>;
-    return Variant{DIR, NW, NSTAGE, K::U, K::SMEM_BYTES, K::THREADS, (int)sizeof(T),
-                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, NW, NSTAGE>)};
+    using K = PanelCfg<T, DIR, UT, NW, NSTAGE>;
+    return Variant{DIR, NW, NSTAGE, UT, K::SUB, K::SMEM_BYTES, K::THREADS, (int)sizeof(T),
+                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE>)};
 }
 
 constexpr int NVAR = 4;   // shape variants per (dtype, dir); index 0 is the default
-template <typename T>
-void add_shapes(std::vector<Variant>& v)
+void add_shapes_f64(std::vector<Variant>& v)
 {
-    v.push_back(make_variant<T, 0, 8, 2>());
-    v.push_back(make_variant<T, 0, 4, 3>());
-    v.push_back(make_variant<T, 0, 4, 2>());
-    v.push_back(make_variant<T, 0, 6, 2>());
-    v.push_back(make_variant<T, 1, 8, 3>());
-    v.push_back(make_variant<T, 1, 4, 3>());
-    v.push_back(make_variant<T, 1, 8, 2>());
-    v.push_back(make_variant<T, 1, 4, 4>());
+    v.push_back(make_variant<double, 0, 8, 16, 2>());
+    v.push_back(make_variant<double, 0, 8, 8, 3>());
+    v.push_back(make_variant<double, 0, 16, 8, 2>());
+    v.push_back(make_variant<double, 0, 4, 16, 2>());
+    v.push_back(make_variant<double, 1, 8, 16, 3>());
+    v.push_back(make_variant<double, 1, 8, 8, 3>());
+    v.push_back(make_variant<double, 1, 16, 8, 3>());
+    v.push_back(make_variant<double, 1, 8, 16, 2>());
+}
+void add_shapes_f32(std::vector<Variant>& v)
+{
+    v.push_back(make_variant<float, 0, 16, 16, 2>());
+    v.push_back(make_variant<float, 0, 8, 16, 2>());
+    v.push_back(make_variant<float, 0, 32, 8, 2>());
+    v.push_back(make_variant<float, 0, 16, 8, 3>());
+    v.push_back(make_variant<float, 1, 8, 16, 3>());
+    v.push_back(make_variant<float, 1, 8, 8, 3>());
+    v.push_back(make_variant<float, 1, 16, 8, 3>());
+    v.push_back(make_variant<float, 1, 8, 16, 4>());
 }
 
 const std::vector<Variant>& variants()
 {
     static std::vector<Variant> v = [] {
         std::vector<Variant> w;
-        add_shapes<double>(w);
-        add_shapes<float>(w);
+        add_shapes_f64(w);
+        add_shapes_f32(w);
         return w;
     }();
     return v;
@@ -121,7 +131,7 @@ struct wave2d_s {
     double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
     bool plan_ok = false;
     DirPlan plan[2];
-    CUtensorMap tm_load[2][3], tm_edge[3];    // [dir][buffer]; x: unit tile (load and store) + 16-byte edge box
+    CUtensorMap tm_load[2][3], tm_store[3], tm_edge[3];   // [dir][buffer]; x: load tile, store tile, 16-byte edge box
     Piece* d_pieces[2] = {nullptr, nullptr};
     int* d_cta_off[2] = {nullptr, nullptr};
     cudaGraphExec_t gexec = nullptr;
@@ -203,7 +213,8 @@ void build_table(wave2d_t* h)
     }
 }
 
-int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, bool swizzle)
+// swizzle: 0 (none) or the row span in bytes of the swizzle mode (32 / 64 / 128)
+int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, int swizzle)
 {
     EncodeTiledFn enc = encode_tiled();
     if (!enc) {
@@ -216,7 +227,8 @@ int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, bool
     const cuuint32_t es[2] = {1, 1};
     CUresult r = enc(tm, h->dtype == WAVE2D_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
                      base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                     swizzle == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                     : swizzle == 32 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE,
                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         char msg[160];
@@ -230,7 +242,7 @@ int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, bool
 
 // Cut the (panel, unit) space into pieces, `quota` stages per CTA.  A cut costs 2 nbk extra units (carry warm-up
 // before the cut, look-ahead after it).  Returns false if a CTA could make no progress (quota too small).
-bool build_pieces(DirPlan& P, int nw, int quota)
+bool build_pieces(DirPlan& P, int nw, int sub, int quota)
 {
     P.pieces.clear();
     P.cta_off.assign(1, 0);
@@ -239,7 +251,7 @@ bool build_pieces(DirPlan& P, int nw, int quota)
     while (panel < P.npanels) {
         int left = quota;
         while (left > 0 && panel < P.npanels) {
-            const int ua0 = std::max(ua - P.nbk, 0);
+            const int ua0 = std::max(ua - P.nbk, 0) / sub * sub;   // stages start on a load-tile boundary
             const int rest = (UT - ua0 + nw - 1) / nw;
             if (rest <= left) {
                 P.pieces.push_back(Piece{panel, ua, UT, rest});
@@ -323,7 +335,7 @@ int plan_dir(wave2d_t* h, int d)
     int quota = (int)std::max<long long>(1, (total + slots - 1) / slots);
     if (h->opt_quota[d] > 0) quota = h->opt_quota[d];
     for (;; ++quota) {
-        if (!build_pieces(P, V.nw, quota)) continue;
+        if (!build_pieces(P, V.nw, V.sub, quota)) continue;
         if (h->opt_quota[d] > 0 || (int)P.cta_off.size() - 1 <= slots) break;
     }
     P.quota = quota;
@@ -357,13 +369,14 @@ int ensure_plan(wave2d_t* h)
     for (int b = 0; b < 3; ++b) {
         if (h->plan[0].solver == WAVE2D_SOLVER_STREAM) {
             const int U = h->plan[0].var->unit;
-            st = make_tmap(h, &h->tm_load[0][b], h->buf[b], U, 32, true);       // unit tile; also the store box
-            if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_edge[b], h->buf[b], 16 / h->elem, 32, false);
+            st = make_tmap(h, &h->tm_load[0][b], h->buf[b], 128 / h->elem, 32, 128);   // load tile: 128-byte rows
+            if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_store[b], h->buf[b], U, 32, U * h->elem);   // one warp's unit
+            if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_edge[b], h->buf[b], 16 / h->elem, 32, 0);
             if (st) return st;
         }
         if (h->plan[1].solver == WAVE2D_SOLVER_STREAM) {
             const Variant& V = *h->plan[1].var;
-            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32, V.unit * V.nw + 2, false);
+            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32, V.unit * V.nw + 2, 0);
             if (st) return st;
         }
     }
@@ -413,7 +426,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         a.g2 = 2.0 * h->gamma;
         CUtensorMap* tp = &h->tm_load[d][n_abs % 3];
         CUtensorMap* tc = &h->tm_load[d][(n_abs + 1) % 3];
-        CUtensorMap* to = &h->tm_load[0][(n_abs + 2) % 3];   // x sweep: TMA store box; unused by the y sweep
+        CUtensorMap* to = &h->tm_store[(n_abs + 2) % 3];     // x sweep: TMA store box; unused by the y sweep
         CUtensorMap* te = &h->tm_edge[n_abs % 3];            // x sweep: neighbours of a stage in w_{n-1}
         if (h->plan[0].solver != WAVE2D_SOLVER_STREAM) { to = tp; te = tp; }   // y sweep alone: placeholders
         void* args[5] = {tp, tc, to, te, &a};

@@ -124,20 +124,20 @@ def test_large_tau_falls_back_to_exact_solver():
     assert e.value.status == -5
 
 
-@pytest.mark.parametrize("ratio,nbk", [(2.3, 3), (4.0, 5), (6.0, 8)])
-def test_moderate_tau_uses_longer_carry_series(ratio, nbk):
-    """tau = 2.3 h / 4 h / 6 h (alpha = 2.6 / 8 / 18, rho = 0.43 / 0.61 / 0.72): rho^H <= 1e-17 needs
-    H = 47 / 79 / 120 points in fp64, i.e. a carry series of 3 / 5 / 8 units of 16 points (the kernels carry up
-    to 8); the boundary pivots still converge inside the 128-row table.  Cut lines (quota) exercise warm-up."""
+@pytest.mark.parametrize("ratio,H", [(2.3, 47), (3.0, 60)])
+def test_moderate_tau_uses_longer_carry_series(ratio, H):
+    """tau = 2.3 h / 3 h (alpha = 2.6 / 4.5, rho = 0.43 / 0.52): rho^H <= 1e-17 needs H = 47 / 60 points in
+    fp64, i.e. a carry series of 6 / 8 units of 8 points (the kernels carry up to 8 units); the boundary pivots
+    still converge inside the 128-row table.  Cut lines (quota) exercise the carry warm-up."""
     N, M = 600, 8
     w = W.cfg2(N=N, M=M)
     w.tau = ratio / N
     w.c_half = np.ones(2 * M + 1)
     r = ref(w)
     for opts in ({}, {"quota_x": 4, "quota_y": 4}):
-        u, info = gpu_info(w, ("nbk_x", "nbk_y"), **opts)
+        u, info = gpu_info(w, ("nbk_x", "nbk_y", "unit_x", "unit_y"), **opts)
         assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
-        assert info["nbk_x"] == nbk and info["nbk_y"] == nbk
+        assert info["nbk_x"] == -(-H // info["unit_x"]) and info["nbk_y"] == -(-H // info["unit_y"])
         assert relerr(u, r) <= 1e-10
 
 
