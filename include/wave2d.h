@@ -90,6 +90,7 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "graph"  1 (default): the step loop is replayed as a CUDA Graph; 0: plain launches.
  *   "graph_steps"  time steps per graph replay (multiple of 3, the period of the buffer ring).  Default 12.
  *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (units per stage = consumer warps / stages).
+ *   "trace"  1: sweep kernels record per-CTA timing (see wave2d_get_trace).  Default 0.
  *   "quota_x", "quota_y"   tuning: stages of work per CTA (0 = planned: one wave over the resident CTA slots);
  *                          lines are cut where a CTA's quota ends.
  * Errors: ERR_ARG (unknown name / bad value), ERR_STATE.
@@ -155,6 +156,17 @@ int wave2d_get_info(wave2d_t *h, const char *name, double *value);
  * y-sweep kernels.  Synchronous.  Counts toward the step total like wave2d_run.
  */
 int wave2d_profile_sweeps(wave2d_t *h, int steps, double *ms_x, double *ms_y);
+
+/*
+ * Tracing (option "trace" = 1, before the first run): every CTA of a sweep kernel records its start and end
+ * time (GPU global timer, ns), the SM it ran on and the cycles its first warp spent waiting for TMA data.
+ * Copies the records of the most recent launch of direction dir (0 = x, 1 = y) to the host array
+ * out[16 * capacity], 16 values per CTA: start_ns, end_ns, sm_id, wait_cycles, then for the first and for
+ * the last warp six cycle counters each (wait for data; load + forward; barrier 1; carry + backward;
+ * barrier 2; finish + store); *count = CTAs in the grid.
+ * Errors: ERR_ARG (capacity < *count), ERR_STATE (tracing off or nothing planned).  Synchronises the stream.
+ */
+int wave2d_get_trace(wave2d_t *h, int dir, unsigned long long *out, int capacity, int *count);
 
 const char *wave2d_strerror(int status);
 const char *wave2d_last_error(const wave2d_t *h);

@@ -20,8 +20,8 @@ SOLVER_AUTO, SOLVER_EXACT, SOLVER_STREAM = 0, 1, 2
 EXPORTS = [
     "wave2d_create", "wave2d_destroy", "wave2d_set_stream", "wave2d_set_option", "wave2d_set_initial",
     "wave2d_set_speed", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
-    "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_strerror",
-    "wave2d_last_error",
+    "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
+    "wave2d_strerror", "wave2d_last_error",
 ]
 
 
@@ -61,6 +61,7 @@ def load_library() -> C.CDLL:
     L.wave2d_sync.argtypes = [vp]
     L.wave2d_get_info.argtypes = [vp, C.c_char_p, dp]
     L.wave2d_profile_sweeps.argtypes = [vp, C.c_int, dp, dp]
+    L.wave2d_get_trace.argtypes = [vp, C.c_int, vp, C.c_int, C.POINTER(C.c_int)]
     L.wave2d_strerror.argtypes = [C.c_int]
     L.wave2d_strerror.restype = C.c_char_p
     L.wave2d_last_error.argtypes = [vp]
@@ -197,6 +198,15 @@ class Wave2D:
         v = C.c_double()
         self._check(self._L.wave2d_get_info(self._h, name.encode(), C.byref(v)), "wave2d_get_info")
         return v.value
+
+    def trace(self, direction: int) -> np.ndarray:
+        """Per-CTA records of the last launch of a direction: 16 uint64 per CTA (include/wave2d.h)."""
+        cap = 4096
+        buf = np.zeros((cap, 16), dtype=np.uint64)
+        cnt = C.c_int()
+        self._check(self._L.wave2d_get_trace(self._h, int(direction), buf.ctypes.data_as(C.c_void_p), cap,
+                                             C.byref(cnt)), "wave2d_get_trace")
+        return buf[:cnt.value]
 
     def profile_sweeps(self, steps: int):
         a, b = C.c_double(), C.c_double()

@@ -56,6 +56,7 @@ struct SweepArgs {
     const void* src;       // compact source window, [p - sp0][line - sl0] (line fastest), or NULL
     int sl0, snl, sp0, snp;
     double g2;             // 2 gamma
+    unsigned long long* trace;   // NULL, or [grid][16]: CTA start ns, end ns, SM id, wait cycles, phase cycles of the first and last warp
 };
 
 // UT = points per thread ("unit"), NW = consumer warps = units per stage, NSTAGE = TMA stages in flight.
@@ -73,7 +74,7 @@ struct PanelCfg {
     static constexpr int FIELD_BYTES = DIR == 0 ? NT * 4096 : (U * NW + 2) * TL * (int)sizeof(T);
     static constexpr int EDGE_BYTES = DIR == 0 ? 512 : 0;
     static constexpr int STAGE_BYTES = 2 * FIELD_BYTES + 2 * EDGE_BYTES;
-    static constexpr int OUT_BYTES = DIR == 0 ? NW * 32 * RB : 0;
+    static constexpr int OUT_BYTES = DIR == 0 ? NW * 2 * 32 * RB : 0;   // two store tiles per warp
     static constexpr int BAR_BYTES = ((NSTAGE * 8) + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * KMAX * (int)sizeof(T);
     static constexpr int XCH_BYTES = (4 * NW * TL + 2 * NW) * (int)sizeof(T);   // L[2NW][32], H[2NW][32], A[2NW]
@@ -149,8 +150,8 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 //           warps whose look-ahead heads are all in this stage finish and store their unit now, the last
 //           few keep it one more stage ("deferred").
 // ---------------------------------------------------------------------------------------------------
-template <typename T, int DIR, int UT, int NW, int NSTAGE>
-__global__ void __launch_bounds__(32 * NW, 1)
+template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB>
+__global__ void __launch_bounds__(32 * NW, MINB)
 wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_constant__ CUtensorMap tm_cur,
                    const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_edge,
                    const SweepArgs a)
@@ -188,30 +189,49 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     __syncthreads();
 
     const int pc_begin = a.cta_off[blockIdx.x], pc_end = a.cta_off[blockIdx.x + 1];
-    const int nbk = a.nbk, n = a.n;
+    const int nbk = a.nbk, n = a.n, kb = a.kb, nlines = a.nlines;
+    const long long pitch = a.pitch;
+    [[maybe_unused]] T* const out_lane = reinterpret_cast<T*>(a.out) + (threadIdx.x & 31);
+    unsigned long long t_start = 0;
+    long long t_ph[6] = {0, 0, 0, 0, 0, 0}, t_last = 0;
+    const bool tracing = a.trace != nullptr && lane == 0 && (warp == 0 || warp == NW - 1);
+    auto tick = [&](int k) {
+        if (tracing) {
+            const long long c = clock64();
+            t_ph[k] += c - t_last;
+            t_last = c;
+        }
+    };
+    if (a.trace && threadIdx.x == 0) t_start = globaltimer_ns();
 
-    // ---- producer cursor (thread 0 only): the next stage to request, NSTAGE ahead of the consumers
+    // ---- producer cursor (kept by every thread): the next stage to request, NSTAGE ahead of the consumers.
+    // The TMA requests of a stage are spread over the warps (lane 0 of each issues its own tile), so that no
+    // warp is late at the next barrier; thread 0 posts the stage's byte count on the mbarrier.
+    const int sub = DIR == 0 ? warp % SUB : 0, tix = DIR == 0 ? warp / SUB : warp;
     int q_pi = pc_begin, q_s = 0, q_slot = 0;
     Piece q_pc = Piece{0, 0, 0, 0};
     if (pc_begin < pc_end) q_pc = a.pieces[pc_begin];
-    auto produce = [&]() {   // thread 0: request the next stage into slot q_slot (which must be free)
+    auto produce = [&]() {   // request the next stage into slot q_slot (which must be free)
         if (q_pi >= pc_end) return;
-        const int line0 = q_pc.panel * TL;
-        const int g0 = (max(q_pc.ua - nbk, 0) & ~(SUB - 1)) + q_s * NW;
-        const uint32_t full = bar32 + 8 * q_slot;
-        const uint32_t dst = sm32 + q_slot * K::STAGE_BYTES;
-        mbar_arrive_expect_tx(full, K::STAGE_BYTES);
-        if constexpr (DIR == 0) {
-#pragma unroll
-            for (int t = 0; t < NT; ++t) {
-                tma_load_2d(dst + t * 4096, &tm_prev, (g0 + t * SUB) * U, line0, full);
-                tma_load_2d(dst + K::FIELD_BYTES + t * 4096, &tm_cur, (g0 + t * SUB) * U, line0, full);
+        if (lane == 0) {
+            const int line0 = q_pc.panel * TL;
+            const int g0 = (max(q_pc.ua - nbk, 0) & ~(SUB - 1)) + q_s * NW;
+            const uint32_t full = bar32 + 8 * q_slot;
+            const uint32_t dst = sm32 + q_slot * K::STAGE_BYTES;
+            if (warp == 0) mbar_arrive_expect_tx(full, K::STAGE_BYTES);
+            if constexpr (DIR == 0) {
+                if (sub == 0) {
+                    tma_load_2d(dst + tix * 4096, &tm_prev, (g0 + tix * SUB) * U, line0, full);
+                    tma_load_2d(dst + K::FIELD_BYTES + tix * 4096, &tm_cur, (g0 + tix * SUB) * U, line0, full);
+                }
+                if (warp == (SUB > 1 ? 1 : 0))
+                    tma_load_2d(dst + 2 * K::FIELD_BYTES, &tm_edge, g0 * U - V, line0, full);
+                if (warp == (SUB > 1 ? SUB + 1 : NW - 1))
+                    tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
+            } else {
+                if (warp == 0) tma_load_2d(dst, &tm_prev, line0, g0 * U - 1, full);
+                if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0, g0 * U - 1, full);
             }
-            tma_load_2d(dst + 2 * K::FIELD_BYTES, &tm_edge, g0 * U - V, line0, full);
-            tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
-        } else {
-            tma_load_2d(dst, &tm_prev, line0, g0 * U - 1, full);
-            tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0, g0 * U - 1, full);
         }
         q_slot = q_slot + 1 == NSTAGE ? 0 : q_slot + 1;
         if (++q_s == q_pc.nst) {
@@ -219,10 +239,8 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             if (++q_pi < pc_end) q_pc = a.pieces[q_pi];
         }
     };
-    if (threadIdx.x == 0) {
 #pragma unroll
-        for (int s = 0; s < NSTAGE; ++s) produce();
-    }
+    for (int s = 0; s < NSTAGE; ++s) produce();
 
     // ---- consumers (all warps)
     const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), rho = static_cast<T>(row[ROW_RHO]);
@@ -237,19 +255,24 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     // warps [0, wdef) finish their unit in the stage that computed it; warps [wdef, NW) one stage later
     const int wdef = ((NW - nbk) / SUB) * SUB;
     const bool deferred = warp >= wdef;
-    [[maybe_unused]] unsigned char* my_out = sm + NSTAGE * K::STAGE_BYTES + warp * (32 * K::RB);
-    [[maybe_unused]] const int sub = warp % SUB, tix = warp / SUB;
+    [[maybe_unused]] unsigned char* const my_out0 = sm + NSTAGE * K::STAGE_BYTES + warp * (2 * 32 * K::RB);
+    [[maybe_unused]] unsigned char* my_out = my_out0;   // alternates between the warp's two store tiles
 
     // finish unit gp (local x in v[]): add the carry from the right, store
     auto finish = [&](T (&v)[U], int gp, int ring, const Piece& pc) {
         T Xin = T(0);   // x at the start of unit gp+1
-        for (int j = nbk; j >= 1; --j) {
-            const int idx = (ring + j) & (RING - 1);
-            Xin = fma(s_A[idx], Xin, s_H[idx * TL + lane]);
+        if (nbk > 4) {
+#pragma unroll
+            for (int j = NBK_MAX; j > 4; --j)
+                if (j <= nbk) Xin = fma(s_A[(ring + j) & (RING - 1)], Xin, s_H[((ring + j) & (RING - 1)) * TL + lane]);
         }
+#pragma unroll
+        for (int j = 4; j >= 1; --j)
+            if (j <= nbk) Xin = fma(s_A[(ring + j) & (RING - 1)], Xin, s_H[((ring + j) & (RING - 1)) * TL + lane]);
         if (gp < pc.ua || gp >= pc.ub) return;   // warp-uniform
         const int pp0 = gp * U;
-        if (gp >= a.kb && pp0 + U <= n) {
+        const bool full = pp0 + U <= n;
+        if (gp >= kb && full) {
 #pragma unroll
             for (int e = 0; e < U; ++e) v[e] = fma(pw[U - 1 - e], Xin, v[e]);
         } else {
@@ -260,24 +283,28 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 v[e] += c;
             }
         }
-        const int line0 = pc.panel * TL;
         if constexpr (DIR == 0) {
-            if (lane == 0) tma_wait_read<0>();   // the previous store of this warp has read the tile
+            if (lane == 0) tma_wait_read<1>();   // the store before the previous one has read this tile
             __syncwarp();
             store_unit_x<T, U>(my_out, lane, v);
             fence_async_smem();
             __syncwarp();
             if (lane == 0) {
-                tma_store_2d(&tm_out, pp0, line0, smem_u32(my_out));
+                tma_store_2d(&tm_out, pp0, pc.panel * TL, smem_u32(my_out));
                 tma_commit();
             }
+            my_out = my_out == my_out0 ? my_out0 + 32 * K::RB : my_out0;
         } else {
-            const int line = line0 + lane;
-            if (line < a.nlines) {
-                T* o = reinterpret_cast<T*>(a.out) + static_cast<long long>(pp0) * a.pitch + line;
+            if (pc.panel * TL + lane < nlines) {
+                T* o = out_lane + pc.panel * TL + static_cast<long long>(pp0) * pitch;
+                if (full) {
 #pragma unroll
-                for (int e = 0; e < U; ++e)
-                    if (pp0 + e < n) o[static_cast<long long>(e) * a.pitch] = v[e];
+                    for (int e = 0; e < U; ++e, o += pitch) *o = v[e];
+                } else {
+#pragma unroll
+                    for (int e = 0; e < U; ++e, o += pitch)
+                        if (pp0 + e < n) *o = v[e];
+                }
             }
         }
     };
@@ -304,7 +331,9 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             const int g = gbase + s * NW + warp, p0 = g * U;
             T xl[U];
             // ---- shared memory -> registers
+            if (tracing) t_last = clock64();
             mbar_wait(bar32 + 8 * slot, phase);
+            tick(0);
             const unsigned char* st = sm + slot * K::STAGE_BYTES;
             if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
             T wp[U], wc[U], wl, wr;
@@ -330,16 +359,26 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             }
             // ---- RHS + local forward elimination
             const bool src_k = src_tile && p0 < a.sp0 + a.snp && p0 + U > a.sp0;
-            const bool fast = g >= a.kb && p0 + U <= n && !src_k;
+            const bool fast = g >= kb && p0 + U <= n;   // stationary pivots, whole unit inside the line
             T Aval;
-            if (fast) {   // stationary pivots: y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
-                T fy = T(0);
+            if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
 #pragma unroll
                 for (int e = 0; e < U; ++e) {
                     const T left = e == 0 ? wl : wp[e - 1];
                     const T right = e == U - 1 ? wr : wp[e + 1];
-                    const T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
-                    fy = fma(rho, fy, r * inv);
+                    xl[e] = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                }
+                if (src_k && src_line) {
+#pragma unroll
+                    for (int e = 0; e < U; ++e) {
+                        const int ps = p0 + e - a.sp0;
+                        if (ps >= 0 && ps < a.snp) xl[e] = fma(q, srcp[static_cast<size_t>(ps) * a.snl], xl[e]);
+                    }
+                }
+                T fy = T(0);
+#pragma unroll
+                for (int e = 0; e < U; ++e) {
+                    fy = fma(rho, fy, xl[e] * inv);
                     xl[e] = fy;
                 }
                 Aval = pw[U - 1];
@@ -364,15 +403,21 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             }
             s_L[ring * TL + lane] = xl[U - 1];
             if (lane == 0) s_A[ring] = Aval;
+            tick(1);
             named_bar_sync(1, NW * 32);
-            if (threadIdx.x == 0) produce();   // every warp holds its stage data in registers: refill the slot
+            tick(2);
+            produce();   // every warp holds its stage data in registers: refill the slot
 
             // ---- carry from the left, local back substitution
             T Yin = T(0);   // y at the end of unit g-1
-            for (int j = nbk; j >= 1; --j) {
-                const int idx = (ring - j) & (RING - 1);
-                Yin = fma(s_A[idx], Yin, s_L[idx * TL + lane]);
+            if (nbk > 4) {
+#pragma unroll
+                for (int j = NBK_MAX; j > 4; --j)
+                    if (j <= nbk) Yin = fma(s_A[(ring - j) & (RING - 1)], Yin, s_L[((ring - j) & (RING - 1)) * TL + lane]);
             }
+#pragma unroll
+            for (int j = 4; j >= 1; --j)
+                if (j <= nbk) Yin = fma(s_A[(ring - j) & (RING - 1)], Yin, s_L[((ring - j) & (RING - 1)) * TL + lane]);
             if (fast) {
 #pragma unroll
                 for (int e = 0; e < U; ++e) xl[e] = fma(pw[e], Yin, xl[e]);
@@ -389,7 +434,9 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 for (int e = U - 2; e >= 0; --e) xl[e] = fma(cp_at(p0 + e), xl[e + 1], xl[e]);
             }
             s_H[ring * TL + lane] = xl[0];
+            tick(3);
             named_bar_sync(1, NW * 32);
+            tick(4);
 
             // ---- carry from the right, store
             if (deferred) {
@@ -399,6 +446,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             } else {
                 finish(xl, g, ring, pc);
             }
+            tick(5);
         }
         // ---- flush: the deferred units of the last stage see zero heads beyond it
         const int ringf = (pc.nst & 1) * NW + warp;
@@ -408,6 +456,20 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     }
     if constexpr (DIR == 0) {
         if (lane == 0) tma_wait_read<0>();
+    }
+    if (a.trace) {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long* t = a.trace + 16 * static_cast<size_t>(blockIdx.x);
+            t[0] = t_start;
+            t[1] = globaltimer_ns();
+            t[2] = smid();
+            t[3] = static_cast<unsigned long long>(t_ph[0]);
+        }
+        if (tracing) {
+            unsigned long long* t = a.trace + 16 * static_cast<size_t>(blockIdx.x) + (warp == 0 ? 4 : 10);
+            for (int k = 0; k < 6; ++k) t[k] = static_cast<unsigned long long>(t_ph[k]);
+        }
     }
 }
 

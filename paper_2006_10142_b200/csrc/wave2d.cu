@@ -28,34 +28,34 @@ struct Variant {
     const void* fn;
 };
 
-template <typename T, int DIR, int UT, int NW, int NSTAGE>
+template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB = 1>
 Variant make_variant()
 {
     using K = PanelCfg<T, DIR, UT, NW, NSTAGE>;
     return Variant{DIR, NW, NSTAGE, UT, K::SUB, K::SMEM_BYTES, K::THREADS, (int)sizeof(T),
-                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE>)};
+                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB>)};
 }
 
 constexpr int NVAR = 4;   // shape variants per (dtype, dir); index 0 is the default
 void add_shapes_f64(std::vector<Variant>& v)
 {
     v.push_back(make_variant<double, 0, 8, 16, 2>());
-    v.push_back(make_variant<double, 0, 8, 8, 3>());
+    v.push_back(make_variant<double, 0, 8, 8, 2, 2>());
     v.push_back(make_variant<double, 0, 16, 8, 2>());
     v.push_back(make_variant<double, 0, 4, 16, 2>());
     v.push_back(make_variant<double, 1, 8, 16, 3>());
-    v.push_back(make_variant<double, 1, 8, 8, 3>());
+    v.push_back(make_variant<double, 1, 8, 8, 3, 2>());
     v.push_back(make_variant<double, 1, 16, 8, 3>());
     v.push_back(make_variant<double, 1, 8, 16, 2>());
 }
 void add_shapes_f32(std::vector<Variant>& v)
 {
     v.push_back(make_variant<float, 0, 16, 16, 2>());
-    v.push_back(make_variant<float, 0, 8, 16, 2>());
+    v.push_back(make_variant<float, 0, 16, 8, 2, 2>());
     v.push_back(make_variant<float, 0, 32, 8, 2>());
-    v.push_back(make_variant<float, 0, 16, 8, 3>());
+    v.push_back(make_variant<float, 0, 8, 16, 2>());
     v.push_back(make_variant<float, 1, 8, 16, 3>());
-    v.push_back(make_variant<float, 1, 8, 8, 3>());
+    v.push_back(make_variant<float, 1, 8, 8, 3, 2>());
     v.push_back(make_variant<float, 1, 16, 8, 3>());
     v.push_back(make_variant<float, 1, 8, 16, 4>());
 }
@@ -134,6 +134,8 @@ struct wave2d_s {
     CUtensorMap tm_load[2][3], tm_store[3], tm_edge[3];   // [dir][buffer]; x: load tile, store tile, 16-byte edge box
     Piece* d_pieces[2] = {nullptr, nullptr};
     int* d_cta_off[2] = {nullptr, nullptr};
+    int opt_trace = 0;
+    unsigned long long* d_trace[2] = {nullptr, nullptr};   // per-CTA trace of the last launch per direction
     cudaGraphExec_t gexec = nullptr;
     int gexec_steps = 0;
 
@@ -383,8 +385,10 @@ int ensure_plan(wave2d_t* h)
     for (int d = 0; d < 2; ++d) {
         cudaFree(h->d_pieces[d]);
         cudaFree(h->d_cta_off[d]);
+        cudaFree(h->d_trace[d]);
         h->d_pieces[d] = nullptr;
         h->d_cta_off[d] = nullptr;
+        h->d_trace[d] = nullptr;
         const DirPlan& P = h->plan[d];
         if (P.solver != WAVE2D_SOLVER_STREAM) continue;
         const size_t pb = std::max<size_t>(1, P.pieces.size()) * sizeof(Piece), ob = P.cta_off.size() * sizeof(int);
@@ -394,6 +398,11 @@ int ensure_plan(wave2d_t* h)
         if (!P.pieces.empty())
             W2D_CUDA(h, cudaMemcpy(h->d_pieces[d], P.pieces.data(), P.pieces.size() * sizeof(Piece), cudaMemcpyHostToDevice));
         W2D_CUDA(h, cudaMemcpy(h->d_cta_off[d], P.cta_off.data(), ob, cudaMemcpyHostToDevice));
+        if (h->opt_trace) {
+            st = dev_alloc(h, reinterpret_cast<void**>(&h->d_trace[d]), (size_t)P.grid * 16 * sizeof(unsigned long long));
+            if (st) return st;
+            W2D_CUDA(h, cudaMemset(h->d_trace[d], 0, (size_t)P.grid * 16 * sizeof(unsigned long long)));
+        }
     }
     if ((h->plan[0].solver == WAVE2D_SOLVER_EXACT || h->plan[1].solver == WAVE2D_SOLVER_EXACT) && !h->d_piv) {
         st = dev_alloc(h, reinterpret_cast<void**>(&h->d_piv), sizeof(double) * 2 * (size_t)std::max(h->n1, h->n2));
@@ -424,6 +433,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         a.out = out; a.pitch = h->pitch;
         a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
         a.g2 = 2.0 * h->gamma;
+        a.trace = h->opt_trace ? h->d_trace[d] : nullptr;
         CUtensorMap* tp = &h->tm_load[d][n_abs % 3];
         CUtensorMap* tc = &h->tm_load[d][(n_abs + 1) % 3];
         CUtensorMap* to = &h->tm_store[(n_abs + 2) % 3];     // x sweep: TMA store box; unused by the y sweep
@@ -592,6 +602,7 @@ void wave2d_destroy(wave2d_t* h)
     for (int d = 0; d < 2; ++d) {
         cudaFree(h->d_pieces[d]);
         cudaFree(h->d_cta_off[d]);
+        cudaFree(h->d_trace[d]);
     }
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
     (void)cudaGetLastError();
@@ -619,6 +630,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "graph_steps")) { if (iv < 3 || iv % 3) return WAVE2D_ERR_ARG; h->opt_graph_steps = iv; }
     else if (!strcmp(name, "shape_x")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[0] = iv; }
     else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
+    else if (!strcmp(name, "trace")) h->opt_trace = iv != 0;
     else if (!strcmp(name, "quota_x")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[0] = iv; }
     else if (!strcmp(name, "quota_y")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[1] = iv; }
     else return WAVE2D_ERR_ARG;
@@ -842,6 +854,18 @@ int wave2d_profile_sweeps(wave2d_t* h, int steps, double* ms_x, double* ms_y)
     for (auto& e : ev) cudaEventDestroy(e);
     *ms_x = sx / steps;
     *ms_y = sy / steps;
+    return WAVE2D_OK;
+}
+
+int wave2d_get_trace(wave2d_t* h, int dir, unsigned long long* out, int capacity, int* count)
+{
+    if (!h || dir < 0 || dir > 1 || !out || !count) return WAVE2D_ERR_ARG;
+    if (!h->plan_ok || !h->opt_trace || !h->d_trace[dir]) return WAVE2D_ERR_STATE;
+    const int g = h->plan[dir].grid;
+    *count = g;
+    if (capacity < g) return WAVE2D_ERR_ARG;
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    W2D_CUDA(h, cudaMemcpy(out, h->d_trace[dir], (size_t)g * 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
     return WAVE2D_OK;
 }
 
