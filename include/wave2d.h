@@ -159,11 +159,10 @@ int wave2d_profile_sweeps(wave2d_t *h, int steps, double *ms_x, double *ms_y);
 
 /*
  * Tracing (option "trace" = 1, before the first run): every CTA of a sweep kernel records its start and end
- * time (GPU global timer, ns), the SM it ran on and the cycles its first warp spent waiting for TMA data.
+ * time (GPU global timer, ns), the SM it ran on and the number of pieces of work it had.
  * Copies the records of the most recent launch of direction dir (0 = x, 1 = y) to the host array
- * out[16 * capacity], 16 values per CTA: start_ns, end_ns, sm_id, wait_cycles, then for the first and for
- * the last warp six cycle counters each (wait for data; load + forward; barrier 1; carry + backward;
- * barrier 2; finish + store); *count = CTAs in the grid.
+ * out[16 * capacity], 16 values per CTA: start_ns, end_ns, sm_id, pieces of work, 12 reserved;
+ * *count = CTAs in the grid.
  * Errors: ERR_ARG (capacity < *count), ERR_STATE (tracing off or nothing planned).  Synchronises the stream.
  */
 int wave2d_get_trace(wave2d_t *h, int dir, unsigned long long *out, int capacity, int *count);

@@ -77,7 +77,7 @@ struct PanelCfg {
     static constexpr int OUT_BYTES = DIR == 0 ? NW * 2 * 32 * RB : 0;   // two store tiles per warp
     static constexpr int BAR_BYTES = ((NSTAGE * 8) + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * KMAX * (int)sizeof(T);
-    static constexpr int XCH_BYTES = (4 * NW * TL + 2 * NW) * (int)sizeof(T);   // L[2NW][32], H[2NW][32], A[2NW]
+    static constexpr int XCH_BYTES = (4 * NW * TL + 2 * NW + UT) * (int)sizeof(T);   // L[2NW][32], H[2NW][32], A[2NW], pw[UT]
     static constexpr int SMEM_BYTES = 1024 + NSTAGE * STAGE_BYTES + OUT_BYTES + BAR_BYTES + TAB_BYTES + XCH_BYTES;
     static constexpr int THREADS = 32 * NW;
     static_assert((NW & (NW - 1)) == 0, "NW must be a power of two (ring indexing)");
@@ -170,6 +170,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     T* s_L = s_inv + KMAX;           // [RING][32]  last local y of a unit
     T* s_H = s_L + RING * TL;        // [RING][32]  first local x of a unit
     T* s_A = s_H + RING * TL;        // [RING]      product of the unit's cp
+    T* s_pw = s_A + RING;            // [U]         rho^(e+1)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nh = a.n_off + (a.d_k ? 2 * (*a.d_k) : 0);
@@ -178,6 +179,10 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     for (int i = threadIdx.x; i < KMAX; i += K::THREADS) {
         s_cp[i] = static_cast<T>(row[ROW_CP + i]);
         s_inv[i] = static_cast<T>(row[ROW_INVP + i]);
+    }
+    if (threadIdx.x == 32 % K::THREADS) {
+        T pwr = static_cast<T>(row[ROW_RHO]);
+        for (int e = 0; e < U; ++e, pwr *= static_cast<T>(row[ROW_RHO])) s_pw[e] = pwr;
     }
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -193,15 +198,6 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     const long long pitch = a.pitch;
     [[maybe_unused]] T* const out_lane = reinterpret_cast<T*>(a.out) + (threadIdx.x & 31);
     unsigned long long t_start = 0;
-    long long t_ph[6] = {0, 0, 0, 0, 0, 0}, t_last = 0;
-    const bool tracing = a.trace != nullptr && lane == 0 && (warp == 0 || warp == NW - 1);
-    auto tick = [&](int k) {
-        if (tracing) {
-            const long long c = clock64();
-            t_ph[k] += c - t_last;
-            t_last = c;
-        }
-    };
     if (a.trace && threadIdx.x == 0) t_start = globaltimer_ns();
 
     // ---- producer cursor (kept by every thread): the next stage to request, NSTAGE ahead of the consumers.
@@ -243,38 +239,50 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     for (int s = 0; s < NSTAGE; ++s) produce();
 
     // ---- consumers (all warps)
-    const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), rho = static_cast<T>(row[ROW_RHO]);
-    const T inv = static_cast<T>(row[ROW_INV]), c1 = static_cast<T>(row[ROW_C1]), g2 = static_cast<T>(a.g2);
-    T pw[U];   // pw[e] = rho^(e+1)
-    pw[0] = rho;
-#pragma unroll
-    for (int e = 1; e < U; ++e) pw[e] = pw[e - 1] * rho;
+    const T rho = static_cast<T>(row[ROW_RHO]), inv = static_cast<T>(row[ROW_INV]);
+    const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]);
+    const T c1 = static_cast<T>(row[ROW_C1]), g2 = static_cast<T>(a.g2);
+    const T ami = am * inv, c1i = c1 * inv, g2i = g2 * inv, qi = q * inv;   // stationary rows: r_e inv in one go
     auto cp_at = [&](int p) -> T { return p < KMAX ? s_cp[p] : rho; };
     auto inv_at = [&](int p) -> T { return p < KMAX ? s_inv[p] : inv; };
+    auto pw_at = [&](int e) -> T { return s_pw[e]; };   // rho^(e+1), broadcast read
 
     // warps [0, wdef) finish their unit in the stage that computed it; warps [wdef, NW) one stage later
     const int wdef = ((NW - nbk) / SUB) * SUB;
-    const bool deferred = warp >= wdef;
     [[maybe_unused]] unsigned char* const my_out0 = sm + NSTAGE * K::STAGE_BYTES + warp * (2 * 32 * K::RB);
     [[maybe_unused]] unsigned char* my_out = my_out0;   // alternates between the warp's two store tiles
+    const T* const sL_lane = s_L + lane;
+    const T* const sH_lane = s_H + lane;
 
-    // finish unit gp (local x in v[]): add the carry from the right, store
-    auto finish = [&](T (&v)[U], int gp, int ring, const Piece& pc) {
-        T Xin = T(0);   // x at the start of unit gp+1
+    // carry series: value entering unit `ring` from the left (dirn = -1, over L) or from the right (+1, over H)
+    auto carry = [&](const T* vals_lane, int ring, int dirn) -> T {
+        T c = T(0);
         if (nbk > 4) {
 #pragma unroll
             for (int j = NBK_MAX; j > 4; --j)
-                if (j <= nbk) Xin = fma(s_A[(ring + j) & (RING - 1)], Xin, s_H[((ring + j) & (RING - 1)) * TL + lane]);
+                if (j <= nbk) {
+                    const int idx = (ring + dirn * j) & (RING - 1);
+                    c = fma(s_A[idx], c, vals_lane[idx * TL]);
+                }
         }
 #pragma unroll
         for (int j = 4; j >= 1; --j)
-            if (j <= nbk) Xin = fma(s_A[(ring + j) & (RING - 1)], Xin, s_H[((ring + j) & (RING - 1)) * TL + lane]);
-        if (gp < pc.ua || gp >= pc.ub) return;   // warp-uniform
+            if (j <= nbk) {
+                const int idx = (ring + dirn * j) & (RING - 1);
+                c = fma(s_A[idx], c, vals_lane[idx * TL]);
+            }
+        return c;
+    };
+
+    // finish unit gp (local x in v[]): add the carry from the right, store
+    auto finish = [&](T (&v)[U], int gp, int ring, const Piece& pc) {
+        const T Xin = carry(sH_lane, ring, +1);   // x at the start of unit gp+1
+        if (gp < pc.ua || gp >= pc.ub) return;    // warp-uniform
         const int pp0 = gp * U;
         const bool full = pp0 + U <= n;
         if (gp >= kb && full) {
 #pragma unroll
-            for (int e = 0; e < U; ++e) v[e] = fma(pw[U - 1 - e], Xin, v[e]);
+            for (int e = 0; e < U; ++e) v[e] = fma(pw_at(U - 1 - e), Xin, v[e]);
         } else {
             T c = Xin;
 #pragma unroll
@@ -309,151 +317,141 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
         }
     };
 
-    T pend[U];
-#pragma unroll
-    for (int e = 0; e < U; ++e) pend[e] = T(0);
     int slot = 0, phase = 0;
 
-    for (int pi = pc_begin; pi < pc_end; ++pi) {
-        const Piece pc = a.pieces[pi];
-        const int line0 = pc.panel * TL, line = line0 + lane;
-        const int gbase = max(pc.ua - nbk, 0) & ~(SUB - 1);
-        const bool src_tile = a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
-        const bool src_line = line >= a.sl0 && line < a.sl0 + a.snl;
-        const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
+    // The stage loop, compiled twice: DEF = false for warps that finish their unit in the same stage,
+    // DEF = true for the last few warps, which keep the local x of their unit in registers for one stage.
+    auto run_pieces = [&](auto def_c) {
+        constexpr bool DEF = decltype(def_c)::value;
+        T pend[DEF ? U : 1];
+#pragma unroll
+        for (int e = 0; e < (DEF ? U : 1); ++e) pend[e] = T(0);
 
-        __syncthreads();   // the previous piece is completely finished
-        s_L[(NW + warp) * TL + lane] = T(0);   // "stage -1": zero carries
-        if (lane == 0) s_A[NW + warp] = T(0);
+        for (int pi = pc_begin; pi < pc_end; ++pi) {
+            const Piece pc = a.pieces[pi];
+            const int line0 = pc.panel * TL, line = line0 + lane;
+            const int gbase = max(pc.ua - nbk, 0) & ~(SUB - 1);
+            const bool src_tile = a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
+            const bool src_line = line >= a.sl0 && line < a.sl0 + a.snl;
+            const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
 
-        for (int s = 0; s < pc.nst; ++s) {
-            const int ring = (s & 1) * NW + warp;
-            const int g = gbase + s * NW + warp, p0 = g * U;
-            T xl[U];
-            // ---- shared memory -> registers
-            if (tracing) t_last = clock64();
-            mbar_wait(bar32 + 8 * slot, phase);
-            tick(0);
-            const unsigned char* st = sm + slot * K::STAGE_BYTES;
-            if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
-            T wp[U], wc[U], wl, wr;
-            if constexpr (DIR == 0) {
-                const unsigned char* tp = st + tix * 4096;
-                load_unit_x<T, U>(tp, lane, sub, wp);
-                load_unit_x<T, U>(tp + K::FIELD_BYTES, lane, sub, wc);
-                if (sub > 0) wl = tile_elem_x<T>(tp, lane, sub * U - 1);
-                else if (tix > 0) wl = tile_elem_x<T>(tp - 4096, lane, K::TU - 1);
-                else wl = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES)[lane * V + V - 1];
-                if (sub < SUB - 1) wr = tile_elem_x<T>(tp, lane, (sub + 1) * U);
-                else if (tix < NT - 1) wr = tile_elem_x<T>(tp + 4096, lane, 0);
-                else wr = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V];
-            } else {
-                const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
-                const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
-                wl = cpv[0];
+            named_bar_sync(1, NW * 32);   // the previous piece is completely finished
+            s_L[(NW + warp) * TL + lane] = T(0);   // "stage -1": zero carries
+            if (lane == 0) s_A[NW + warp] = T(0);
+
+            for (int s = 0; s < pc.nst; ++s) {
+                const int ring = (s & 1) * NW + warp;
+                const int g = gbase + s * NW + warp, p0 = g * U;
+                T xl[U];
+                // ---- shared memory -> registers
+                mbar_wait(bar32 + 8 * slot, phase);
+                const unsigned char* st = sm + slot * K::STAGE_BYTES;
+                if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
+                T wp[U], wc[U], wl, wr;
+                if constexpr (DIR == 0) {
+                    const unsigned char* tp = st + tix * 4096;
+                    load_unit_x<T, U>(tp, lane, sub, wp);
+                    load_unit_x<T, U>(tp + K::FIELD_BYTES, lane, sub, wc);
+                    if (sub > 0) wl = tile_elem_x<T>(tp, lane, sub * U - 1);
+                    else if (tix > 0) wl = tile_elem_x<T>(tp - 4096, lane, K::TU - 1);
+                    else wl = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES)[lane * V + V - 1];
+                    if (sub < SUB - 1) wr = tile_elem_x<T>(tp, lane, (sub + 1) * U);
+                    else if (tix < NT - 1) wr = tile_elem_x<T>(tp + 4096, lane, 0);
+                    else wr = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V];
+                } else {
+                    const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
+                    const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
+                    wl = cpv[0];
 #pragma unroll
-                for (int e = 0; e < U; ++e) wp[e] = cpv[(e + 1) * TL];
-                wr = cpv[(U + 1) * TL];
+                    for (int e = 0; e < U; ++e) wp[e] = cpv[(e + 1) * TL];
+                    wr = cpv[(U + 1) * TL];
 #pragma unroll
-                for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
-            }
-            // ---- RHS + local forward elimination
-            const bool src_k = src_tile && p0 < a.sp0 + a.snp && p0 + U > a.sp0;
-            const bool fast = g >= kb && p0 + U <= n;   // stationary pivots, whole unit inside the line
-            T Aval;
-            if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
-#pragma unroll
-                for (int e = 0; e < U; ++e) {
-                    const T left = e == 0 ? wl : wp[e - 1];
-                    const T right = e == U - 1 ? wr : wp[e + 1];
-                    xl[e] = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                    for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
                 }
-                if (src_k && src_line) {
+                // ---- RHS + local forward elimination
+                const bool fast = g >= kb && p0 + U <= n;   // stationary pivots, whole unit inside the line
+                T Aval;
+                if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
 #pragma unroll
                     for (int e = 0; e < U; ++e) {
-                        const int ps = p0 + e - a.sp0;
-                        if (ps >= 0 && ps < a.snp) xl[e] = fma(q, srcp[static_cast<size_t>(ps) * a.snl], xl[e]);
+                        const T left = e == 0 ? wl : wp[e - 1];
+                        const T right = e == U - 1 ? wr : wp[e + 1];
+                        xl[e] = fma(g2i, wc[e], fma(ami, left + right, c1i * wp[e]));
                     }
-                }
-                T fy = T(0);
+                    if (src_tile && src_line && p0 < a.sp0 + a.snp && p0 + U > a.sp0) {
 #pragma unroll
-                for (int e = 0; e < U; ++e) {
-                    fy = fma(rho, fy, xl[e] * inv);
-                    xl[e] = fy;
-                }
-                Aval = pw[U - 1];
-            } else {
-                const bool src_unit = src_k && src_line;
-                T fy = T(0), prod = T(1);
+                        for (int e = 0; e < U; ++e) {
+                            const int ps = p0 + e - a.sp0;
+                            if (ps >= 0 && ps < a.snp) xl[e] = fma(qi, srcp[static_cast<size_t>(ps) * a.snl], xl[e]);
+                        }
+                    }
 #pragma unroll
-                for (int e = 0; e < U; ++e) {
-                    const int p = p0 + e;
-                    const T left = e == 0 ? wl : wp[e - 1];
-                    const T right = e == U - 1 ? wr : wp[e + 1];
-                    T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
-                    if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
-                        r = fma(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
-                    const T cpe = cp_at(p);
-                    fy = fma(cpe, fy, r * inv_at(p));
-                    if (p >= n) fy = T(0);
-                    prod *= cpe;
-                    xl[e] = fy;
+                    for (int e = 1; e < U; ++e) xl[e] = fma(rho, xl[e - 1], xl[e]);
+                    Aval = pw_at(U - 1);
+                } else {
+                    const bool src_unit = src_tile && src_line;
+                    T fy = T(0), prod = T(1);
+#pragma unroll
+                    for (int e = 0; e < U; ++e) {
+                        const int p = p0 + e;
+                        const T left = e == 0 ? wl : wp[e - 1];
+                        const T right = e == U - 1 ? wr : wp[e + 1];
+                        T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                        if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
+                            r = fma(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
+                        const T cpe = cp_at(p);
+                        fy = fma(cpe, fy, r * inv_at(p));
+                        if (p >= n) fy = T(0);
+                        prod *= cpe;
+                        xl[e] = fy;
+                    }
+                    Aval = prod;
                 }
-                Aval = prod;
-            }
-            s_L[ring * TL + lane] = xl[U - 1];
-            if (lane == 0) s_A[ring] = Aval;
-            tick(1);
-            named_bar_sync(1, NW * 32);
-            tick(2);
-            produce();   // every warp holds its stage data in registers: refill the slot
+                s_L[ring * TL + lane] = xl[U - 1];
+                if (lane == 0) s_A[ring] = Aval;
+                named_bar_sync(1, NW * 32);
+                produce();   // every warp holds its stage data in registers: refill the slot
 
-            // ---- carry from the left, local back substitution
-            T Yin = T(0);   // y at the end of unit g-1
-            if (nbk > 4) {
+                // ---- carry from the left, local back substitution
+                const T Yin = carry(sL_lane, ring, -1);   // y at the end of unit g-1
+                if (fast) {
+                    xl[U - 1] = fma(pw_at(U - 1), Yin, xl[U - 1]);
 #pragma unroll
-                for (int j = NBK_MAX; j > 4; --j)
-                    if (j <= nbk) Yin = fma(s_A[(ring - j) & (RING - 1)], Yin, s_L[((ring - j) & (RING - 1)) * TL + lane]);
-            }
+                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(rho, xl[e + 1], fma(pw_at(e), Yin, xl[e]));
+                } else {
+                    T c = Yin;
 #pragma unroll
-            for (int j = 4; j >= 1; --j)
-                if (j <= nbk) Yin = fma(s_A[(ring - j) & (RING - 1)], Yin, s_L[((ring - j) & (RING - 1)) * TL + lane]);
-            if (fast) {
+                    for (int e = 0; e < U; ++e) {
+                        c *= cp_at(p0 + e);
+                        xl[e] = p0 + e < n ? xl[e] + c : T(0);
+                    }
 #pragma unroll
-                for (int e = 0; e < U; ++e) xl[e] = fma(pw[e], Yin, xl[e]);
-#pragma unroll
-                for (int e = U - 2; e >= 0; --e) xl[e] = fma(rho, xl[e + 1], xl[e]);
-            } else {
-                T c = Yin;
-#pragma unroll
-                for (int e = 0; e < U; ++e) {
-                    c *= cp_at(p0 + e);
-                    xl[e] = p0 + e < n ? xl[e] + c : T(0);
+                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(cp_at(p0 + e), xl[e + 1], xl[e]);
                 }
-#pragma unroll
-                for (int e = U - 2; e >= 0; --e) xl[e] = fma(cp_at(p0 + e), xl[e + 1], xl[e]);
-            }
-            s_H[ring * TL + lane] = xl[0];
-            tick(3);
-            named_bar_sync(1, NW * 32);
-            tick(4);
+                s_H[ring * TL + lane] = xl[0];
+                named_bar_sync(1, NW * 32);
 
-            // ---- carry from the right, store
-            if (deferred) {
-                if (s > 0) finish(pend, g - NW, ring ^ NW, pc);
+                // ---- carry from the right, store
+                if constexpr (DEF) {
+                    if (s > 0) finish(pend, g - NW, ring ^ NW, pc);
 #pragma unroll
-                for (int e = 0; e < U; ++e) pend[e] = xl[e];
-            } else {
-                finish(xl, g, ring, pc);
+                    for (int e = 0; e < U; ++e) pend[e] = xl[e];
+                } else {
+                    finish(xl, g, ring, pc);
+                }
             }
-            tick(5);
+            // ---- flush: the deferred units of the last stage see zero heads beyond it
+            const int ringf = (pc.nst & 1) * NW + warp;
+            s_H[ringf * TL + lane] = T(0);
+            named_bar_sync(1, NW * 32);
+            if constexpr (DEF) {
+                if (pc.nst > 0) finish(pend, gbase + (pc.nst - 1) * NW + warp, ringf ^ NW, pc);
+            }
         }
-        // ---- flush: the deferred units of the last stage see zero heads beyond it
-        const int ringf = (pc.nst & 1) * NW + warp;
-        s_H[ringf * TL + lane] = T(0);
-        named_bar_sync(1, NW * 32);
-        if (deferred && pc.nst > 0) finish(pend, gbase + (pc.nst - 1) * NW + warp, ringf ^ NW, pc);
-    }
+    };
+    if (warp >= wdef) run_pieces(std::true_type{});
+    else run_pieces(std::false_type{});
+
     if constexpr (DIR == 0) {
         if (lane == 0) tma_wait_read<0>();
     }
@@ -464,11 +462,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             t[0] = t_start;
             t[1] = globaltimer_ns();
             t[2] = smid();
-            t[3] = static_cast<unsigned long long>(t_ph[0]);
-        }
-        if (tracing) {
-            unsigned long long* t = a.trace + 16 * static_cast<size_t>(blockIdx.x) + (warp == 0 ? 4 : 10);
-            for (int k = 0; k < 6; ++k) t[k] = static_cast<unsigned long long>(t_ph[k]);
+            t[3] = static_cast<unsigned long long>(pc_end - pc_begin);
         }
     }
 }
