@@ -91,8 +91,8 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "graph_steps"  time steps per graph replay (multiple of 3, the period of the buffer ring).  Default 12.
  *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (units per stage = consumer warps / stages).
  *   "trace"  1: sweep kernels record per-CTA timing (see wave2d_get_trace).  Default 0.
- *   "quota_x", "quota_y"   tuning: stages of work per CTA (0 = planned: one wave over the resident CTA slots);
- *                          lines are cut where a CTA's quota ends.
+ *   "quota_x", "quota_y"   tuning: length in stages of every piece of work a line is cut into (0 = planned:
+ *                          guided self-scheduling, long pieces first, short ones last).
  * Errors: ERR_ARG (unknown name / bad value), ERR_STATE.
  */
 int wave2d_set_option(wave2d_t *h, const char *name, double value);

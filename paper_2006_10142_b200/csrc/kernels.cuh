@@ -50,7 +50,10 @@ struct SweepArgs {
     int nbk;               // carry series length in units (<= NW, <= NBK_MAX)
     int kb;                // units [0, kb) use the boundary pivots of the table
     const Piece* pieces;   // device
-    const int* cta_off;    // device: CTA b owns pieces [cta_off[b], cta_off[b+1])
+    int npieces;           // all pieces
+    int nstatic;           // pieces [0, nstatic) are dealt out statically, the rest through the ticket counter
+    const int* cta_off;    // device: CTA b first works pieces [cta_off[b], cta_off[b+1])
+    int* tickets;          // device: one zeroed counter per half-step (indexed like `table`)
     void* out;             // y sweep: output field (direct coalesced stores)
     long long pitch;       // row pitch in elements
     const void* src;       // compact source window, [p - sp0][line - sl0] (line fastest), or NULL
@@ -193,7 +196,23 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     }
     __syncthreads();
 
-    const int pc_begin = a.cta_off[blockIdx.x], pc_end = a.cta_off[blockIdx.x + 1];
+    // ---- work queue: a CTA first works its own share of the pieces, then draws more from the half-step's
+    // ticket counter.  Thread 0 draws one piece ahead of the producer cursor into a ring in shared memory;
+    // the other threads read an entry only after a later CTA barrier.
+    constexpr int QR = 16;
+    __shared__ int s_q[QR];
+    int* const ticket = a.tickets + nh;
+    int own_next = a.cta_off[blockIdx.x];
+    const int own_end = a.cta_off[blockIdx.x + 1], nstatic = a.nstatic;
+    auto draw = [&]() -> int {   // thread 0: the next piece of this CTA: its own share first, then the queue
+        return own_next < own_end ? own_next++ : nstatic + atomicAdd(ticket, 1);
+    };
+    if (threadIdx.x == 0) {
+        s_q[0] = draw();
+        s_q[1] = draw();
+    }
+    __syncthreads();
+    const int npieces = a.npieces;
     const int nbk = a.nbk, n = a.n, kb = a.kb, nlines = a.nlines;
     const long long pitch = a.pitch;
     [[maybe_unused]] T* const out_lane = reinterpret_cast<T*>(a.out) + (threadIdx.x & 31);
@@ -204,11 +223,12 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     // The TMA requests of a stage are spread over the warps (lane 0 of each issues its own tile), so that no
     // warp is late at the next barrier; thread 0 posts the stage's byte count on the mbarrier.
     const int sub = DIR == 0 ? warp % SUB : 0, tix = DIR == 0 ? warp / SUB : warp;
-    int q_pi = pc_begin, q_s = 0, q_slot = 0;
+    int q_ord = 0, q_s = 0, q_slot = 0;   // ordinal of the producer's piece in this CTA's sequence
+    int q_id = s_q[0];
     Piece q_pc = Piece{0, 0, 0, 0};
-    if (pc_begin < pc_end) q_pc = a.pieces[pc_begin];
-    auto produce = [&]() {   // request the next stage into slot q_slot (which must be free)
-        if (q_pi >= pc_end) return;
+    if (q_id < npieces) q_pc = a.pieces[q_id];
+    auto produce = [&]() -> bool {   // request the next stage into slot q_slot (which must be free)
+        if (q_id >= npieces) return false;
         if (lane == 0) {
             const int line0 = q_pc.panel * TL;
             const int g0 = (max(q_pc.ua - nbk, 0) & ~(SUB - 1)) + q_s * NW;
@@ -232,11 +252,17 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
         q_slot = q_slot + 1 == NSTAGE ? 0 : q_slot + 1;
         if (++q_s == q_pc.nst) {
             q_s = 0;
-            if (++q_pi < pc_end) q_pc = a.pieces[q_pi];
+            ++q_ord;
+            q_id = s_q[q_ord & (QR - 1)];
+            if (q_id < npieces) q_pc = a.pieces[q_id];
+            if (threadIdx.x == 0) s_q[(q_ord + 1) & (QR - 1)] = draw();   // read after a later CTA barrier
+            return true;
         }
+        return false;
     };
 #pragma unroll
-    for (int s = 0; s < NSTAGE; ++s) produce();
+    for (int s = 0; s < NSTAGE; ++s)
+        if (produce()) __syncthreads();
 
     // ---- consumers (all warps)
     const T rho = static_cast<T>(row[ROW_RHO]), inv = static_cast<T>(row[ROW_INV]);
@@ -327,8 +353,10 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 #pragma unroll
         for (int e = 0; e < (DEF ? U : 1); ++e) pend[e] = T(0);
 
-        for (int pi = pc_begin; pi < pc_end; ++pi) {
-            const Piece pc = a.pieces[pi];
+        for (int ord = 0;; ++ord) {
+            const int pid = s_q[ord & (QR - 1)];
+            if (pid >= npieces) break;
+            const Piece pc = a.pieces[pid];
             const int line0 = pc.panel * TL, line = line0 + lane;
             const int gbase = max(pc.ua - nbk, 0) & ~(SUB - 1);
             const bool src_tile = a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
@@ -462,7 +490,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             t[0] = t_start;
             t[1] = globaltimer_ns();
             t[2] = smid();
-            t[3] = static_cast<unsigned long long>(pc_end - pc_begin);
+            t[3] = static_cast<unsigned long long>(q_ord);
         }
     }
 }

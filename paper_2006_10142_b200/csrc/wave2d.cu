@@ -105,7 +105,8 @@ struct DirPlan {
     const Variant* var = nullptr;
     int n = 0, nlines = 0, npanels = 0, total_units = 0, grid = 0, ctas_per_sm = 0, quota = 0;
     std::vector<Piece> pieces;
-    std::vector<int> cta_off;
+    std::vector<int> cta_off;   // CTA b's static share: pieces [cta_off[b], cta_off[b+1]); pieces >= nstatic are drawn
+    int nstatic = 0;
 };
 
 }  // namespace
@@ -133,7 +134,9 @@ struct wave2d_s {
     DirPlan plan[2];
     CUtensorMap tm_load[2][3], tm_store[3], tm_edge[3];   // [dir][buffer]; x: load tile, store tile, 16-byte edge box
     Piece* d_pieces[2] = {nullptr, nullptr};
+    int* d_tickets = nullptr;              // one work-queue counter per half-step
     int* d_cta_off[2] = {nullptr, nullptr};
+    double opt_static_frac = 0.75;
     int opt_trace = 0;
     unsigned long long* d_trace[2] = {nullptr, nullptr};   // per-CTA trace of the last launch per direction
     cudaGraphExec_t gexec = nullptr;
@@ -242,38 +245,54 @@ int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, int 
     return WAVE2D_OK;
 }
 
-// Cut the (panel, unit) space into pieces, `quota` stages per CTA.  A cut costs 2 nbk extra units (carry warm-up
-// before the cut, look-ahead after it).  Returns false if a CTA could make no progress (quota too small).
-bool build_pieces(DirPlan& P, int nw, int sub, int quota)
+// Cut the (panel, unit) space into pieces of work (panel-major).  A cut costs 2 nbk extra units (carry warm-up
+// before the cut, look-ahead after it).  The first part of the space is dealt out statically, `quota` stages to
+// each of `slots` CTAs (cta_off); the rest is cut into short pieces that the CTAs draw from an atomic ticket
+// counter once their own share is done, so that CTAs the memory system serves more slowly get less of it.  The
+// short pieces follow guided self-scheduling (remaining / (2 slots) stages, between 2 and 6).
+// `fixed` > 0 (tests): no static part, every piece `fixed` stages long.
+void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double static_frac)
 {
     P.pieces.clear();
     P.cta_off.assign(1, 0);
-    const int UT = P.total_units;
+    const int UT = P.total_units, SL = (UT + nw - 1) / nw;
+    const int min_st = std::max(2, (2 * P.nbk + sub) / nw + 1);   // a piece must get past its own warm-up
+    const long long total = (long long)P.npanels * SL;
     int panel = 0, ua = 0;
-    while (panel < P.npanels) {
-        int left = quota;
-        while (left > 0 && panel < P.npanels) {
-            const int ua0 = std::max(ua - P.nbk, 0) / sub * sub;   // stages start on a load-tile boundary
-            const int rest = (UT - ua0 + nw - 1) / nw;
-            if (rest <= left) {
-                P.pieces.push_back(Piece{panel, ua, UT, rest});
-                left -= rest;
-                ++panel;
-                ua = 0;
-            } else {
-                const int ub = ua0 + left * nw - P.nbk;
-                if (ub <= ua) {
-                    if (left == quota) return false;
-                    break;
-                }
-                P.pieces.push_back(Piece{panel, ua, ub, left});
-                ua = ub;
-                left = 0;
-            }
+    auto take = [&](int st) {   // append the next piece of about st stages of the current line
+        const int ua0 = std::max(ua - P.nbk, 0) / sub * sub;   // stages start on a load-tile boundary
+        const int rest = (UT - ua0 + nw - 1) / nw;
+        int ub = UT, nst = rest;
+        if (rest > st + (st + 1) / 2) {
+            ub = ua0 + st * nw - P.nbk;
+            nst = st;
         }
-        P.cta_off.push_back((int)P.pieces.size());
+        P.pieces.push_back(Piece{panel, ua, ub, nst});
+        ua = ub;
+        if (ua >= UT) { ++panel; ua = 0; }
+        return nst;
+    };
+    const int quota = fixed > 0 ? 0 : (int)(static_frac * (double)total / slots);
+    if (quota >= 2 * min_st && total >= 4LL * slots) {
+        for (int c = 0; c < slots && panel < P.npanels; ++c) {
+            int left = quota;
+            while (left >= min_st && panel < P.npanels) left -= take(left);
+            P.cta_off.push_back((int)P.pieces.size());
+        }
     }
-    return true;
+    P.nstatic = (int)P.pieces.size();
+    double remaining = 0.0;
+    if (panel < P.npanels) remaining = (double)(P.npanels - panel) * SL - (double)ua / nw;
+    while (panel < P.npanels) {
+        int st = fixed > 0 ? fixed : std::min(6, (int)(remaining / (2.0 * slots)));
+        st = std::max(st, min_st);
+        const int ua_before = ua, panel_before = panel;
+        take(st);
+        const Piece& pc = P.pieces.back();
+        (void)ua_before; (void)panel_before;
+        remaining -= (double)(pc.ub - pc.ua) / nw;
+    }
+    while ((int)P.cta_off.size() < slots + 1) P.cta_off.push_back(P.nstatic);   // CTAs without a static share
 }
 
 int plan_dir(wave2d_t* h, int d)
@@ -331,17 +350,11 @@ int plan_dir(wave2d_t* h, int d)
     P.ctas_per_sm = per_sm;
     P.npanels = (P.nlines + 31) / 32;
     P.total_units = (P.n + U - 1) / U;
-    // Persistent grid, one wave: the smallest per-CTA quota of stages whose pieces fit the resident CTA slots.
+    // Persistent grid, one wave; the CTAs draw the pieces from an atomic ticket counter.
     const int slots = per_sm * h->num_sms;
-    const long long total = (long long)P.npanels * ((P.total_units + V.nw - 1) / V.nw);
-    int quota = (int)std::max<long long>(1, (total + slots - 1) / slots);
-    if (h->opt_quota[d] > 0) quota = h->opt_quota[d];
-    for (;; ++quota) {
-        if (!build_pieces(P, V.nw, V.sub, quota)) continue;
-        if (h->opt_quota[d] > 0 || (int)P.cta_off.size() - 1 <= slots) break;
-    }
-    P.quota = quota;
-    P.grid = (int)P.cta_off.size() - 1;
+    build_pieces(P, V.nw, V.sub, slots, h->opt_quota[d], h->opt_static_frac);
+    P.quota = h->opt_quota[d];
+    P.grid = slots;
     return WAVE2D_OK;
 }
 
@@ -395,9 +408,9 @@ int ensure_plan(wave2d_t* h)
         st = dev_alloc(h, reinterpret_cast<void**>(&h->d_pieces[d]), pb);
         if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_cta_off[d]), ob);
         if (st) return st;
+        W2D_CUDA(h, cudaMemcpy(h->d_cta_off[d], P.cta_off.data(), ob, cudaMemcpyHostToDevice));
         if (!P.pieces.empty())
             W2D_CUDA(h, cudaMemcpy(h->d_pieces[d], P.pieces.data(), P.pieces.size() * sizeof(Piece), cudaMemcpyHostToDevice));
-        W2D_CUDA(h, cudaMemcpy(h->d_cta_off[d], P.cta_off.data(), ob, cudaMemcpyHostToDevice));
         if (h->opt_trace) {
             st = dev_alloc(h, reinterpret_cast<void**>(&h->d_trace[d]), (size_t)P.grid * 16 * sizeof(unsigned long long));
             if (st) return st;
@@ -429,7 +442,8 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         SweepArgs a;
         a.table = h->d_table; a.d_k = dk; a.n_off = n_off;
         a.n = P.n; a.nlines = P.nlines; a.nbk = P.nbk; a.kb = P.kb;
-        a.pieces = h->d_pieces[d]; a.cta_off = h->d_cta_off[d];
+        a.pieces = h->d_pieces[d]; a.npieces = (int)P.pieces.size(); a.tickets = h->d_tickets;
+        a.cta_off = h->d_cta_off[d]; a.nstatic = P.nstatic;
         a.out = out; a.pitch = h->pitch;
         a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
         a.g2 = 2.0 * h->gamma;
@@ -573,9 +587,12 @@ int wave2d_create(wave2d_t** out, int N1, int N2, double l, double tau, int M, i
     int st = WAVE2D_OK;
     for (int b = 0; b < 3 && st == WAVE2D_OK; ++b) st = dev_alloc(h, &h->buf[b], fbytes);
     if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_k), sizeof(int));
+    const size_t tk_bytes = ((size_t)2 * M + 2) * sizeof(int);
+    if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_tickets), tk_bytes);
     if (st == WAVE2D_OK) {
         for (int b = 0; b < 3; ++b) cudaMemsetAsync(h->buf[b], 0, fbytes, h->stream);
         cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream);
+        cudaMemsetAsync(h->d_tickets, 0, tk_bytes, h->stream);
         if (cudaStreamSynchronize(h->stream) != cudaSuccess) st = WAVE2D_ERR_CUDA;
     }
     if (st != WAVE2D_OK) {
@@ -604,6 +621,7 @@ void wave2d_destroy(wave2d_t* h)
         cudaFree(h->d_cta_off[d]);
         cudaFree(h->d_trace[d]);
     }
+    cudaFree(h->d_tickets);
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
     (void)cudaGetLastError();
     delete h;
@@ -631,6 +649,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "shape_x")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[0] = iv; }
     else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
     else if (!strcmp(name, "trace")) h->opt_trace = iv != 0;
+    else if (!strcmp(name, "static_frac")) { if (!(value >= 0.0 && value <= 1.0)) return WAVE2D_ERR_ARG; h->opt_static_frac = value; }
     else if (!strcmp(name, "quota_x")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[0] = iv; }
     else if (!strcmp(name, "quota_y")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[1] = iv; }
     else return WAVE2D_ERR_ARG;
@@ -659,6 +678,7 @@ int wave2d_set_initial(wave2d_t* h, const void* phi, const void* psi, long ld)
                                                             h->pitch, 0.5 * h->tau);
     W2D_CUDA(h, cudaGetLastError());
     W2D_CUDA(h, cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream));
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)2 * h->M + 2) * sizeof(int), h->stream));   // work queues
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_initial = true;
     h->k = 0;
