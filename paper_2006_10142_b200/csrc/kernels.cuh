@@ -306,6 +306,11 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
         if (gp < pc.ua || gp >= pc.ub) return;    // warp-uniform
         const int pp0 = gp * U;
         const bool full = pp0 + U <= n;
+#ifdef W2D_COPY_PROBE
+        if (true) {
+            v[0] += Xin;
+        } else
+#endif
         if (gp >= kb && full) {
 #pragma unroll
             for (int e = 0; e < U; ++e) v[e] = fma(pw_at(U - 1 - e), Xin, v[e]);
@@ -399,6 +404,14 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 // ---- RHS + local forward elimination
                 const bool fast = g >= kb && p0 + U <= n;   // stationary pivots, whole unit inside the line
                 T Aval;
+#ifdef W2D_COPY_PROBE   // bandwidth probe (not the method): same data movement and barriers, no solve
+                if (true) {
+#pragma unroll
+                    for (int e = 0; e < U; ++e) xl[e] = wp[e] + wc[e];
+                    xl[0] += wl + wr;
+                    Aval = T(0);
+                } else
+#endif
                 if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
 #pragma unroll
                     for (int e = 0; e < U; ++e) {
@@ -442,6 +455,11 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 
                 // ---- carry from the left, local back substitution
                 const T Yin = carry(sL_lane, ring, -1);   // y at the end of unit g-1
+#ifdef W2D_COPY_PROBE
+                if (true) {
+                    xl[0] += Yin;
+                } else
+#endif
                 if (fast) {
                     xl[U - 1] = fma(pw_at(U - 1), Yin, xl[U - 1]);
 #pragma unroll
