@@ -90,6 +90,8 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "graph"  1 (default): the step loop is replayed as a CUDA Graph; 0: plain launches.
  *   "graph_steps"  time steps per graph replay (multiple of 3, the period of the buffer ring).  Default 12.
  *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (units per stage = consumer warps / stages).
+ *   "pdl"    1 (default): sweep kernels are launched with programmatic stream serialization, so that a kernel's
+ *            prologue overlaps the tail of the previous one (it waits for it before touching the fields).
  *   "trace"  1: sweep kernels record per-CTA timing (see wave2d_get_trace).  Default 0.
  *   "quota_x", "quota_y"   tuning: length in stages of every piece of work a line is cut into (0 = planned:
  *                          guided self-scheduling, long pieces first, short ones last).

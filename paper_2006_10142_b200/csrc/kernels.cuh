@@ -201,6 +201,10 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     // the other threads read an entry only after a later CTA barrier.
     constexpr int QR = 16;
     __shared__ int s_q[QR];
+    // Everything above touched only data no earlier kernel writes (the scalar table, the step counter, which
+    // changes between graph launches only).  From here on the fields of the previous half-step are read.
+    pdl_launch_dependents();
+    pdl_wait();
     int* const ticket = a.tickets + nh;
     int own_next = a.cta_off[blockIdx.x];
     const int own_end = a.cta_off[blockIdx.x + 1], nstatic = a.nstatic;

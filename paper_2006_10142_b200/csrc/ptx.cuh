@@ -73,6 +73,12 @@ __device__ __forceinline__ void tma_wait_read()
 // make generic-proxy writes to shared memory visible to the async proxy (before a TMA store)
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// ---- programmatic dependent launch ------------------------------------------------------------------
+// launch_dependents: the next kernel in the stream may start launching (its CTAs take SMs as ours exit);
+// wait: block until the previous kernel in the stream has completed and its writes are visible.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // ---- tracing ------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned long long globaltimer_ns()
 {
