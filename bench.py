@@ -270,26 +270,19 @@ def run_reference(args):
 
 def run_ours(args):
     import torch
-    import torch.distributed as dist
+    from paper_2006_10142_b200.replicas import Ranks
 
     rank, world, local = dist_env()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the hot path is CUDA only, there is no CPU fallback")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ranks = Ranks("nccl", torch.device("cuda", local))
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        ranks.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    max_over_ranks = ranks.max_over_ranks
 
     from paper_2006_10142_b200 import binding as B
     K, Wm = args.steps, args.warmup
@@ -410,8 +403,7 @@ def run_ours(args):
             oracle.build()
             line["cpu_baseline"] = time_oracle(w, budget_s=15.0)
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 def main():
