@@ -240,13 +240,12 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             const uint32_t dst = sm32 + q_slot * K::STAGE_BYTES;
             if (warp == 0) mbar_arrive_expect_tx(full, K::STAGE_BYTES);
             if constexpr (DIR == 0) {
-                if (sub == 0) {
-                    tma_load_2d(dst + tix * 4096, &tm_prev, (g0 + tix * SUB) * U, line0, full);
-                    tma_load_2d(dst + K::FIELD_BYTES + tix * 4096, &tm_cur, (g0 + tix * SUB) * U, line0, full);
-                }
-                if (warp == (SUB > 1 ? 1 : 0))
+                // fields: one 3D box each, [NT tiles][32 rows][128 B] = 1 KB contiguous per row in global memory
+                if (warp == 0) tma_load_3d(dst, &tm_prev, 0, line0, g0 / SUB, full);
+                if (warp == NW / 2) tma_load_3d(dst + K::FIELD_BYTES, &tm_cur, 0, line0, g0 / SUB, full);
+                if (warp == NW / 4)
                     tma_load_2d(dst + 2 * K::FIELD_BYTES, &tm_edge, g0 * U - V, line0, full);
-                if (warp == (SUB > 1 ? SUB + 1 : NW - 1))
+                if (warp == 3 * NW / 4)
                     tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
             } else {
                 if (warp == 0) tma_load_2d(dst, &tm_prev, line0, g0 * U - 1, full);

@@ -295,6 +295,34 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
     while ((int)P.cta_off.size() < slots + 1) P.cta_off.push_back(P.nstatic);   // CTAs without a static share
 }
 
+// x sweep load map: the field seen as (128-byte tile row, grid row, tile index along the row); a box of
+// [ntiles][32 rows][128 B] lands in shared memory tile after tile, each 128B-swizzled, and is 32 rows x
+// ntiles * 128 contiguous bytes in global memory.  Elements beyond n1 inside the last tile are the zero pad columns.
+int make_tmap_x3(wave2d_t* h, CUtensorMap* tm, void* base, int ntiles)
+{
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) {
+        h->err = "cuTensorMapEncodeTiled entry point not available";
+        return WAVE2D_ERR_CUDA;
+    }
+    const int tu = 128 / h->elem;
+    const cuuint64_t dims[3] = {(cuuint64_t)tu, (cuuint64_t)h->n2, (cuuint64_t)(h->pitch / tu)};
+    const cuuint64_t strides[2] = {(cuuint64_t)h->pitch * h->elem, 128};
+    const cuuint32_t box[3] = {(cuuint32_t)tu, 32, (cuuint32_t)ntiles};
+    const cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = enc(tm, h->dtype == WAVE2D_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3,
+                     base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        char msg[160];
+        snprintf(msg, sizeof msg, "cuTensorMapEncodeTiled (x sweep 3D map) failed (%d) n=%dx%d pitch=%lld", (int)r, h->n1,
+                 h->n2, h->pitch);
+        h->err = msg;
+        return WAVE2D_ERR_CUDA;
+    }
+    return WAVE2D_OK;
+}
+
 int plan_dir(wave2d_t* h, int d)
 {
     DirPlan& P = h->plan[d];
@@ -384,7 +412,7 @@ int ensure_plan(wave2d_t* h)
     for (int b = 0; b < 3; ++b) {
         if (h->plan[0].solver == WAVE2D_SOLVER_STREAM) {
             const int U = h->plan[0].var->unit;
-            st = make_tmap(h, &h->tm_load[0][b], h->buf[b], 128 / h->elem, 32, 128);   // load tile: 128-byte rows
+            st = make_tmap_x3(h, &h->tm_load[0][b], h->buf[b], h->plan[0].var->nw / h->plan[0].var->sub);
             if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_store[b], h->buf[b], U, 32, U * h->elem);   // one warp's unit
             if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_edge[b], h->buf[b], 16 / h->elem, 32, 0);
             if (st) return st;
