@@ -197,8 +197,8 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     __syncthreads();
 
     // ---- work queue: a CTA first works its own share of the pieces, then draws more from the half-step's
-    // ticket counter.  Thread 0 draws one piece ahead of the producer cursor into a ring in shared memory;
-    // the other threads read an entry only after a later CTA barrier.
+    // ticket counter.  Thread 0 draws for the producer cursor into a ring in shared memory; the other threads
+    // read an entry only after a CTA barrier.
     constexpr int QR = 16;
     __shared__ int s_q[QR];
     // Everything above touched only data no earlier kernel writes (the scalar table, the step counter, which
@@ -211,10 +211,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     auto draw = [&]() -> int {   // thread 0: the next piece of this CTA: its own share first, then the queue
         return own_next < own_end ? own_next++ : nstatic + atomicAdd(ticket, 1);
     };
-    if (threadIdx.x == 0) {
-        s_q[0] = draw();
-        s_q[1] = draw();
-    }
+    if (threadIdx.x == 0) s_q[0] = draw();
     __syncthreads();
     const int npieces = a.npieces;
     const int nbk = a.nbk, n = a.n, kb = a.kb, nlines = a.nlines;
@@ -231,8 +228,8 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     int q_id = s_q[0];
     Piece q_pc = Piece{0, 0, 0, 0};
     if (q_id < npieces) q_pc = a.pieces[q_id];
-    auto produce = [&]() -> bool {   // request the next stage into slot q_slot (which must be free)
-        if (q_id >= npieces) return false;
+    auto produce = [&]() {   // request the next stage into slot q_slot (which must be free)
+        if (q_id >= npieces) return;
         if (lane == 0) {
             const int line0 = q_pc.panel * TL;
             const int g0 = (max(q_pc.ua - nbk, 0) & ~(SUB - 1)) + q_s * NW;
@@ -258,14 +255,20 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             ++q_ord;
             q_id = s_q[q_ord & (QR - 1)];
             if (q_id < npieces) q_pc = a.pieces[q_id];
-            if (threadIdx.x == 0) s_q[(q_ord + 1) & (QR - 1)] = draw();   // read after a later CTA barrier
-            return true;
         }
-        return false;
+    };
+    // Thread 0 draws the producer's next piece as late as possible: in the stage whose produce() call finishes
+    // the current piece, before that stage's CTA barrier (produce() runs right after it).
+    auto will_advance = [&]() -> bool { return q_id < npieces && q_s + 1 == q_pc.nst; };
+    auto draw_ahead = [&]() {
+        if (threadIdx.x == 0 && will_advance()) s_q[(q_ord + 1) & (QR - 1)] = draw();
     };
 #pragma unroll
-    for (int s = 0; s < NSTAGE; ++s)
-        if (produce()) __syncthreads();
+    for (int s = 0; s < NSTAGE; ++s) {
+        draw_ahead();
+        if (will_advance()) __syncthreads();
+        produce();
+    }
 
     // ---- consumers (all warps)
     const T rho = static_cast<T>(row[ROW_RHO]), inv = static_cast<T>(row[ROW_INV]);
@@ -381,6 +384,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 T xl[U];
                 // ---- shared memory -> registers
                 mbar_wait(bar32 + 8 * slot, phase);
+                draw_ahead();   // (thread 0) the ticket's round trip overlaps this stage's first half
                 const unsigned char* st = sm + slot * K::STAGE_BYTES;
                 if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
                 T wp[U], wc[U], wl, wr;

@@ -54,8 +54,8 @@ void add_shapes_f32(std::vector<Variant>& v)
     v.push_back(make_variant<float, 0, 16, 8, 2, 2>());
     v.push_back(make_variant<float, 0, 32, 8, 2>());
     v.push_back(make_variant<float, 0, 8, 16, 2>());
-    v.push_back(make_variant<float, 1, 8, 16, 3>());
     v.push_back(make_variant<float, 1, 8, 8, 3, 2>());
+    v.push_back(make_variant<float, 1, 8, 16, 3>());
     v.push_back(make_variant<float, 1, 16, 8, 3>());
     v.push_back(make_variant<float, 1, 8, 16, 4>());
 }
@@ -136,7 +136,8 @@ struct wave2d_s {
     Piece* d_pieces[2] = {nullptr, nullptr};
     int* d_tickets = nullptr;              // one work-queue counter per half-step
     int* d_cta_off[2] = {nullptr, nullptr};
-    double opt_static_frac = 0.75;
+    double opt_static_frac = 0.75, opt_tail_div = 2.0;
+    int opt_tail_min = 2;
     int opt_trace = 0, opt_pdl = 1;
     unsigned long long* d_trace[2] = {nullptr, nullptr};   // per-CTA trace of the last launch per direction
     cudaGraphExec_t gexec = nullptr;
@@ -251,12 +252,12 @@ int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, int 
 // counter once their own share is done, so that CTAs the memory system serves more slowly get less of it.  The
 // short pieces follow guided self-scheduling (remaining / (2 slots) stages, between 2 and 6).
 // `fixed` > 0 (tests): no static part, every piece `fixed` stages long.
-void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double static_frac)
+void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double static_frac, int tail_min, double tail_div)
 {
     P.pieces.clear();
     P.cta_off.assign(1, 0);
     const int UT = P.total_units, SL = (UT + nw - 1) / nw;
-    const int min_st = std::max(2, (2 * P.nbk + sub) / nw + 1);   // a piece must get past its own warm-up
+    const int min_st = std::max(tail_min, (2 * P.nbk + sub) / nw + 1);   // a piece must get past its own warm-up
     const long long total = (long long)P.npanels * SL;
     int panel = 0, ua = 0;
     auto take = [&](int st) {   // append the next piece of about st stages of the current line
@@ -284,7 +285,7 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
     double remaining = 0.0;
     if (panel < P.npanels) remaining = (double)(P.npanels - panel) * SL - (double)ua / nw;
     while (panel < P.npanels) {
-        int st = fixed > 0 ? fixed : std::min(6, (int)(remaining / (2.0 * slots)));
+        int st = fixed > 0 ? fixed : std::min(6, (int)(remaining / (tail_div * slots)));
         st = std::max(st, min_st);
         const int ua_before = ua, panel_before = panel;
         take(st);
@@ -380,7 +381,7 @@ int plan_dir(wave2d_t* h, int d)
     P.total_units = (P.n + U - 1) / U;
     // Persistent grid, one wave; the CTAs draw the pieces from an atomic ticket counter.
     const int slots = per_sm * h->num_sms;
-    build_pieces(P, V.nw, V.sub, slots, h->opt_quota[d], h->opt_static_frac);
+    build_pieces(P, V.nw, V.sub, slots, h->opt_quota[d], h->opt_static_frac, h->opt_tail_min, h->opt_tail_div);
     P.quota = h->opt_quota[d];
     P.grid = slots;
     return WAVE2D_OK;
@@ -688,6 +689,8 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
     else if (!strcmp(name, "trace")) h->opt_trace = iv != 0;
     else if (!strcmp(name, "pdl")) h->opt_pdl = iv != 0;
+    else if (!strcmp(name, "tail_min")) { if (iv < 1) return WAVE2D_ERR_ARG; h->opt_tail_min = iv; }
+    else if (!strcmp(name, "tail_div")) { if (!(value >= 0.25)) return WAVE2D_ERR_ARG; h->opt_tail_div = value; }
     else if (!strcmp(name, "static_frac")) { if (!(value >= 0.0 && value <= 1.0)) return WAVE2D_ERR_ARG; h->opt_static_frac = value; }
     else if (!strcmp(name, "quota_x")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[0] = iv; }
     else if (!strcmp(name, "quota_y")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[1] = iv; }
