@@ -169,6 +169,26 @@ int wave2d_profile_sweeps(wave2d_t *h, int steps, double *ms_x, double *ms_y);
  */
 int wave2d_get_trace(wave2d_t *h, int dir, unsigned long long *out, int capacity, int *count);
 
+/*
+ * Host-only planning logic, exposed for inspection and tests; no device is touched.
+ *
+ * wave2d_host_scalars: the per-half-step scalar row for alpha+ = tau^2 c_{n+1}/(2 h^2),
+ * alpha- = tau^2 c_{n-1}/(2 h^2), q = kappa tau^2 g_n ((2.11)-(2.12) times tau^2).  out[0..7] =
+ * alpha-, q, rho, 1/(beta - alpha+ rho), -(gamma + 2 alpha-), alpha+, beta = gamma + 2 alpha+, 0; then K boundary
+ * values cp_p = alpha+/u_pp and K values inv_p = 1/u_pp, u_pp the LU pivots of tridiag(-alpha+, beta, -alpha+),
+ * K = (*count - 8) / 2.  Errors: ERR_ARG (also capacity < *count).
+ *
+ * wave2d_host_plan: how a sweep over `nlines` lines of n unknowns is cut into pieces of work for `slots` CTAs
+ * (DESIGN.md 8.1): pieces[4 i ..] = (panel of 32 lines, first output unit, end output unit, stages); pieces
+ * [0, *nstatic) are dealt out statically, CTA c owning [cta_off[c], cta_off[c+1]) (cta_off has slots + 1
+ * entries), the rest is drawn at run time.  fixed_stages > 0: every piece that many stages, nothing static.
+ */
+int wave2d_host_scalars(double gamma, double alpha_plus, double alpha_minus, double q, double *out, int capacity,
+                        int *count);
+int wave2d_host_plan(int n, int nlines, int unit, int units_per_stage, int units_per_tile, int nbk, int slots,
+                     int fixed_stages, double static_frac, int *pieces, int capacity, int *npieces, int *nstatic,
+                     int *cta_off);
+
 const char *wave2d_strerror(int status);
 const char *wave2d_last_error(const wave2d_t *h);
 

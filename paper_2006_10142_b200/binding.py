@@ -21,7 +21,7 @@ EXPORTS = [
     "wave2d_create", "wave2d_destroy", "wave2d_set_stream", "wave2d_set_option", "wave2d_set_initial",
     "wave2d_set_speed", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
     "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
-    "wave2d_strerror", "wave2d_last_error",
+    "wave2d_host_scalars", "wave2d_host_plan", "wave2d_strerror", "wave2d_last_error",
 ]
 
 
@@ -62,6 +62,9 @@ def load_library() -> C.CDLL:
     L.wave2d_get_info.argtypes = [vp, C.c_char_p, dp]
     L.wave2d_profile_sweeps.argtypes = [vp, C.c_int, dp, dp]
     L.wave2d_get_trace.argtypes = [vp, C.c_int, vp, C.c_int, C.POINTER(C.c_int)]
+    ip = C.POINTER(C.c_int)
+    L.wave2d_host_scalars.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, dp, C.c_int, ip]
+    L.wave2d_host_plan.argtypes = [C.c_int] * 8 + [C.c_double, ip, C.c_int, ip, ip, ip]
     L.wave2d_strerror.argtypes = [C.c_int]
     L.wave2d_strerror.restype = C.c_char_p
     L.wave2d_last_error.argtypes = [vp]
@@ -229,3 +232,32 @@ def from_workload(w, dtype=None, solver=None, graph=None) -> "Wave2D":
         h.set_source(w.s.astype(npdt, copy=False), w.g_half)
     h.set_initial(w.phi.astype(npdt, copy=False), None if w.psi is None else w.psi.astype(npdt, copy=False))
     return h
+
+
+def host_scalars(gamma: float, alpha_plus: float, alpha_minus: float, q: float = 0.0) -> np.ndarray:
+    """wave2d_host_scalars: the scalar row of one half-step (host only, no device)."""
+    L = load_library()
+    out = np.zeros(4096, dtype=np.float64)
+    cnt = C.c_int()
+    st = L.wave2d_host_scalars(gamma, alpha_plus, alpha_minus, q, out.ctypes.data_as(C.POINTER(C.c_double)),
+                               out.size, C.byref(cnt))
+    if st != 0:
+        raise Wave2DError(st, "wave2d_host_scalars", L.wave2d_strerror(st).decode())
+    return out[:cnt.value].copy()
+
+
+def host_plan(n: int, nlines: int, unit: int, units_per_stage: int, units_per_tile: int, nbk: int, slots: int,
+              fixed_stages: int = 0, static_frac: float = 0.75):
+    """wave2d_host_plan: (pieces[npieces, 4], nstatic, cta_off[slots + 1]) (host only, no device)."""
+    L = load_library()
+    cap = 1 << 20
+    pieces = np.zeros((cap, 4), dtype=np.int32)
+    cta_off = np.zeros(slots + 1, dtype=np.int32)
+    npieces, nstatic = C.c_int(), C.c_int()
+    ip = C.POINTER(C.c_int)
+    st = L.wave2d_host_plan(n, nlines, unit, units_per_stage, units_per_tile, nbk, slots, fixed_stages,
+                            float(static_frac), pieces.ctypes.data_as(ip), cap, C.byref(npieces), C.byref(nstatic),
+                            cta_off.ctypes.data_as(ip))
+    if st != 0:
+        raise Wave2DError(st, "wave2d_host_plan", L.wave2d_strerror(st).decode())
+    return pieces[:npieces.value].copy(), nstatic.value, cta_off

@@ -189,33 +189,38 @@ void invalidate_plan(wave2d_t* h)
 }
 
 // ---- A0: per-half-step scalars, fp64 on the host -----------------------------------------
+// One table row: half-step with alpha+ = ap, alpha- = am, source factor qv (0 without a source).
+void fill_row(double* row, double gamma, double ap, double am, double qv)
+{
+    const double beta = gamma + 2.0 * ap;
+    const double rho = 2.0 * ap / (beta + std::sqrt(beta * beta - 4.0 * ap * ap));   // small root of ap z^2 - beta z + ap
+    row[ROW_AM] = am;
+    row[ROW_Q] = qv;
+    row[ROW_RHO] = rho;
+    row[ROW_INV] = 1.0 / (beta - ap * rho);
+    row[ROW_C1] = -(gamma + 2.0 * am);
+    row[ROW_AP] = ap;
+    row[ROW_BETA] = beta;
+    double cp = 0.0;
+    for (int p = 0; p < KMAX; ++p) {   // LU pivots of tridiag(-ap, beta, -ap): inv_p = 1/u_pp, cp_p = ap/u_pp
+        const double iv = 1.0 / (beta - ap * cp);
+        cp = ap * iv;
+        row[ROW_CP + p] = cp;
+        row[ROW_INVP + p] = iv;
+    }
+}
+
 void build_table(wave2d_t* h)
 {
     const int nhalf = 2 * h->M;
     h->table.assign(static_cast<size_t>(std::max(nhalf, 1)) * ROW_DOUBLES, 0.0);
     const double t2 = h->tau * h->tau;
     for (int n = 0; n < nhalf; ++n) {
-        double* row = &h->table[static_cast<size_t>(n) * ROW_DOUBLES];
-        const double hd = h->l / ((n & 1) == 0 ? h->N1 : h->N2);                  // reading A3
+        const double hd = h->l / ((n & 1) == 0 ? h->N1 : h->N2);                  // reading R3
         const double ap = t2 * h->c_half[n + 1] / (2.0 * hd * hd);
-        const double am = t2 * h->c_half[n > 0 ? n - 1 : 0] / (2.0 * hd * hd);      // reading A5: c_{-1} := c_0
-        const double g = h->g_half.empty() ? 1.0 : h->g_half[n];                   // reading A8
-        const double beta = h->gamma + 2.0 * ap;
-        const double rho = 2.0 * ap / (beta + std::sqrt(beta * beta - 4.0 * ap * ap));
-        row[ROW_AM] = am;
-        row[ROW_Q] = h->have_src ? h->kappa * t2 * g : 0.0;
-        row[ROW_RHO] = rho;
-        row[ROW_INV] = 1.0 / (beta - ap * rho);
-        row[ROW_C1] = -(h->gamma + 2.0 * am);
-        row[ROW_AP] = ap;
-        row[ROW_BETA] = beta;
-        double cp = 0.0;
-        for (int p = 0; p < KMAX; ++p) {
-            const double iv = 1.0 / (beta - ap * cp);
-            cp = ap * iv;
-            row[ROW_CP + p] = cp;
-            row[ROW_INVP + p] = iv;
-        }
+        const double am = t2 * h->c_half[n > 0 ? n - 1 : 0] / (2.0 * hd * hd);      // reading R5: c_{-1} := c_0
+        const double g = h->g_half.empty() ? 1.0 : h->g_half[n];                   // reading R8
+        fill_row(&h->table[static_cast<size_t>(n) * ROW_DOUBLES], h->gamma, ap, am, h->have_src ? h->kappa * t2 * g : 0.0);
     }
 }
 
@@ -260,11 +265,11 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
     const int min_st = std::max(tail_min, (2 * P.nbk + sub) / nw + 1);   // a piece must get past its own warm-up
     const long long total = (long long)P.npanels * SL;
     int panel = 0, ua = 0;
-    auto take = [&](int st) {   // append the next piece of about st stages of the current line
+    auto take = [&](int st, int slack) {   // append the next piece of st stages (up to st + slack if that ends the line)
         const int ua0 = std::max(ua - P.nbk, 0) / sub * sub;   // stages start on a load-tile boundary
         const int rest = (UT - ua0 + nw - 1) / nw;
         int ub = UT, nst = rest;
-        if (rest > st + (st + 1) / 2) {
+        if (rest > st + slack) {
             ub = ua0 + st * nw - P.nbk;
             nst = st;
         }
@@ -277,7 +282,7 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
     if (quota >= 2 * min_st && total >= 4LL * slots) {
         for (int c = 0; c < slots && panel < P.npanels; ++c) {
             int left = quota;
-            while (left >= min_st && panel < P.npanels) left -= take(left);
+            while (left >= min_st && panel < P.npanels) left -= take(left, 1);
             P.cta_off.push_back((int)P.pieces.size());
         }
     }
@@ -288,7 +293,7 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
         int st = fixed > 0 ? fixed : std::min(6, (int)(remaining / (tail_div * slots)));
         st = std::max(st, min_st);
         const int ua_before = ua, panel_before = panel;
-        take(st);
+        take(st, (st + 1) / 2);
         const Piece& pc = P.pieces.back();
         (void)ua_before; (void)panel_before;
         remaining -= (double)(pc.ub - pc.ua) / nw;
@@ -928,6 +933,41 @@ int wave2d_get_trace(wave2d_t* h, int dir, unsigned long long* out, int capacity
     if (capacity < g) return WAVE2D_ERR_ARG;
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     W2D_CUDA(h, cudaMemcpy(out, h->d_trace[dir], (size_t)g * 16 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    return WAVE2D_OK;
+}
+
+// ---- host-only entry points (no device needed): the planning logic, for inspection and tests ----------------
+int wave2d_host_scalars(double gamma, double alpha_plus, double alpha_minus, double q, double* out, int capacity,
+                        int* count)
+{
+    if (!out || !count || !(gamma > 0.0) || !(alpha_plus > 0.0) || !(alpha_minus >= 0.0)) return WAVE2D_ERR_ARG;
+    *count = ROW_DOUBLES;
+    if (capacity < ROW_DOUBLES) return WAVE2D_ERR_ARG;
+    fill_row(out, gamma, alpha_plus, alpha_minus, q);
+    return WAVE2D_OK;
+}
+
+int wave2d_host_plan(int n, int nlines, int unit, int units_per_stage, int units_per_tile, int nbk, int slots,
+                     int fixed_stages, double static_frac, int* pieces, int capacity, int* npieces, int* nstatic,
+                     int* cta_off)
+{
+    if (n < 1 || nlines < 1 || unit < 1 || units_per_stage < 1 || units_per_tile < 1 || nbk < 1 ||
+        nbk > units_per_stage || slots < 1 || fixed_stages < 0 || !(static_frac >= 0.0 && static_frac <= 1.0) ||
+        !pieces || !npieces || !nstatic || !cta_off)
+        return WAVE2D_ERR_ARG;
+    DirPlan P;
+    P.n = n; P.nlines = nlines; P.nbk = nbk;
+    P.npanels = (nlines + 31) / 32;
+    P.total_units = (n + unit - 1) / unit;
+    build_pieces(P, units_per_stage, units_per_tile, slots, fixed_stages, static_frac, 2, 2.0);
+    *npieces = (int)P.pieces.size();
+    *nstatic = P.nstatic;
+    if (capacity < *npieces) return WAVE2D_ERR_ARG;
+    for (size_t i = 0; i < P.pieces.size(); ++i) {
+        pieces[4 * i] = P.pieces[i].panel; pieces[4 * i + 1] = P.pieces[i].ua;
+        pieces[4 * i + 2] = P.pieces[i].ub; pieces[4 * i + 3] = P.pieces[i].nst;
+    }
+    for (int c = 0; c <= slots; ++c) cta_off[c] = P.cta_off[c];
     return WAVE2D_OK;
 }
 
