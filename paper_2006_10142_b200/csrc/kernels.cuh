@@ -209,7 +209,8 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     int own_next = a.cta_off[blockIdx.x];
     const int own_end = a.cta_off[blockIdx.x + 1], nstatic = a.nstatic;
     auto draw = [&]() -> int {   // thread 0: the next piece of this CTA: its own share first, then the queue
-        return own_next < own_end ? own_next++ : nstatic + atomicAdd(ticket, 1);
+        if (own_next < own_end) return own_next++;
+        return nstatic < a.npieces ? nstatic + atomicAdd(ticket, 1) : nstatic;   // nothing to draw: no round trip
     };
     if (threadIdx.x == 0) s_q[0] = draw();
     __syncthreads();

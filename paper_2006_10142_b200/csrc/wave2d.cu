@@ -287,6 +287,17 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
         }
     }
     P.nstatic = (int)P.pieces.size();
+    if (fixed == 0 && P.nstatic == 0 && total < 4LL * slots) {
+        // Small problem (a CTA gets at most a few stages): one wave of equal pieces, at most one per CTA, because a
+        // second piece on some CTAs would double the kernel time.  k pieces per line, each st stages.
+        const int k = (int)std::max<long long>(1, std::min<long long>(slots / P.npanels, SL / min_st));
+        const int st = std::max(min_st, (UT + (k - 1) * 2 * P.nbk + k * nw - 1) / (k * nw));
+        while (panel < P.npanels) take(st, st - 1);
+        P.nstatic = (int)P.pieces.size();   // all static (CTA c owns pieces c, c + slots, ...: here just piece c):
+        const int per = (P.nstatic + slots - 1) / slots;   // no ticket is ever drawn
+        for (int c = 1; c <= slots; ++c) P.cta_off.push_back(std::min(P.nstatic, c * per));
+        return;
+    }
     double remaining = 0.0;
     if (panel < P.npanels) remaining = (double)(P.npanels - panel) * SL - (double)ua / nw;
     while (panel < P.npanels) {
