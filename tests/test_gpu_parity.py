@@ -273,3 +273,55 @@ def test_cfg5_full_size_full_M_against_modal_closed_form():
     scale = max(abs(A) for _, _, A in w.modes)
     assert np.abs(u[rows] - expect).max() <= 1e-10 * scale
     assert np.isfinite(u).all()
+
+
+def test_results_do_not_depend_on_which_cta_runs_a_piece():
+    """The pieces of the dynamic tail are drawn by whichever CTA is free, and every stage goes through two CTA
+    barriers, an mbarrier ring and double-buffered store tiles: any race or order dependence would show up as
+    run-to-run differences.  Three runs of a 2047^2 grid (several pieces per CTA) must agree bit for bit, and so
+    must runs under different work distributions (what a thread computes never depends on the cut positions of
+    other pieces)."""
+    w = W.cfg3(N=2048, M=30)
+    w.g_half = W.ricker(W.half_times(w.tau, 2 * w.M) + 0.058)
+    runs = [gpu(w)[0] for _ in range(3)]
+    assert np.array_equal(runs[0], runs[1]) and np.array_equal(runs[0], runs[2])
+    assert relerr(runs[0], ref(w)) <= 1e-10
+    other, info = gpu(w, static_frac=0.3, shape_y=3)
+    assert relerr(other, runs[0]) <= 1e-13      # different cuts: same to rounding of the carry truncation
+
+
+def test_trace_records_every_cta():
+    w = W.cfg2(N=700, M=6)
+    h = B.from_workload(w)
+    try:
+        h.set_option("trace", 1)
+        h.run(w.M)
+        for d in (0, 1):
+            t = h.trace(d).astype(np.int64)
+            assert len(t) == int(h.info("grid_x" if d == 0 else "grid_y"))
+            assert np.all(t[:, 1] > t[:, 0]) and np.all(t[:, 2] < 160)      # end after start; SM ids
+            assert t[:, 3].sum() == int(h.info("chunks_x" if d == 0 else "chunks_y"))   # every piece ran exactly once
+        u = h.get()
+    finally:
+        h.close()
+    assert relerr(u, ref(w)) <= 1e-10
+
+
+def test_zero_steps_and_M_zero():
+    w = W.cfg2(N=64, M=4)
+    h = B.from_workload(w)
+    try:
+        h.run(0)
+        assert h.steps_done() == 0
+        assert np.array_equal(h.get(), w.phi)           # u^0 = phi, untouched
+    finally:
+        h.close()
+    h = B.Wave2D(16, 16, 1.0, 0.01, 0)                   # M = 0: nothing can be run, nothing breaks
+    try:
+        h.set_initial(np.ones((15, 15)))
+        h.run(0)
+        with pytest.raises(B.Wave2DError):
+            h.run(1)
+        assert np.array_equal(h.get(), np.ones((15, 15)))
+    finally:
+        h.close()
