@@ -29,6 +29,28 @@
 
 namespace w2d {
 
+// ---- two fp32 lines in one lane --------------------------------------------------------------------
+// The fp32 y sweep runs the kernel below with T = vec2f: a lane owns two adjacent grid columns (8 bytes), so
+// a panel is 64 columns and its rows are 256 contiguous bytes like in the fp64 y sweep.  All arithmetic is
+// element-wise; the scalar table entries are broadcast to both elements.
+struct __align__(8) vec2f {
+    float x, y;
+    vec2f() = default;
+    __device__ __forceinline__ vec2f(float a, float b) : x(a), y(b) {}
+    __device__ __forceinline__ vec2f(int a) : x(static_cast<float>(a)), y(static_cast<float>(a)) {}
+    __device__ __forceinline__ explicit vec2f(double a) : x(static_cast<float>(a)), y(static_cast<float>(a)) {}
+    __device__ __forceinline__ vec2f& operator+=(const vec2f& b) { x += b.x; y += b.y; return *this; }
+    __device__ __forceinline__ vec2f& operator*=(const vec2f& b) { x *= b.x; y *= b.y; return *this; }
+};
+__device__ __forceinline__ vec2f operator+(const vec2f& a, const vec2f& b) { return vec2f(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ vec2f operator*(const vec2f& a, const vec2f& b) { return vec2f(a.x * b.x, a.y * b.y); }
+__device__ __forceinline__ vec2f fmaT(const vec2f& a, const vec2f& b, const vec2f& c)
+{
+    return vec2f(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y));
+}
+__device__ __forceinline__ double fmaT(double a, double b, double c) { return ::fma(a, b, c); }
+__device__ __forceinline__ float fmaT(float a, float b, float c) { return ::fmaf(a, b, c); }
+
 // ---- per-half-step scalar table (fp64, built on the host; row n serves half-step n -> n+1) ------
 constexpr int KMAX = 128;    // boundary rows with their own (cp_p, inv_p)
 constexpr int NBK_MAX = 8;   // longest carry series (units)
@@ -246,8 +268,9 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 if (warp == 3 * NW / 4)
                     tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
             } else {
-                if (warp == 0) tma_load_2d(dst, &tm_prev, line0, g0 * U - 1, full);
-                if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0, g0 * U - 1, full);
+                constexpr int VEC = std::is_same<T, vec2f>::value ? 2 : 1;   // tensor-map columns per lane
+                if (warp == 0) tma_load_2d(dst, &tm_prev, line0 * VEC, g0 * U - 1, full);
+                if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0 * VEC, g0 * U - 1, full);
             }
         }
         q_slot = q_slot + 1 == NSTAGE ? 0 : q_slot + 1;
@@ -295,14 +318,14 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             for (int j = NBK_MAX; j > 4; --j)
                 if (j <= nbk) {
                     const int idx = (ring + dirn * j) & (RING - 1);
-                    c = fma(s_A[idx], c, vals_lane[idx * TL]);
+                    c = fmaT(s_A[idx], c, vals_lane[idx * TL]);
                 }
         }
 #pragma unroll
         for (int j = 4; j >= 1; --j)
             if (j <= nbk) {
                 const int idx = (ring + dirn * j) & (RING - 1);
-                c = fma(s_A[idx], c, vals_lane[idx * TL]);
+                c = fmaT(s_A[idx], c, vals_lane[idx * TL]);
             }
         return c;
     };
@@ -320,7 +343,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 #endif
         if (gp >= kb && full) {
 #pragma unroll
-            for (int e = 0; e < U; ++e) v[e] = fma(pw_at(U - 1 - e), Xin, v[e]);
+            for (int e = 0; e < U; ++e) v[e] = fmaT(pw_at(U - 1 - e), Xin, v[e]);
         } else {
             T c = Xin;
 #pragma unroll
@@ -425,17 +448,17 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                     for (int e = 0; e < U; ++e) {
                         const T left = e == 0 ? wl : wp[e - 1];
                         const T right = e == U - 1 ? wr : wp[e + 1];
-                        xl[e] = fma(g2i, wc[e], fma(ami, left + right, c1i * wp[e]));
+                        xl[e] = fmaT(g2i, wc[e], fmaT(ami, left + right, c1i * wp[e]));
                     }
                     if (src_tile && src_line && p0 < a.sp0 + a.snp && p0 + U > a.sp0) {
 #pragma unroll
                         for (int e = 0; e < U; ++e) {
                             const int ps = p0 + e - a.sp0;
-                            if (ps >= 0 && ps < a.snp) xl[e] = fma(qi, srcp[static_cast<size_t>(ps) * a.snl], xl[e]);
+                            if (ps >= 0 && ps < a.snp) xl[e] = fmaT(qi, srcp[static_cast<size_t>(ps) * a.snl], xl[e]);
                         }
                     }
 #pragma unroll
-                    for (int e = 1; e < U; ++e) xl[e] = fma(rho, xl[e - 1], xl[e]);
+                    for (int e = 1; e < U; ++e) xl[e] = fmaT(rho, xl[e - 1], xl[e]);
                     Aval = pw_at(U - 1);
                 } else {
                     const bool src_unit = src_tile && src_line;
@@ -445,11 +468,11 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                         const int p = p0 + e;
                         const T left = e == 0 ? wl : wp[e - 1];
                         const T right = e == U - 1 ? wr : wp[e + 1];
-                        T r = fma(g2, wc[e], fma(am, left + right, c1 * wp[e]));
+                        T r = fmaT(g2, wc[e], fmaT(am, left + right, c1 * wp[e]));
                         if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
-                            r = fma(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
+                            r = fmaT(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
                         const T cpe = cp_at(p);
-                        fy = fma(cpe, fy, r * inv_at(p));
+                        fy = fmaT(cpe, fy, r * inv_at(p));
                         if (p >= n) fy = T(0);
                         prod *= cpe;
                         xl[e] = fy;
@@ -469,9 +492,9 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 } else
 #endif
                 if (fast) {
-                    xl[U - 1] = fma(pw_at(U - 1), Yin, xl[U - 1]);
+                    xl[U - 1] = fmaT(pw_at(U - 1), Yin, xl[U - 1]);
 #pragma unroll
-                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(rho, xl[e + 1], fma(pw_at(e), Yin, xl[e]));
+                    for (int e = U - 2; e >= 0; --e) xl[e] = fmaT(rho, xl[e + 1], fmaT(pw_at(e), Yin, xl[e]));
                 } else {
                     T c = Yin;
 #pragma unroll
@@ -480,7 +503,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                         xl[e] = p0 + e < n ? xl[e] + c : T(0);
                     }
 #pragma unroll
-                    for (int e = U - 2; e >= 0; --e) xl[e] = fma(cp_at(p0 + e), xl[e + 1], xl[e]);
+                    for (int e = U - 2; e >= 0; --e) xl[e] = fmaT(cp_at(p0 + e), xl[e + 1], xl[e]);
                 }
                 s_H[ring * TL + lane] = xl[0];
                 named_bar_sync(1, NW * 32);

@@ -24,7 +24,8 @@ namespace {
 // Kernel variants: (NW consumer warps = units per stage, NSTAGE) per dtype and direction.
 // ------------------------------------------------------------------------------------------------
 struct Variant {
-    int dir, nw, nstage, unit, sub, smem, threads, elem;   // elem = sizeof(T), unit = points per thread
+    int dir, nw, nstage, unit, sub, smem, threads, elem;   // elem = bytes per grid value, unit = points per thread
+    int vec;                                               // grid lines per lane (2: fp32 y sweep on vec2f)
     const void* fn;
 };
 
@@ -32,7 +33,8 @@ template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB = 1>
 Variant make_variant()
 {
     using K = PanelCfg<T, DIR, UT, NW, NSTAGE>;
-    return Variant{DIR, NW, NSTAGE, UT, K::SUB, K::SMEM_BYTES, K::THREADS, (int)sizeof(T),
+    constexpr int VEC = std::is_same<T, vec2f>::value ? 2 : 1;
+    return Variant{DIR, NW, NSTAGE, UT, K::SUB, K::SMEM_BYTES, K::THREADS, (int)sizeof(T) / VEC, VEC,
                    reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB>)};
 }
 
@@ -54,8 +56,8 @@ void add_shapes_f32(std::vector<Variant>& v)
     v.push_back(make_variant<float, 0, 16, 8, 2, 2>());
     v.push_back(make_variant<float, 0, 32, 8, 2>());
     v.push_back(make_variant<float, 0, 8, 16, 2>());
+    v.push_back(make_variant<vec2f, 1, 8, 16, 2>());    // two columns per lane; not with a source (falls to shape 1)
     v.push_back(make_variant<float, 1, 8, 8, 3, 2>());
-    v.push_back(make_variant<float, 1, 8, 16, 3>());
     v.push_back(make_variant<float, 1, 16, 8, 3>());
     v.push_back(make_variant<float, 1, 8, 16, 4>());
 }
@@ -348,6 +350,7 @@ int plan_dir(wave2d_t* h, int d)
     P.nlines = d == 0 ? h->n2 : h->n1;
     P.shape = h->opt_shape[d];
     P.var = find_variant(h->elem, d, P.shape);
+    if (P.var && P.var->vec == 2 && (h->have_src || (h->pitch & 1))) P.var = find_variant(h->elem, d, P.shape + 1);
     if (!P.var) {
         h->err = "no kernel variant for this shape index";
         return WAVE2D_ERR_ARG;
@@ -393,7 +396,7 @@ int plan_dir(wave2d_t* h, int d)
         return WAVE2D_ERR_UNSUPPORTED;
     }
     P.ctas_per_sm = per_sm;
-    P.npanels = (P.nlines + 31) / 32;
+    P.npanels = ((P.nlines + V.vec - 1) / V.vec + 31) / 32;   // 32 lanes, V.vec lines each
     P.total_units = (P.n + U - 1) / U;
     // Persistent grid, one wave; the CTAs draw the pieces from an atomic ticket counter.
     const int slots = per_sm * h->num_sms;
@@ -436,7 +439,7 @@ int ensure_plan(wave2d_t* h)
         }
         if (h->plan[1].solver == WAVE2D_SOLVER_STREAM) {
             const Variant& V = *h->plan[1].var;
-            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32, V.unit * V.nw + 2, 0);
+            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32 * V.vec, V.unit * V.nw + 2, 0);
             if (st) return st;
         }
     }
@@ -486,10 +489,10 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     if (P.solver == WAVE2D_SOLVER_STREAM) {
         SweepArgs a;
         a.table = h->d_table; a.d_k = dk; a.n_off = n_off;
-        a.n = P.n; a.nlines = P.nlines; a.nbk = P.nbk; a.kb = P.kb;
+        a.n = P.n; a.nlines = (P.nlines + P.var->vec - 1) / P.var->vec; a.nbk = P.nbk; a.kb = P.kb;
         a.pieces = h->d_pieces[d]; a.npieces = (int)P.pieces.size(); a.tickets = h->d_tickets;
         a.cta_off = h->d_cta_off[d]; a.nstatic = P.nstatic;
-        a.out = out; a.pitch = h->pitch;
+        a.out = out; a.pitch = h->pitch / P.var->vec;   // in units of the kernel's T
         a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
         a.g2 = 2.0 * h->gamma;
         a.trace = h->opt_trace ? h->d_trace[d] : nullptr;
