@@ -45,6 +45,8 @@ def lib() -> C.CDLL:
             L.oracle_half_step.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                            C.c_double, _dp, _dp, _dp, _dp]
             L.oracle_half_step.restype = None
+            L.oracle_factored_step.argtypes = [C.c_int, C.c_int] + [C.c_double] * 5 + [_dp, _dp, _dp, _dp]
+            L.oracle_factored_step.restype = None
             L.oracle_wave2d_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_double,
                                                C.c_double, C.c_int]
             L.oracle_wave2d_destroy.argtypes = [C.c_void_p]
@@ -96,6 +98,17 @@ def half_step(direction: int, ap: float, am: float, gamma: float, q: float, w_pr
     n2, n1 = w_prev.shape
     out = np.empty_like(w_prev)
     lib().oracle_half_step(n1, n2, int(direction), ap, am, gamma, q, _p(w_prev), _p(w_cur), _p(s), _p(out))
+    return out
+
+
+def factored_step(axp, axm, ayp, aym, q, u_prev, u_cur, s=None) -> np.ndarray:
+    """One step k -> k+1 of the factorised unsplit scheme (2.8) (oracle_factored_step); arrays (n2, n1)."""
+    u_prev = _f64(u_prev)
+    u_cur = _f64(u_cur, u_prev.shape)
+    s = _f64(s, u_prev.shape) if s is not None else None
+    n2, n1 = u_prev.shape
+    out = np.empty_like(u_prev)
+    lib().oracle_factored_step(n1, n2, axp, axm, ayp, aym, q, _p(u_prev), _p(u_cur), _p(s), _p(out))
     return out
 
 
@@ -169,10 +182,13 @@ class Wave2DOracle:
 
 
 def solve(N1, N2, l, tau, M, phi, psi=None, c_half=None, s=None, g_half=None, steps=None,
-          gamma=None, kappa=None) -> np.ndarray:
-    """Convenience: run `steps` (default M) time steps and return u^steps."""
+          gamma=None, kappa=None, scheme=0) -> np.ndarray:
+    """Convenience: advance to time level `steps` (default M) and return u^steps.
+    scheme 1 (factorised (2.8)): set_initial already stands at level 1, so steps - 1 solves are run."""
     o = Wave2DOracle(N1, N2, l, tau, M)
     try:
+        if scheme:
+            o.set_option("scheme", scheme)
         if gamma is not None:
             o.set_option("gamma", gamma)
         if kappa is not None:
@@ -182,7 +198,7 @@ def solve(N1, N2, l, tau, M, phi, psi=None, c_half=None, s=None, g_half=None, st
         if s is not None:
             o.set_source(s, g_half)
         o.set_initial(phi, psi)
-        o.run(M if steps is None else steps)
+        o.run((M if steps is None else steps) - o.steps_done())
         return o.get()
     finally:
         o.close()

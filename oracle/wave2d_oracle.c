@@ -33,6 +33,9 @@
  *   a_p = c_p = -ap,  b_p = gamma + 2 ap,
  *   f_p = gamma (2 w_n[p] - w_{n-1}[p]) + am (w_{n-1}[p-1] - 2 w_{n-1}[p] + w_{n-1}[p+1]) + kappa tau^2 g_n s[p].
  *
+ * A second scheme (option "scheme" = 1, oracle_factored_step below) is the factorised form of the unsplit
+ * scheme (2.8); it has its own pins (tests/test_oracle_factored.py).
+ *
  * Parity pins (tests/test_oracle_*.py): dense LU of the Kronecker system on tiny grids, the exact
  * discrete modal recurrence, the PDE standing wave (observed order 1), forced response, tridiagonal
  * residuals, linearity / reflection invariants.  Nothing here is "parity unpinned".
@@ -115,6 +118,68 @@ void oracle_half_step(int n1, int n2, int dir, double ap, double am, double gamm
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * Scheme 1: the factorised form of the UNSPLIT three-level scheme (2.8).
+ * (2.8) times tau^2 reads, with a_d^+- = tau^2 c^{k+-1} / (2 h_d^2) and D_d the undivided second difference
+ * along d with zero Dirichlet ghosts (2.10),
+ *
+ *     (I - ax+ Dx - ay+ Dy) u^{k+1} = 2 u^k - (I - ax- Dx - ay- Dy) u^{k-1} + tau^2 f^k.
+ *
+ * Replacing both operators by their products (the alternating-direction factorisation; the added terms
+ * a^2 Dx Dy u are O(tau^4)) gives one x solve and one y solve per step:
+ *
+ *     z = (I - ay- Dy) u^{k-1}                                   explicit
+ *     R = 2 u^k - (I - ax- Dx) z + tau^2 g_k s                   explicit
+ *     (I - ax+ Dx) v = R                                         Thomas on every grid row
+ *     (I - ay+ Dy) u^{k+1} = v                                   Thomas on every grid column
+ *
+ * Every operator is applied / inverted literally here, point by point.  Arrays: n2 rows x n1 columns.
+ * ---------------------------------------------------------------------------------------------- */
+void oracle_factored_step(int n1, int n2, double axp, double axm, double ayp, double aym, double q,
+                          const double *u_prev, const double *u_cur, const double *s, double *u_next)
+{
+    const size_t npts = (size_t)n1 * (size_t)n2;
+    double *z = (double *)malloc(sizeof(double) * 2 * (npts ? npts : 1));
+    double *v = z + npts;
+#pragma omp parallel for schedule(static)
+    for (int j = 0; j < n2; ++j)
+        for (int i = 0; i < n1; ++i) {
+            const double up = j > 0 ? u_prev[(size_t)(j - 1) * n1 + i] : 0.0;
+            const double dn = j < n2 - 1 ? u_prev[(size_t)(j + 1) * n1 + i] : 0.0;
+            const double c0 = u_prev[(size_t)j * n1 + i];
+            z[(size_t)j * n1 + i] = c0 - aym * (up - 2.0 * c0 + dn);
+        }
+#pragma omp parallel
+    {
+        const int nmax = n1 > n2 ? n1 : n2;
+        double *a = (double *)malloc(sizeof(double) * 7 * (size_t)(nmax > 0 ? nmax : 1));
+        double *b = a + nmax, *c = b + nmax, *f = c + nmax, *x = f + nmax, *cp = x + nmax, *fp = cp + nmax;
+#pragma omp for schedule(static)
+        for (int j = 0; j < n2; ++j) {   /* x solve, one system per grid row */
+            const double *zr = z + (size_t)j * n1;
+            for (int i = 0; i < n1; ++i) {
+                const double zl = i > 0 ? zr[i - 1] : 0.0, zq = i < n1 - 1 ? zr[i + 1] : 0.0;
+                a[i] = -axp; b[i] = 1.0 + 2.0 * axp; c[i] = -axp;
+                f[i] = 2.0 * u_cur[(size_t)j * n1 + i] - (zr[i] - axm * (zl - 2.0 * zr[i] + zq));
+                if (s) f[i] += q * s[(size_t)j * n1 + i];
+            }
+            oracle_thomas(n1, a, b, c, f, x, cp, fp);
+            memcpy(v + (size_t)j * n1, x, sizeof(double) * (size_t)n1);
+        }
+#pragma omp for schedule(static)
+        for (int i = 0; i < n1; ++i) {   /* y solve, one system per grid column */
+            for (int j = 0; j < n2; ++j) {
+                a[j] = -ayp; b[j] = 1.0 + 2.0 * ayp; c[j] = -ayp;
+                f[j] = v[(size_t)j * n1 + i];
+            }
+            oracle_thomas(n2, a, b, c, f, x, cp, fp);
+            for (int j = 0; j < n2; ++j) u_next[(size_t)j * n1 + i] = x[j];
+        }
+        free(a);
+    }
+    free(z);
+}
+
+/* ------------------------------------------------------------------------------------------------
  * Handle API, mirroring the wave2d_* C ABI (include/wave2d.h) with host pointers and fp64 only.
  * ---------------------------------------------------------------------------------------------- */
 typedef struct oracle_wave2d_s {
@@ -125,7 +190,8 @@ typedef struct oracle_wave2d_s {
     double *s;        /* n2 x n1 source shape, or NULL (no source)                 */
     double *w[3];     /* w[0] = w_{n-1}, w[1] = w_n, w[2] = scratch for w_{n+1}     */
     int have_initial; /* set_initial called                                        */
-    int n_done;       /* half-steps taken so far                                   */
+    int n_done;       /* half-steps taken so far (scheme 1: 2 x the time level k)  */
+    int scheme;       /* 0: split scheme (2.11)-(2.12); 1: factorised (2.8)        */
 } oracle_wave2d_t;
 
 int oracle_wave2d_create(oracle_wave2d_t **out, int N1, int N2, double l, double tau, int M)
@@ -161,6 +227,11 @@ int oracle_wave2d_set_option(oracle_wave2d_t *h, const char *name, double value)
     if (h->n_done > 0) return ORACLE_ERR_STATE;
     if (!strcmp(name, "gamma")) { if (!(value > 0.0)) return ORACLE_ERR_ARG; h->gamma = value; return ORACLE_OK; }
     if (!strcmp(name, "kappa")) { h->kappa = value; return ORACLE_OK; }
+    if (!strcmp(name, "scheme")) {   /* before set_initial */
+        if ((value != 0.0 && value != 1.0) || h->have_initial) return ORACLE_ERR_ARG;
+        h->scheme = (int)value;
+        return ORACLE_OK;
+    }
     return ORACLE_ERR_ARG;
 }
 
@@ -169,15 +240,21 @@ int oracle_wave2d_set_option(oracle_wave2d_t *h, const char *name, double value)
 int oracle_wave2d_set_initial(oracle_wave2d_t *h, const double *phi, const double *psi, long ld)
 {
     if (!h || !phi || ld < h->n1) return ORACLE_ERR_ARG;
+    if (h->scheme == 1 && h->M < 1) return ORACLE_ERR_RANGE;
     for (int j = 0; j < h->n2; ++j)
         for (int i = 0; i < h->n1; ++i) {
             double p = phi[(long)j * ld + i];
             double q = psi ? psi[(long)j * ld + i] : 0.0;
-            h->w[1][(size_t)j * h->n1 + i] = p;
-            h->w[0][(size_t)j * h->n1 + i] = p - 0.5 * h->tau * q;
+            if (h->scheme == 0) {
+                h->w[1][(size_t)j * h->n1 + i] = p;
+                h->w[0][(size_t)j * h->n1 + i] = p - 0.5 * h->tau * q;
+            } else {   /* (2.9) as printed: u^0 = phi, u^1 = u^0 + tau psi; the state is level k = 1 */
+                h->w[0][(size_t)j * h->n1 + i] = p;
+                h->w[1][(size_t)j * h->n1 + i] = p + h->tau * q;
+            }
         }
     h->have_initial = 1;
-    h->n_done = 0;
+    h->n_done = h->scheme == 1 ? 2 : 0;
     return ORACLE_OK;
 }
 
@@ -217,6 +294,21 @@ int oracle_wave2d_run(oracle_wave2d_t *h, int steps)
     if (!h || steps < 0) return ORACLE_ERR_ARG;
     if (!h->have_initial) return ORACLE_ERR_STATE;
     if (h->n_done / 2 + steps > h->M) return ORACLE_ERR_RANGE;
+    if (h->scheme == 1) {   /* (2.8) factorised: level k -> k+1 needs c^{k-1}, c^{k+1}, g^k (integer levels) */
+        for (int it = 0; it < steps; ++it) {
+            const int k = h->n_done / 2;
+            const double t2 = h->tau * h->tau, h1 = h->l / h->N1, h2 = h->l / h->N2;
+            const double cp1 = h->c_half[2 * (k + 1)], cm1 = h->c_half[2 * (k - 1)];
+            const double g = h->g_half ? h->g_half[2 * k] : 1.0;
+            oracle_factored_step(h->n1, h->n2, t2 * cp1 / (2.0 * h1 * h1), t2 * cm1 / (2.0 * h1 * h1),
+                                 t2 * cp1 / (2.0 * h2 * h2), t2 * cm1 / (2.0 * h2 * h2), t2 * g,
+                                 h->w[0], h->w[1], h->s, h->w[2]);
+            double *old = h->w[0];
+            h->w[0] = h->w[1]; h->w[1] = h->w[2]; h->w[2] = old;
+            h->n_done += 2;
+        }
+        return ORACLE_OK;
+    }
     for (int it = 0; it < 2 * steps; ++it) {
         const int n = h->n_done;
         const int dir = n & 1;                                   /* x if n even, y if n odd */
@@ -243,7 +335,7 @@ static int copy_out(const oracle_wave2d_t *h, const double *src, double *dst, lo
     return ORACLE_OK;
 }
 
-/* u^k (k = steps done) and u^{k-1/2}. */
+/* u^k (k = steps done) and u^{k-1/2} (scheme 1: u^{k-1}). */
 int oracle_wave2d_get(const oracle_wave2d_t *h, double *u_out, long ld) { return h ? copy_out(h, h->w[1], u_out, ld) : ORACLE_ERR_ARG; }
 int oracle_wave2d_get_prev(const oracle_wave2d_t *h, double *u_out, long ld) { return h ? copy_out(h, h->w[0], u_out, ld) : ORACLE_ERR_ARG; }
 int oracle_wave2d_steps_done(const oracle_wave2d_t *h, int *k) { if (!h || !k) return ORACLE_ERR_ARG; *k = h->n_done / 2; return ORACLE_OK; }

@@ -32,3 +32,26 @@ def modal_amplitudes(N1, N2, l, tau, m, n, A, B, c_half, nhalf, S=0.0, g_half=No
         a_prev, a_cur = a_cur, rhs / lhs
         out.append(a_cur)
     return out
+
+
+def modal_amplitudes_factored(N1, N2, l, tau, m, n, A, B, c_half, K, S=0.0, g_half=None):
+    """Factorised form of the unsplit scheme (2.8), same mode ansatz:
+    -(undivided second difference) has the eigenvalue lam_d = 4 sin^2(m_d pi h_d / (2 l)) on the mode, so with
+    a_d(c) = tau^2 c / (2 h_d^2) every integer level k obeys
+
+        (1 + a_x(c_{k+1}) lam_x)(1 + a_y(c_{k+1}) lam_y) A_{k+1}
+            = 2 A_k - (1 + a_x(c_{k-1}) lam_x)(1 + a_y(c_{k-1}) lam_y) A_{k-1} + tau^2 g_k S,
+
+    A_0 = A, A_1 = A + tau B ((2.9)); c_k = c_half[2k], g_k = g_half[2k].  Returns [A_0 .. A_K]."""
+    h1, h2 = l / N1, l / N2
+    lam = (4.0 * math.sin(m * math.pi * h1 / (2 * l)) ** 2, 4.0 * math.sin(n * math.pi * h2 / (2 * l)) ** 2)
+    t2 = tau * tau
+
+    def op(c):
+        return (1.0 + t2 * c / (2 * h1 * h1) * lam[0]) * (1.0 + t2 * c / (2 * h2 * h2) * lam[1])
+
+    out = [A, A + tau * B]
+    for k in range(1, K):
+        g = 1.0 if g_half is None else g_half[2 * k]
+        out.append((2.0 * out[k] - op(c_half[2 * (k - 1)]) * out[k - 1] + t2 * g * S) / op(c_half[2 * (k + 1)]))
+    return out[:K + 1]
