@@ -636,6 +636,17 @@ __global__ void wave2d_init_prev(T* __restrict__ prev, const T* __restrict__ phi
     prev[o] = psi ? static_cast<T>(phi[o] - static_cast<T>(half_tau) * psi[o]) : phi[o];
 }
 
+// out = (I - ay Dy) in: in - ay (in[j-1] - 2 in[j] + in[j+1]) with zero ghosts (scheme 1 start, one-time)
+template <typename T>
+__global__ void wave2d_apply_y(T* __restrict__ out, const T* __restrict__ in, int n1, int n2, long long pitch, double ay)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= n1 || j >= n2) return;
+    const long long o = j * pitch + i;
+    const T up = j > 0 ? in[o - pitch] : T(0), dn = j < n2 - 1 ? in[o + pitch] : T(0), c0 = in[o];
+    out[o] = c0 - static_cast<T>(ay) * (up - T(2) * c0 + dn);
+}
+
 // dst[p][l] = src[l][p] for a small window (compact source, transposed copy for the x sweep)
 template <typename T>
 __global__ void wave2d_transpose_small(T* __restrict__ dst, const T* __restrict__ src, int rows, int cols)

@@ -122,7 +122,9 @@ struct wave2d_s {
     int num_sms = 0;
 
     long long pitch = 0;                 // elements
-    void* buf[3] = {nullptr, nullptr, nullptr};
+    int scheme = 0;                      // 0: split scheme (2.11)-(2.12); 1: factorised unsplit scheme (2.8)
+    bool v_ready = false;                // scheme 1: V^0, V^1 computed from U^0, U^1 (needs the final c samples)
+    void* buf[4] = {nullptr, nullptr, nullptr, nullptr};   // scheme 0 uses 3
     std::vector<double> c_half, g_half;  // g_half empty: g == 1
     bool have_src = false;
     void* src_dev[2] = {nullptr, nullptr};    // [0]: x sweep (transposed window), [1]: y sweep (natural window)
@@ -134,7 +136,7 @@ struct wave2d_s {
     double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
     bool plan_ok = false;
     DirPlan plan[2];
-    CUtensorMap tm_load[2][3], tm_store[3], tm_edge[3];   // [dir][buffer]; x: load tile, store tile, 16-byte edge box
+    CUtensorMap tm_load[2][4], tm_store[4], tm_edge[4];   // [dir][buffer]; x: load tile, store tile, 16-byte edge box
     Piece* d_pieces[2] = {nullptr, nullptr};
     int* d_tickets = nullptr;              // one work-queue counter per half-step
     int* d_cta_off[2] = {nullptr, nullptr};
@@ -217,6 +219,21 @@ void build_table(wave2d_t* h)
     const int nhalf = 2 * h->M;
     h->table.assign(static_cast<size_t>(std::max(nhalf, 1)) * ROW_DOUBLES, 0.0);
     const double t2 = h->tau * h->tau;
+    if (h->scheme == 1) {
+        // Factorised (2.8): step k -> k+1 (k = t + 1) is sweep 2t (x) and 2t+1 (y), both with
+        // gamma = 1:  x: (I - ax+ Dx) V^{k+1} = 2 U^k - (I - ax- Dx) V^{k-1} + tau^2 g_k s,  y: (I - ay+ Dy) U^{k+1} = V^{k+1}
+        // (V^j = (I - ay(c^j) Dy) U^j is carried); a_d^+- = tau^2 c^{k+-1} / (2 h_d^2).
+        for (int t = 0; t + 2 <= h->M; ++t) {
+            const int k = t + 1;
+            const double h1 = h->l / h->N1, h2 = h->l / h->N2;
+            const double cp1 = h->c_half[2 * (k + 1)], cm1 = h->c_half[2 * (k - 1)];
+            const double g = h->g_half.empty() ? 1.0 : h->g_half[2 * k];
+            fill_row(&h->table[static_cast<size_t>(2 * t) * ROW_DOUBLES], 1.0, t2 * cp1 / (2.0 * h1 * h1),
+                     t2 * cm1 / (2.0 * h1 * h1), h->have_src ? t2 * g : 0.0);
+            fill_row(&h->table[static_cast<size_t>(2 * t + 1) * ROW_DOUBLES], 1.0, t2 * cp1 / (2.0 * h2 * h2), 0.0, 0.0);
+        }
+        return;
+    }
     for (int n = 0; n < nhalf; ++n) {
         const double hd = h->l / ((n & 1) == 0 ? h->N1 : h->N2);                  // reading R3
         const double ap = t2 * h->c_half[n + 1] / (2.0 * hd * hd);
@@ -363,6 +380,7 @@ int plan_dir(wave2d_t* h, int d)
     int pconv = 0;   // rows [pconv, n) have stationary pivots (to tol) in every half-step
     for (int n = d; n < 2 * h->M; n += 2) {
         const double* row = &h->table[static_cast<size_t>(n) * ROW_DOUBLES];
+        if (row[ROW_BETA] == 0.0) continue;   // unused row (scheme 1 has M - 1 steps)
         rho = std::max(rho, row[ROW_RHO]);
         int pc = KMAX + 1;
         for (int p = KMAX - 1; p >= 0 && std::fabs(row[ROW_CP + p] - row[ROW_RHO]) <= tolp * row[ROW_RHO] &&
@@ -429,7 +447,7 @@ int ensure_plan(wave2d_t* h)
         st = plan_dir(h, d);
         if (st) return st;
     }
-    for (int b = 0; b < 3; ++b) {
+    for (int b = 0; b < (h->scheme == 1 ? 4 : 3); ++b) {
         if (h->plan[0].solver == WAVE2D_SOLVER_STREAM) {
             const int U = h->plan[0].var->unit;
             st = make_tmap_x3(h, &h->tm_load[0][b], h->buf[b], h->plan[0].var->nw / h->plan[0].var->sub);
@@ -473,15 +491,32 @@ int ensure_plan(wave2d_t* h)
     return WAVE2D_OK;
 }
 
+// Buffer roles of sweep n_abs (two sweeps per time step).
+//   scheme 0: ring of 3 (A6): reads w_{n-1} = B[n % 3], w_n = B[(n+1) % 3], writes w_{n+1} = B[(n+2) % 3].
+//   scheme 1: ring of 4, t = n_abs / 2 solves done: U^k = B[t % 4], V^{k-1} = B[(t+1) % 4], V^k = B[(t+2) % 4];
+//             x sweep: "prev" = V^{k-1}, "cur" = U^k, writes V^{k+1} into B[(t+3) % 4];
+//             y sweep: right-hand side V^{k+1} (as "prev" and "cur": 2 V - V), writes U^{k+1} over V^{k-1}.
+struct Roles {
+    int prev, cur, out;
+};
+Roles roles(const wave2d_t* h, int n_abs)
+{
+    if (h->scheme == 0) return Roles{n_abs % 3, (n_abs + 1) % 3, (n_abs + 2) % 3};
+    const int t = n_abs >> 1;
+    if ((n_abs & 1) == 0) return Roles{(t + 1) & 3, t & 3, (t + 3) & 3};
+    return Roles{(t + 3) & 3, (t + 3) & 3, (t + 1) & 3};
+}
+
 // One half-step n -> n+1.  With use_counter the kernels read the step count from d_k (graph replay) and
 // n_off is relative to it; otherwise n_off is the absolute half-step index.
 int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
 {
     const int d = n_abs & 1;
     const DirPlan& P = h->plan[d];
-    void* prev = h->buf[n_abs % 3];
-    void* cur = h->buf[(n_abs + 1) % 3];
-    void* out = h->buf[(n_abs + 2) % 3];
+    const Roles R = roles(h, n_abs);
+    void* prev = h->buf[R.prev];
+    void* cur = h->buf[R.cur];
+    void* out = h->buf[R.out];
     const int* dk = use_counter ? h->d_k : nullptr;
     const void* src = h->have_src ? h->src_dev[d] : nullptr;
     const int sl0 = d == 0 ? h->win_j0 : h->win_i0, snl = d == 0 ? h->win_h : h->win_w;
@@ -494,12 +529,12 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         a.cta_off = h->d_cta_off[d]; a.nstatic = P.nstatic;
         a.out = out; a.pitch = h->pitch / P.var->vec;   // in units of the kernel's T
         a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
-        a.g2 = 2.0 * h->gamma;
+        a.g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
         a.trace = h->opt_trace ? h->d_trace[d] : nullptr;
-        CUtensorMap* tp = &h->tm_load[d][n_abs % 3];
-        CUtensorMap* tc = &h->tm_load[d][(n_abs + 1) % 3];
-        CUtensorMap* to = &h->tm_store[(n_abs + 2) % 3];     // x sweep: TMA store box; unused by the y sweep
-        CUtensorMap* te = &h->tm_edge[n_abs % 3];            // x sweep: neighbours of a stage in w_{n-1}
+        CUtensorMap* tp = &h->tm_load[d][R.prev];
+        CUtensorMap* tc = &h->tm_load[d][R.cur];
+        CUtensorMap* to = &h->tm_store[R.out];               // x sweep: TMA store box; unused by the y sweep
+        CUtensorMap* te = &h->tm_edge[R.prev];               // x sweep: neighbours of a stage in "prev"
         if (h->plan[0].solver != WAVE2D_SOLVER_STREAM) { to = tp; te = tp; }   // y sweep alone: placeholders
         void* args[5] = {tp, tc, to, te, &a};
         cudaLaunchConfig_t cfg = {};
@@ -521,7 +556,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     double* ivv = h->d_piv + std::max(h->n1, h->n2);
     wave2d_exact_pivots<<<1, 256, 0, h->stream>>>(h->d_table, dk, n_off, P.n, cpv, ivv);
     const int tb = 128, gb = (P.nlines + tb - 1) / tb;
-    const double g2 = 2.0 * h->gamma;
+    const double g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
 #define W2D_EXACT(T, D)                                                                                               \
     do {                                                                                                              \
         wave2d_exact_forward<T, D><<<gb, tb, 0, h->stream>>>((const T*)prev, (const T*)cur, (T*)out, h->d_table, dk,  \
@@ -609,6 +644,57 @@ int copy_out(wave2d_t* h, void* dst, long ld, const void* src)
     return WAVE2D_OK;
 }
 
+// solves done so far: the device step counter and the table / ring index are counted in these
+int solves_done(const wave2d_t* h) { return h->scheme == 1 ? h->k - 1 : h->k; }
+int ring_period(const wave2d_t* h) { return h->scheme == 1 ? 4 : 3; }
+
+// Scheme 1 start, (2.9) as printed: U^0 = phi -> buf[3], U^1 = phi + tau psi -> buf[0]; the state
+// is time level k = 1.  V^0, V^1 follow at the first run (they need the final speed samples).
+int set_initial_factored(wave2d_t* h, const void* phi, const void* psi, long ld)
+{
+    if (h->M < 1) return WAVE2D_ERR_RANGE;
+    int st = copy_in(h, h->buf[3], phi, ld);
+    if (st == WAVE2D_OK && psi) st = copy_in(h, h->buf[2], psi, ld);
+    if (st) return st;
+    const dim3 blk(128), grd((h->n1 + 127) / 128, h->n2);
+    if (h->dtype == WAVE2D_F64)
+        wave2d_init_prev<double><<<grd, blk, 0, h->stream>>>((double*)h->buf[0], (const double*)h->buf[3],
+                                                             psi ? (const double*)h->buf[2] : nullptr, h->n1, h->n2,
+                                                             h->pitch, -h->tau);
+    else
+        wave2d_init_prev<float><<<grd, blk, 0, h->stream>>>((float*)h->buf[0], (const float*)h->buf[3],
+                                                            psi ? (const float*)h->buf[2] : nullptr, h->n1, h->n2,
+                                                            h->pitch, -h->tau);
+    W2D_CUDA(h, cudaGetLastError());
+    W2D_CUDA(h, cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream));
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)2 * h->M + 2) * sizeof(int), h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->have_initial = true;
+    h->v_ready = false;
+    h->k = 1;
+    h->ran = false;
+    return WAVE2D_OK;
+}
+
+// Scheme 1: V^0 = (I - ay(c^0) Dy) U^0 -> buf[1], V^1 = (I - ay(c^1) Dy) U^1 -> buf[2]   (roles of solve t = 0)
+int init_factored_v(wave2d_t* h)
+{
+    const double h2 = h->l / h->N2, t2 = h->tau * h->tau;
+    const double ay0 = t2 * h->c_half[0] / (2.0 * h2 * h2), ay1 = t2 * h->c_half[2] / (2.0 * h2 * h2);
+    const dim3 blk(128), grd((h->n1 + 127) / 128, h->n2);
+    if (h->dtype == WAVE2D_F64) {
+        wave2d_apply_y<double><<<grd, blk, 0, h->stream>>>((double*)h->buf[1], (const double*)h->buf[3], h->n1, h->n2, h->pitch, ay0);
+        wave2d_apply_y<double><<<grd, blk, 0, h->stream>>>((double*)h->buf[2], (const double*)h->buf[0], h->n1, h->n2, h->pitch, ay1);
+    } else {
+        wave2d_apply_y<float><<<grd, blk, 0, h->stream>>>((float*)h->buf[1], (const float*)h->buf[3], h->n1, h->n2, h->pitch, ay0);
+        wave2d_apply_y<float><<<grd, blk, 0, h->stream>>>((float*)h->buf[2], (const float*)h->buf[0], h->n1, h->n2, h->pitch, ay1);
+    }
+    W2D_CUDA(h, cudaGetLastError());
+    h->launches += 2;
+    h->v_ready = true;
+    return WAVE2D_OK;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -668,7 +754,7 @@ void wave2d_destroy(wave2d_t* h)
     if (!h) return;
     if (h->stream) cudaStreamSynchronize(h->stream);
     drop_graph(h);
-    for (int b = 0; b < 3; ++b) cudaFree(h->buf[b]);
+    for (int b = 0; b < 4; ++b) cudaFree(h->buf[b]);
     cudaFree(h->src_dev[0]);
     cudaFree(h->src_dev[1]);
     cudaFree(h->d_table);
@@ -701,6 +787,16 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     const int iv = (int)value;
     if (!strcmp(name, "gamma")) { if (!(value > 0.0)) return WAVE2D_ERR_ARG; h->gamma = value; }
     else if (!strcmp(name, "kappa")) h->kappa = value;
+    else if (!strcmp(name, "scheme")) {
+        if ((iv != 0 && iv != 1) || h->have_initial) return WAVE2D_ERR_ARG;
+        if (iv == 1 && !h->buf[3]) {
+            const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
+            int st = dev_alloc(h, &h->buf[3], fbytes);
+            if (st) return st;
+            cudaMemsetAsync(h->buf[3], 0, fbytes, h->stream);
+        }
+        h->scheme = iv;
+    }
     else if (!strcmp(name, "solver")) { if (iv < 0 || iv > 2) return WAVE2D_ERR_ARG; h->opt_solver = iv; }
     else if (!strcmp(name, "graph")) h->opt_graph = iv != 0;
     else if (!strcmp(name, "graph_steps")) { if (iv < 3 || iv % 3) return WAVE2D_ERR_ARG; h->opt_graph_steps = iv; }
@@ -721,6 +817,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
 int wave2d_set_initial(wave2d_t* h, const void* phi, const void* psi, long ld)
 {
     if (!h || !phi || ld < h->n1) return WAVE2D_ERR_ARG;
+    if (h->scheme == 1) return set_initial_factored(h, phi, psi, ld);
     // w_0 = phi -> buf[1]; psi staged in buf[2]; w_{-1} = phi - (tau/2) psi -> buf[0]   (roles of half-step 0)
     int st = copy_in(h, h->buf[1], phi, ld);
     if (st) return st;
@@ -815,19 +912,25 @@ int wave2d_run(wave2d_t* h, int steps)
     int st = ensure_plan(h);
     if (st) return st;
     if (steps > 0) h->ran = true;
+    if (steps > 0 && h->scheme == 1 && !h->v_ready) {
+        st = init_factored_v(h);
+        if (st) return st;
+    }
+    const int period = ring_period(h);
     const bool can_graph = h->opt_graph && h->stream != nullptr && h->stream != cudaStreamLegacy &&
                            h->stream != cudaStreamPerThread;
     int left = steps;
     bool counter_set = false;
     while (left > 0) {
         const int gs = h->opt_graph_steps;
-        if (can_graph && h->k % 3 == 0 && left >= gs) {
+        const int t = solves_done(h);
+        if (can_graph && t % period == 0 && gs % period == 0 && left >= gs) {
             if (!h->gexec || h->gexec_steps != gs) {
                 st = build_graph(h, gs);
                 if (st) return st;
             }
             if (!counter_set) {
-                W2D_CUDA(h, cudaMemcpyAsync(h->d_k, &h->k, sizeof(int), cudaMemcpyHostToDevice, h->stream));
+                W2D_CUDA(h, cudaMemcpyAsync(h->d_k, &t, sizeof(int), cudaMemcpyHostToDevice, h->stream));
                 counter_set = true;
             }
             W2D_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
@@ -835,8 +938,8 @@ int wave2d_run(wave2d_t* h, int steps)
             h->k += gs;
             left -= gs;
         } else {
-            st = launch_half_step(h, 2 * h->k, 2 * h->k, false);
-            if (st == WAVE2D_OK) st = launch_half_step(h, 2 * h->k + 1, 2 * h->k + 1, false);
+            st = launch_half_step(h, 2 * t, 2 * t, false);
+            if (st == WAVE2D_OK) st = launch_half_step(h, 2 * t + 1, 2 * t + 1, false);
             if (st) return st;
             h->k += 1;
             left -= 1;
@@ -849,12 +952,17 @@ int wave2d_run(wave2d_t* h, int steps)
 int wave2d_get(wave2d_t* h, void* u_out, long ld)
 {
     if (!h) return WAVE2D_ERR_ARG;
+    if (h->scheme == 1) return copy_out(h, u_out, ld, h->buf[(h->k - 1) & 3]);   // U^k
     return copy_out(h, u_out, ld, h->buf[(2 * h->k + 1) % 3]);
 }
 
 int wave2d_get_prev(wave2d_t* h, void* u_out, long ld)
 {
     if (!h) return WAVE2D_ERR_ARG;
+    if (h->scheme == 1) {   // the ring carries V^{k-1}, not U^{k-1}; only U^0 is still there before the first solve
+        if (h->k == 1 && !h->v_ready) return copy_out(h, u_out, ld, h->buf[3]);
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
     return copy_out(h, u_out, ld, h->buf[(2 * h->k) % 3]);
 }
 
@@ -915,10 +1023,11 @@ int wave2d_profile_sweeps(wave2d_t* h, int steps, double* ms_x, double* ms_y)
     for (auto& e : ev) W2D_CUDA(h, cudaEventCreate(&e));
     for (int s = 0; s < steps; ++s) {
         W2D_CUDA(h, cudaEventRecord(ev[3 * s], h->stream));
-        st = launch_half_step(h, 2 * h->k, 2 * h->k, false);
+        const int t = solves_done(h);
+        st = launch_half_step(h, 2 * t, 2 * t, false);
         if (st) return st;
         W2D_CUDA(h, cudaEventRecord(ev[3 * s + 1], h->stream));
-        st = launch_half_step(h, 2 * h->k + 1, 2 * h->k + 1, false);
+        st = launch_half_step(h, 2 * t + 1, 2 * t + 1, false);
         if (st) return st;
         W2D_CUDA(h, cudaEventRecord(ev[3 * s + 2], h->stream));
         h->k += 1;

@@ -325,3 +325,94 @@ def test_zero_steps_and_M_zero():
         assert np.array_equal(h.get(), np.ones((15, 15)))
     finally:
         h.close()
+
+
+# ---- scheme 1: the factorised form of the unsplit scheme (2.8) -------------
+def ref1(w, K=None):
+    npdt = np.float64 if w.dtype == "f64" else np.float32
+    cast = lambda a: None if a is None else a.astype(npdt).astype(np.float64)
+    return oracle.solve(w.N1, w.N2, w.l, w.tau, w.M, cast(w.phi), cast(w.psi), c_half=w.c_half, s=cast(w.s),
+                        g_half=w.g_half, steps=K, scheme=1)
+
+
+def gpu1(w, K=None, **opts):
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+    try:
+        h.set_option("scheme", 1)
+        for k, v in opts.items():
+            h.set_option(k, v)
+        npdt = np.float64 if w.dtype == "f64" else np.float32
+        h.set_speed(w.c_half)
+        if w.s is not None:
+            h.set_source(w.s.astype(npdt), w.g_half)
+        h.set_initial(w.phi.astype(npdt), None if w.psi is None else w.psi.astype(npdt))
+        assert h.steps_done() == 1                      # (2.9): set_initial stands at time level 1
+        h.run((w.M if K is None else K) - 1)
+        u = h.get()
+        info = {k: h.info(k) for k in ("solver_x", "solver_y", "launches")}
+    finally:
+        h.close()
+    return u, info
+
+
+def factored_cases():
+    rng = np.random.default_rng(77)
+    a = W.cfg2(N=300, M=30)
+    a.psi = 0.3 * a.phi
+    b = W.cfg3(N=260, M=40)
+    b.g_half = W.ricker(W.half_times(b.tau, 2 * b.M) + 0.058)
+    c = W.cfg4(N1=330, N2=140, M=25)
+    c.psi = rng.uniform(-1, 1, c.phi.shape)
+    d = W.cfg4(N1=330, N2=140, M=25, dtype="f32")
+    e = W.cfg5(N=200, M=26)
+    return [("cfg2_N300_psi", a), ("cfg3_N260_source", b), ("cfg4_330x140_psi", c), ("cfg4_330x140_f32", d),
+            ("cfg5_N200", e)]
+
+
+@pytest.mark.parametrize("name,w", factored_cases(), ids=[c[0] for c in factored_cases()])
+@pytest.mark.parametrize("opts", [{}, {"solver": B.SOLVER_EXACT}, {"graph": 0}, {"quota_x": 3, "quota_y": 3}],
+                         ids=["default", "exact", "nograph", "quota3"])
+def test_factored_scheme_matches_oracle(name, w, opts):
+    r = ref1(w)
+    u, info = gpu1(w, **opts)
+    assert np.isfinite(u).all()
+    assert relerr(u, r) <= TOL[w.dtype]
+    assert info["launches"] >= 2 * (w.M - 1)
+
+
+def test_factored_scheme_levels_one_by_one_and_modal():
+    """Every time level of a single mode against the scalar recurrence of tests/modal.py (c(t), psi != 0)."""
+    from tests.modal import modal_amplitudes_factored
+    N1, N2, M = 96, 80, 23
+    tau = 1.1 / 96
+    x, y = W.grid(N1, N2)
+    shape = np.outer(np.sin(2 * np.pi * y), np.sin(3 * np.pi * x))
+    c_half = 1.0 + 0.4 * np.sin(np.arange(2 * M + 1) * 0.3)
+    amps = modal_amplitudes_factored(N1, N2, 1.0, tau, 3, 2, 0.8, -0.5, c_half, M)
+    h = B.Wave2D(N1, N2, 1.0, tau, M, "f64")
+    try:
+        h.set_option("scheme", 1)
+        h.set_speed(c_half)
+        h.set_initial(0.8 * shape, -0.5 * shape)
+        assert np.abs(h.get_prev() - 0.8 * shape).max() == 0.0          # U^0 until the first solve
+        for K in range(1, M + 1):
+            assert h.steps_done() == K
+            assert np.abs(h.get() - amps[K] * shape).max() <= 1e-12
+            if K < M:
+                h.run(1)
+        with pytest.raises(B.Wave2DError):
+            h.run(1)                                                      # past M
+        with pytest.raises(B.Wave2DError):
+            h.get_prev()                                                  # the ring carries V^{k-1}, not U^{k-1}
+    finally:
+        h.close()
+
+
+def test_factored_scheme_full_grid_4095():
+    w = W.cfg3(N=4096, M=26)
+    w.g_half = W.ricker(W.half_times(w.tau, 2 * w.M) + 0.058)
+    w.phi = W.cfg2(N=4096, M=1).phi
+    r = ref1(w)
+    u, info = gpu1(w)
+    assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
+    assert relerr(u, r) <= 1e-10
