@@ -85,7 +85,8 @@ struct SweepArgs {
 };
 
 // UT = points per thread ("unit"), NW = consumer warps = units per stage, NSTAGE = TMA stages in flight.
-template <typename T, int DIR, int UT, int NW, int NSTAGE>
+// ONE: the right-hand side is the single input field itself (scheme 1's y sweep, (I - ay+ Dy) U = V): one field per stage.
+template <typename T, int DIR, int UT, int NW, int NSTAGE, bool ONE = false>
 struct PanelCfg {
     static constexpr int U = UT;                                      // points per unit
     static constexpr int TL = 32;                                     // lines per panel, one per lane
@@ -98,7 +99,9 @@ struct PanelCfg {
     // y sweep: per field one box [U*NW + 2 rows][32 columns]
     static constexpr int FIELD_BYTES = DIR == 0 ? NT * 4096 : (U * NW + 2) * TL * (int)sizeof(T);
     static constexpr int EDGE_BYTES = DIR == 0 ? 512 : 0;
-    static constexpr int STAGE_BYTES = 2 * FIELD_BYTES + 2 * EDGE_BYTES;
+    static constexpr int NFIELDS = ONE ? 1 : 2;
+    static constexpr int STAGE_BYTES = NFIELDS * FIELD_BYTES + 2 * EDGE_BYTES;
+    static_assert(!ONE || DIR == 1, "single-input variant exists for the y sweep only");
     static constexpr int OUT_BYTES = DIR == 0 ? NW * 2 * 32 * RB : 0;   // two store tiles per warp
     static constexpr int BAR_BYTES = ((NSTAGE * 8) + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * KMAX * (int)sizeof(T);
@@ -175,13 +178,13 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 //           warps whose look-ahead heads are all in this stage finish and store their unit now, the last
 //           few keep it one more stage ("deferred").
 // ---------------------------------------------------------------------------------------------------
-template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB>
+template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB, bool ONE = false>
 __global__ void __launch_bounds__(32 * NW, MINB)
 wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_constant__ CUtensorMap tm_cur,
                    const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_edge,
                    const SweepArgs a)
 {
-    using K = PanelCfg<T, DIR, UT, NW, NSTAGE>;
+    using K = PanelCfg<T, DIR, UT, NW, NSTAGE, ONE>;
     constexpr int U = UT, TL = K::TL, V = K::V, SUB = K::SUB, NT = K::NT, RING = 2 * NW;
 
     extern __shared__ unsigned char smem_raw[];
@@ -269,8 +272,12 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                     tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
             } else {
                 constexpr int VEC = std::is_same<T, vec2f>::value ? 2 : 1;   // tensor-map columns per lane
-                if (warp == 0) tma_load_2d(dst, &tm_prev, line0 * VEC, g0 * U - 1, full);
-                if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0 * VEC, g0 * U - 1, full);
+                if constexpr (ONE) {
+                    if (warp == 0) tma_load_2d(dst, &tm_cur, line0 * VEC, g0 * U - 1, full);
+                } else {
+                    if (warp == 0) tma_load_2d(dst, &tm_prev, line0 * VEC, g0 * U - 1, full);
+                    if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0 * VEC, g0 * U - 1, full);
+                }
             }
         }
         q_slot = q_slot + 1 == NSTAGE ? 0 : q_slot + 1;
@@ -422,6 +429,10 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                     if (sub < SUB - 1) wr = tile_elem_x<T>(tp, lane, (sub + 1) * U);
                     else if (tix < NT - 1) wr = tile_elem_x<T>(tp + 4096, lane, 0);
                     else wr = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V];
+                } else if constexpr (ONE) {
+                    const T* ccv = reinterpret_cast<const T*>(st) + (warp * U + 1) * TL + lane;
+#pragma unroll
+                    for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
                 } else {
                     const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
                     const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
@@ -446,9 +457,13 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
 #pragma unroll
                     for (int e = 0; e < U; ++e) {
-                        const T left = e == 0 ? wl : wp[e - 1];
-                        const T right = e == U - 1 ? wr : wp[e + 1];
-                        xl[e] = fmaT(g2i, wc[e], fmaT(ami, left + right, c1i * wp[e]));
+                        if constexpr (ONE) {
+                            xl[e] = inv * wc[e];
+                        } else {
+                            const T left = e == 0 ? wl : wp[e - 1];
+                            const T right = e == U - 1 ? wr : wp[e + 1];
+                            xl[e] = fmaT(g2i, wc[e], fmaT(ami, left + right, c1i * wp[e]));
+                        }
                     }
                     if (src_tile && src_line && p0 < a.sp0 + a.snp && p0 + U > a.sp0) {
 #pragma unroll
@@ -466,9 +481,14 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 #pragma unroll
                     for (int e = 0; e < U; ++e) {
                         const int p = p0 + e;
-                        const T left = e == 0 ? wl : wp[e - 1];
-                        const T right = e == U - 1 ? wr : wp[e + 1];
-                        T r = fmaT(g2, wc[e], fmaT(am, left + right, c1 * wp[e]));
+                        T r;
+                        if constexpr (ONE) {
+                            r = wc[e];
+                        } else {
+                            const T left = e == 0 ? wl : wp[e - 1];
+                            const T right = e == U - 1 ? wr : wp[e + 1];
+                            r = fmaT(g2, wc[e], fmaT(am, left + right, c1 * wp[e]));
+                        }
                         if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
                             r = fmaT(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
                         const T cpe = cp_at(p);

@@ -26,16 +26,17 @@ namespace {
 struct Variant {
     int dir, nw, nstage, unit, sub, smem, threads, elem;   // elem = bytes per grid value, unit = points per thread
     int vec;                                               // grid lines per lane (2: fp32 y sweep on vec2f)
+    int one;                                               // 1: single-input y sweep of scheme 1
     const void* fn;
 };
 
-template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB = 1>
+template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB = 1, bool ONE = false>
 Variant make_variant()
 {
-    using K = PanelCfg<T, DIR, UT, NW, NSTAGE>;
+    using K = PanelCfg<T, DIR, UT, NW, NSTAGE, ONE>;
     constexpr int VEC = std::is_same<T, vec2f>::value ? 2 : 1;
-    return Variant{DIR, NW, NSTAGE, UT, K::SUB, K::SMEM_BYTES, K::THREADS, (int)sizeof(T) / VEC, VEC,
-                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB>)};
+    return Variant{DIR, NW, NSTAGE, UT, K::SUB, K::SMEM_BYTES, K::THREADS, (int)sizeof(T) / VEC, VEC, ONE ? 1 : 0,
+                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB, ONE>)};
 }
 
 constexpr int NVAR = 4;   // shape variants per (dtype, dir); index 0 is the default
@@ -49,6 +50,13 @@ void add_shapes_f64(std::vector<Variant>& v)
     v.push_back(make_variant<double, 1, 8, 8, 3, 2>());
     v.push_back(make_variant<double, 1, 16, 8, 3>());
     v.push_back(make_variant<double, 1, 8, 16, 3>());
+}
+void add_shapes_one(std::vector<Variant>& v)   // scheme 1 y sweep; shape index 0..1
+{
+    v.push_back(make_variant<double, 1, 8, 16, 3, 1, true>());
+    v.push_back(make_variant<double, 1, 8, 16, 4, 1, true>());
+    v.push_back(make_variant<vec2f, 1, 8, 16, 3, 1, true>());
+    v.push_back(make_variant<float, 1, 8, 8, 4, 2, true>());
 }
 void add_shapes_f32(std::vector<Variant>& v)
 {
@@ -68,16 +76,17 @@ const std::vector<Variant>& variants()
         std::vector<Variant> w;
         add_shapes_f64(w);
         add_shapes_f32(w);
+        add_shapes_one(w);
         return w;
     }();
     return v;
 }
 
-const Variant* find_variant(int elem, int dir, int shape)
+const Variant* find_variant(int elem, int dir, int shape, int one = 0)
 {
     int seen = 0;
     for (const Variant& v : variants())
-        if (v.elem == elem && v.dir == dir) {
+        if (v.elem == elem && v.dir == dir && v.one == one) {
             if (seen == shape) return &v;
             ++seen;
         }
@@ -366,8 +375,10 @@ int plan_dir(wave2d_t* h, int d)
     P.n = d == 0 ? h->n1 : h->n2;
     P.nlines = d == 0 ? h->n2 : h->n1;
     P.shape = h->opt_shape[d];
-    P.var = find_variant(h->elem, d, P.shape);
-    if (P.var && P.var->vec == 2 && (h->have_src || (h->pitch & 1))) P.var = find_variant(h->elem, d, P.shape + 1);
+    const int one = h->scheme == 1 && d == 1;
+    if (one) P.shape = std::min(P.shape, 1);
+    P.var = find_variant(h->elem, d, P.shape, one);
+    if (P.var && P.var->vec == 2 && ((h->have_src && !one) || (h->pitch & 1))) P.var = find_variant(h->elem, d, P.shape + 1, one);
     if (!P.var) {
         h->err = "no kernel variant for this shape index";
         return WAVE2D_ERR_ARG;
