@@ -49,6 +49,9 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=960)
     ap.add_argument("--warmup", type=int, default=24)
     ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--scheme", type=int, default=0, choices=[0, 1],
+                    help="0: the paper's split scheme (2.11)-(2.12) (default, the north_star path); "
+                         "1: factorised unsplit scheme (2.8), 5 field passes per step (SURVEY.md 8f NEXT-2)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps per end-to-end iteration (default: --steps)")
@@ -287,7 +290,8 @@ def run_ours(args):
     from paper_2006_10142_b200 import binding as B
     K, Wm = args.steps, args.warmup
     PROF = 12                                             # per-kernel timing pass (plain launches + events)
-    w = load_workload(args.workload, Wm + K + PROF)
+    w = load_workload(args.workload, Wm + K + PROF + 2)
+    sch = args.scheme
     npdt = np.float64 if w.dtype == "f64" else np.float32
     esz = 8 if w.dtype == "f64" else 4
     fbytes = field_bytes(w)
@@ -300,6 +304,8 @@ def run_ours(args):
     stream = torch.cuda.Stream()
     h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
     h.set_stream(stream)
+    if sch:
+        h.set_option("scheme", sch)      # factorised (2.8): set_initial stands at level 1, every run step is a solve
     h.set_speed(w.c_half)
     if w.s is not None:
         h.set_source(w.s.astype(npdt, copy=False), w.g_half)
@@ -351,7 +357,10 @@ def run_ours(args):
     pts = w.points
     value = world * pts * K / (ms * 1e-3) / 1e9
     dom = "x" if ms_x >= ms_y else "y"
-    sweep_bytes = 3 * fbytes                                           # read 2 fields, write 1
+    # algorithmic bytes per launch: read 2 fields, write 1; scheme 1's y sweep reads 1, writes 1
+    bytes_x, bytes_y = 3 * fbytes, (2 if sch else 3) * fbytes
+    sweep_bytes = bytes_x if dom == "x" else bytes_y
+    passes = 5 if sch else 6
     step_s = ms * 1e-3 / K
     # The timed region is K steps = K launches of each sweep kernel back to back (graph replay), timed by the two
     # events above.  The dominant kernel's average launch duration in that region is its share of the step (from
@@ -364,6 +373,8 @@ def run_ours(args):
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
         "config": {"workload": w.name, "N1": w.N1, "N2": w.N2, "unknowns": [w.n1, w.n2], "tau": w.tau, "M": w.M,
+                   "scheme": ("split (2.11)-(2.12), 6 field passes per step" if not sch else
+                              "factorised unsplit (2.8), 5 field passes per step (SURVEY.md 8f NEXT-2)"),
                    "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
                    "l2": (f"working set {3 * fbytes / 1e6:.0f} MB (3 fields) "
                           + ("> 126 MB L2: inputs larger than L2, no flush needed" if 3 * fbytes > 126e6 * 1.5
@@ -383,16 +394,17 @@ def run_ours(args):
                      "how": "timed region (graph replay, events on the stream) x kernel share of the step",
                      "isolated": {"what": "plain launches, one event pair per kernel (includes a launch gap)",
                                   "ms_x": ms_x, "ms_y": ms_y,
-                                  "gbs_x": sweep_bytes / ms_x / 1e6, "gbs_y": sweep_bytes / ms_y / 1e6,
-                                  "frac_x": sweep_bytes / ms_x / 1e6 / peak, "frac_y": sweep_bytes / ms_y / 1e6 / peak},
-                     "frac_x": sweep_bytes / (step_s * 1e3 * ms_x / (ms_x + ms_y)) / 1e6 / peak,
-                     "frac_y": sweep_bytes / (step_s * 1e3 * ms_y / (ms_x + ms_y)) / 1e6 / peak,
+                                  "gbs_x": bytes_x / ms_x / 1e6, "gbs_y": bytes_y / ms_y / 1e6,
+                                  "frac_x": bytes_x / ms_x / 1e6 / peak, "frac_y": bytes_y / ms_y / 1e6 / peak},
+                     "frac_x": bytes_x / (step_s * 1e3 * ms_x / (ms_x + ms_y)) / 1e6 / peak,
+                     "frac_y": bytes_y / (step_s * 1e3 * ms_y / (ms_x + ms_y)) / 1e6 / peak,
+                     "step_passes": passes, "step_frac": passes * fbytes / step_s / 1e9 / peak,
                      "step_frac6": 6 * fbytes / step_s / 1e9 / peak, "step_frac5": 5 * fbytes / step_s / 1e9 / peak},
     }
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):   # dram bytes per launch from the committed ncu --set full capture
         try:
-            t = json.load(open(traffic_file)).get(f"{w.name}:{dom}")
+            t = json.load(open(traffic_file)).get(f"{w.name}:{dom}" + (":scheme1" if sch else ""))
             if t:
                 line["roofline"]["traffic"] = t
         except Exception:

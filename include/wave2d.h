@@ -86,9 +86,20 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "kappa"  source weight.              Default 0.5.   | locally-one-dimensional form of (2.11)-(2.12);
  *                                                       | gamma = kappa = 1 is the scheme as printed
  *                                                       |, which solves u_tt = 2c Lap u + 4f.
+ *   "scheme" 0 (default): the split scheme (2.11)-(2.12) driven by Algorithm 1.
+ *            1: the factorised form of the unsplit three-level scheme (2.8),
+ *                 (I - ax+ Dx)(I - ay+ Dy) u^{k+1} = 2 u^k - (I - ax- Dx)(I - ay- Dy) u^{k-1} + tau^2 f^k,
+ *               a_d^+- = tau^2 c^{k+-1} / (2 h_d^2): one x solve and one y solve per step, 5 field passes
+ *               instead of 6.  Uses c_half[2k], g_half[2k] only; gamma and kappa do not apply.  Start (2.9) as
+ *               printed: u^0 = phi, u^1 = phi + tau psi, so wave2d_set_initial leaves the handle at time level 1
+ *               (wave2d_steps_done = 1, wave2d_get = u^1; needs M >= 1) and wave2d_run(M - 1) reaches level M.
+ *               wave2d_get_prev is available only before the first solve (it returns u^0), then
+ *               ERR_UNSUPPORTED: the ring carries (I - ay Dy) u^{k-1}, not u^{k-1}.  Must be set before
+ *               wave2d_set_initial (ERR_ARG afterwards).  Uses a fourth field buffer.
  *   "solver" one of WAVE2D_SOLVER_*.     Default AUTO.
  *   "graph"  1 (default): the step loop is replayed as a CUDA Graph; 0: plain launches.
- *   "graph_steps"  time steps per graph replay (multiple of 3, the period of the buffer ring).  Default 12.
+ *   "graph_steps"  time steps per graph replay (multiple of 3; scheme 1 also needs a multiple of 4, the period
+ *            of its ring, else it falls back to plain launches).  Default 12.
  *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (units per stage = consumer warps / stages).
  *   "pdl"    1 (default): sweep kernels are launched with programmatic stream serialization, so that a kernel's
  *            prologue overlaps the tail of the previous one (it waits for it before touching the fields).
