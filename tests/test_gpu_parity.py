@@ -416,3 +416,38 @@ def test_factored_scheme_full_grid_4095():
     u, info = gpu1(w)
     assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
     assert relerr(u, r) <= 1e-10
+
+
+def test_factored_scheme_state_machine():
+    h = B.Wave2D(32, 32, 1.0, 0.01, 4)
+    try:
+        h.set_initial(np.zeros((31, 31)))
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_option("scheme", 1)                   # must precede set_initial
+        assert e.value.status == -1
+    finally:
+        h.close()
+    h = B.Wave2D(32, 32, 1.0, 0.01, 0)
+    try:
+        h.set_option("scheme", 1)
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_initial(np.zeros((31, 31)))           # (2.9) needs level 1 to exist: M >= 1
+        assert e.value.status == -6
+    finally:
+        h.close()
+    h = B.Wave2D(32, 32, 1.0, 0.01, 3)
+    try:
+        h.set_option("scheme", 1)
+        phi = np.ones((31, 31))
+        h.set_initial(phi, 2.0 * phi)
+        assert h.steps_done() == 1 and np.allclose(h.get(), 1.0 + 0.02)   # u^1 = phi + tau psi
+        h.run(0)
+        h.run(2)
+        assert h.steps_done() == 3
+        with pytest.raises(B.Wave2DError) as e:
+            h.run(1)
+        assert e.value.status == -6
+        h.set_initial(phi)                               # reset: back to level 1
+        assert h.steps_done() == 1 and np.array_equal(h.get(), phi)
+    finally:
+        h.close()
