@@ -318,8 +318,21 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     const T* const sH_lane = s_H + lane;
 
     // carry series: value entering unit `ring` from the left (dirn = -1, over L) or from the right (+1, over H)
-    auto carry = [&](const T* vals_lane, int ring, int dirn) -> T {
+    // `stat`: all nbk units of the series are whole units with stationary pivots, so every A is rho^U.
+    const T pwU = pw_at(U - 1);
+    auto carry = [&](const T* vals_lane, int ring, int dirn, bool stat) -> T {
         T c = T(0);
+        if (stat) {
+            if (nbk > 4) {
+#pragma unroll
+                for (int j = NBK_MAX; j > 4; --j)
+                    if (j <= nbk) c = fmaT(pwU, c, vals_lane[((ring + dirn * j) & (RING - 1)) * TL]);
+            }
+#pragma unroll
+            for (int j = 4; j >= 1; --j)
+                if (j <= nbk) c = fmaT(pwU, c, vals_lane[((ring + dirn * j) & (RING - 1)) * TL]);
+            return c;
+        }
         if (nbk > 4) {
 #pragma unroll
             for (int j = NBK_MAX; j > 4; --j)
@@ -339,7 +352,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 
     // finish unit gp (local x in v[]): add the carry from the right, store
     auto finish = [&](T (&v)[U], int gp, int ring, const Piece& pc) {
-        const T Xin = carry(sH_lane, ring, +1);   // x at the start of unit gp+1
+        const T Xin = carry(sH_lane, ring, +1, gp + 1 >= kb && (gp + nbk + 1) * U <= n);   // x at the start of unit gp+1
         if (gp < pc.ua || gp >= pc.ub) return;    // warp-uniform
         const int pp0 = gp * U;
         const bool full = pp0 + U <= n;
@@ -505,7 +518,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 produce();   // every warp holds its stage data in registers: refill the slot
 
                 // ---- carry from the left, local back substitution
-                const T Yin = carry(sL_lane, ring, -1);   // y at the end of unit g-1
+                const T Yin = carry(sL_lane, ring, -1, g - nbk >= kb && p0 <= n);   // y at the end of unit g-1
 #ifdef W2D_COPY_PROBE
                 if (true) {
                     xl[0] += Yin;

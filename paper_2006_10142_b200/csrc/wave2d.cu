@@ -529,7 +529,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     void* cur = h->buf[R.cur];
     void* out = h->buf[R.out];
     const int* dk = use_counter ? h->d_k : nullptr;
-    const void* src = h->have_src ? h->src_dev[d] : nullptr;
+    const void* src = h->have_src && !(h->scheme == 1 && d == 1) ? h->src_dev[d] : nullptr;   // scheme 1: f enters in x only
     const int sl0 = d == 0 ? h->win_j0 : h->win_i0, snl = d == 0 ? h->win_h : h->win_w;
     const int sp0 = d == 0 ? h->win_i0 : h->win_j0, snp = d == 0 ? h->win_w : h->win_h;
     if (P.solver == WAVE2D_SOLVER_STREAM) {

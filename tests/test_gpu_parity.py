@@ -365,8 +365,11 @@ def factored_cases():
     c.psi = rng.uniform(-1, 1, c.phi.shape)
     d = W.cfg4(N1=330, N2=140, M=25, dtype="f32")
     e = W.cfg5(N=200, M=26)
+    f = W.cfg3(N=261, M=40)                          # fp32 with a source: the x sweep adds it, the y sweep has none
+    f.dtype = "f32"
+    f.g_half = W.ricker(W.half_times(f.tau, 2 * f.M) + 0.058)
     return [("cfg2_N300_psi", a), ("cfg3_N260_source", b), ("cfg4_330x140_psi", c), ("cfg4_330x140_f32", d),
-            ("cfg5_N200", e)]
+            ("cfg5_N200", e), ("cfg3_N261_source_f32", f)]
 
 
 @pytest.mark.parametrize("name,w", factored_cases(), ids=[c[0] for c in factored_cases()])
