@@ -97,7 +97,8 @@ struct PanelCfg {
     static constexpr int RB = UT * (int)sizeof(T);                    // x sweep: bytes per row of a warp's store tile
     // x sweep: per field NT tiles [32 rows][128 B] (128B-swizzled) + two edge boxes [32 rows][16 B] of wp
     // y sweep: per field one box [U*NW + 2 rows][32 columns]
-    static constexpr int FIELD_BYTES = DIR == 0 ? NT * 4096 : (U * NW + 2) * TL * (int)sizeof(T);
+    static constexpr int HALO = ONE ? 0 : 1;                          // y sweep: stencil rows above / below a stage
+    static constexpr int FIELD_BYTES = DIR == 0 ? NT * 4096 : (U * NW + 2 * HALO) * TL * (int)sizeof(T);
     static constexpr int EDGE_BYTES = DIR == 0 ? 512 : 0;
     static constexpr int NFIELDS = ONE ? 1 : 2;
     static constexpr int STAGE_BYTES = NFIELDS * FIELD_BYTES + 2 * EDGE_BYTES;
@@ -111,7 +112,7 @@ struct PanelCfg {
     static_assert((NW & (NW - 1)) == 0, "NW must be a power of two (ring indexing)");
     static_assert(DIR == 1 || (TU % UT == 0 && NW % SUB == 0 && RB >= 32), "x sweep: units must tile the 128-byte row");
     static_assert(FIELD_BYTES % 128 == 0 && (32 * RB) % 1024 == 0 || DIR == 1, "TMA smem alignment");
-    static_assert(DIR == 0 || U * NW + 2 <= 256, "TMA box dimension limit");
+    static_assert(DIR == 0 || U * NW + 2 * HALO <= 256, "TMA box dimension limit");
 };
 
 // ---- x sweep shared-memory tiles ---------------------------------------------------------------------
@@ -273,7 +274,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             } else {
                 constexpr int VEC = std::is_same<T, vec2f>::value ? 2 : 1;   // tensor-map columns per lane
                 if constexpr (ONE) {
-                    if (warp == 0) tma_load_2d(dst, &tm_cur, line0 * VEC, g0 * U - 1, full);
+                    if (warp == 0) tma_load_2d(dst, &tm_cur, line0 * VEC, g0 * U, full);
                 } else {
                     if (warp == 0) tma_load_2d(dst, &tm_prev, line0 * VEC, g0 * U - 1, full);
                     if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0 * VEC, g0 * U - 1, full);
@@ -443,7 +444,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                     else if (tix < NT - 1) wr = tile_elem_x<T>(tp + 4096, lane, 0);
                     else wr = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V];
                 } else if constexpr (ONE) {
-                    const T* ccv = reinterpret_cast<const T*>(st) + (warp * U + 1) * TL + lane;
+                    const T* ccv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
 #pragma unroll
                     for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
                 } else {

@@ -54,7 +54,7 @@ void add_shapes_f64(std::vector<Variant>& v)
 void add_shapes_one(std::vector<Variant>& v)   // scheme 1 y sweep; shape index 0..1
 {
     v.push_back(make_variant<double, 1, 8, 16, 3, 1, true>());
-    v.push_back(make_variant<double, 1, 8, 16, 4, 1, true>());
+    v.push_back(make_variant<double, 1, 16, 16, 3, 1, true>());
     v.push_back(make_variant<vec2f, 1, 8, 16, 3, 1, true>());
     v.push_back(make_variant<float, 1, 8, 8, 4, 2, true>());
 }
@@ -468,7 +468,7 @@ int ensure_plan(wave2d_t* h)
         }
         if (h->plan[1].solver == WAVE2D_SOLVER_STREAM) {
             const Variant& V = *h->plan[1].var;
-            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32 * V.vec, V.unit * V.nw + 2, 0);
+            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32 * V.vec, V.unit * V.nw + (V.one ? 0 : 2), 0);
             if (st) return st;
         }
     }
