@@ -118,6 +118,14 @@ int wave2d_set_option(wave2d_t *h, const char *name, double value);
 int wave2d_set_initial(wave2d_t *h, const void *phi, const void *psi, long ld);
 
 /*
+ * Checkpoint / resume (scheme 0): the state of Algorithm 1 is the pair (u, U0) = (u^{k-1/2}, u^k),
+ * which wave2d_get_prev / wave2d_get return.  wave2d_set_state puts a handle at time level k with that pair, so
+ * that a run continued from a checkpoint is bit-identical to the uninterrupted one (same speed / source samples).
+ * Errors: ERR_ARG (k outside 0..M), ERR_UNSUPPORTED (scheme 1).  Synchronous for host pointers.
+ */
+int wave2d_set_state(wave2d_t *h, int k, const void *u_prev_half, const void *u, long ld);
+
+/*
  * Speed samples c_half[n] = c(n tau/2), n = 0..2M (count == 2M+1), or one constant (count == 1).
  * Every value must be > 0 ("positive speed function"), else ERR_ARG.  c_{-1} := c_0.
  */

@@ -19,6 +19,7 @@ SOLVER_AUTO, SOLVER_EXACT, SOLVER_STREAM = 0, 1, 2
 
 EXPORTS = [
     "wave2d_create", "wave2d_destroy", "wave2d_set_stream", "wave2d_set_option", "wave2d_set_initial",
+    "wave2d_set_state",
     "wave2d_set_speed", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
     "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
     "wave2d_host_scalars", "wave2d_host_plan", "wave2d_strerror", "wave2d_last_error",
@@ -52,6 +53,7 @@ def load_library() -> C.CDLL:
     L.wave2d_set_stream.argtypes = [vp, vp]
     L.wave2d_set_option.argtypes = [vp, C.c_char_p, C.c_double]
     L.wave2d_set_initial.argtypes = [vp, vp, vp, C.c_long]
+    L.wave2d_set_state.argtypes = [vp, C.c_int, vp, vp, C.c_long]
     L.wave2d_set_speed.argtypes = [vp, dp, C.c_int]
     L.wave2d_set_source.argtypes = [vp, vp, C.c_long, dp, C.c_int]
     L.wave2d_run.argtypes = [vp, C.c_int]
@@ -156,6 +158,14 @@ class Wave2D:
         if psi is not None and ld2 != ld:
             raise ValueError("phi and psi must share one row stride")
         self._check(self._L.wave2d_set_initial(self._h, p, q, ld), "wave2d_set_initial")
+
+    def set_state(self, k: int, u_prev_half, u):
+        keep = []
+        p, ld = self._field(u_prev_half, keep)
+        q, ld2 = self._field(u, keep)
+        if ld2 != ld:
+            raise ValueError("both fields must share one row stride")
+        self._check(self._L.wave2d_set_state(self._h, int(k), p, q, ld), "wave2d_set_state")
 
     def set_speed(self, c_half):
         c = np.ascontiguousarray(np.atleast_1d(c_half), dtype=np.float64)

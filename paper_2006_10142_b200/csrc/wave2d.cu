@@ -855,6 +855,21 @@ int wave2d_set_initial(wave2d_t* h, const void* phi, const void* psi, long ld)
     return WAVE2D_OK;
 }
 
+int wave2d_set_state(wave2d_t* h, int k, const void* u_prev_half, const void* u, long ld)
+{
+    if (!h || !u_prev_half || !u || ld < h->n1 || k < 0 || k > h->M) return WAVE2D_ERR_ARG;
+    if (h->scheme != 0) return WAVE2D_ERR_UNSUPPORTED;   // scheme 1's ring carries (I - ay Dy) u^{k-1}, not a level
+    // roles of half-step n = 2k: w_{n-1} = u^{k-1/2} -> buf[n % 3], w_n = u^k -> buf[(n+1) % 3]
+    int st = copy_in(h, h->buf[(2 * k) % 3], u_prev_half, ld);
+    if (st == WAVE2D_OK) st = copy_in(h, h->buf[(2 * k + 1) % 3], u, ld);
+    if (st) return st;
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)2 * h->M + 2) * sizeof(int), h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    h->have_initial = true;
+    h->k = k;
+    return WAVE2D_OK;
+}
+
 int wave2d_set_speed(wave2d_t* h, const double* c_half, int count)
 {
     if (!h || !c_half || (count != 1 && count != 2 * h->M + 1)) return WAVE2D_ERR_ARG;

@@ -454,3 +454,40 @@ def test_factored_scheme_state_machine():
         assert h.steps_done() == 1 and np.array_equal(h.get(), phi)
     finally:
         h.close()
+
+
+def test_checkpoint_resume_is_bit_identical():
+    """State of Algorithm 1 = (u^{k-1/2}, u^k): get_prev/get at k = 17, a fresh handle put there
+    with wave2d_set_state, and the continuation equals the uninterrupted run bit for bit."""
+    w = W.cfg3(N=300, M=40)
+    w.g_half = W.ricker(W.half_times(w.tau, 2 * w.M) + 0.058)
+    w.phi = W.cfg2(N=300, M=1).phi
+    h = B.from_workload(w)
+    try:
+        h.run(17)
+        prev, cur = h.get_prev(), h.get()
+        h.run(w.M - 17)
+        full = h.get()
+    finally:
+        h.close()
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+    try:
+        h.set_speed(w.c_half)
+        h.set_source(w.s, w.g_half)
+        h.set_state(17, prev, cur)
+        assert h.steps_done() == 17
+        h.run(w.M - 17)
+        assert np.array_equal(h.get(), full)
+        with pytest.raises(B.Wave2DError):
+            h.set_state(w.M + 1, prev, cur)
+    finally:
+        h.close()
+    assert relerr(full, ref(w)) <= 1e-10
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+    try:
+        h.set_option("scheme", 1)
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_state(3, prev, cur)
+        assert e.value.status == -5
+    finally:
+        h.close()
