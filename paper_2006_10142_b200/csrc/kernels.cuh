@@ -64,7 +64,8 @@ struct Piece {
 };
 
 struct SweepArgs {
-    const double* table;   // device, ROW_DOUBLES per half-step
+    const double* table;   // device, ROW_DOUBLES per half-step (or per period, see table_period)
+    int table_period;      // 0: one row per half-step; p > 0: the rows repeat with period p (constant c and g)
     const int* d_k;        // device: completed time steps at graph start (NULL: 0)
     int n_off;             // half-step index = n_off + 2 * (*d_k)
     int n;                 // unknowns per line
@@ -203,7 +204,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nh = a.n_off + (a.d_k ? 2 * (*a.d_k) : 0);
-    const double* row = a.table + static_cast<size_t>(nh) * ROW_DOUBLES;
+    const double* row = a.table + static_cast<size_t>(a.table_period ? nh % a.table_period : nh) * ROW_DOUBLES;
 
     for (int i = threadIdx.x; i < KMAX; i += K::THREADS) {
         s_cp[i] = static_cast<T>(row[ROW_CP + i]);
@@ -585,11 +586,12 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 // on request (WAVE2D_SOLVER_EXACT).  DIR 1 is coalesced; DIR 0 walks rows and is slow but correct.
 // ---------------------------------------------------------------------------------------------------
 // cpv[p], ivv[p], p < n: one thread block; thread 0 runs the pivot recurrence until it is stationary.
-__global__ void wave2d_exact_pivots(const double* table, const int* d_k, int n_off, int n, double* cpv, double* ivv)
+__global__ void wave2d_exact_pivots(const double* table, int period, const int* d_k, int n_off, int n, double* cpv,
+                                    double* ivv)
 {
     __shared__ int s_conv;
     const int nh = n_off + (d_k ? 2 * (*d_k) : 0);
-    const double* row = table + static_cast<size_t>(nh) * ROW_DOUBLES;
+    const double* row = table + static_cast<size_t>(period ? nh % period : nh) * ROW_DOUBLES;
     const double ap = row[ROW_AP], beta = row[ROW_BETA];
     if (threadIdx.x == 0) {
         double cp = 0.0;
@@ -617,14 +619,14 @@ __global__ void wave2d_exact_pivots(const double* table, const int* d_k, int n_o
 
 template <typename T, int DIR>
 __global__ void wave2d_exact_forward(const T* __restrict__ wprev, const T* __restrict__ wcur, T* __restrict__ out,
-                                     const double* table, const int* d_k, int n_off, int n, int nlines,
+                                     const double* table, int period, const int* d_k, int n_off, int n, int nlines,
                                      long long pitch, const double* __restrict__ cpv, const double* __restrict__ ivv,
                                      const T* __restrict__ src, int sl0, int snl, int sp0, int snp, double g2d)
 {
     const int line = blockIdx.x * blockDim.x + threadIdx.x;
     if (line >= nlines) return;
     const int nh = n_off + (d_k ? 2 * (*d_k) : 0);
-    const double* row = table + static_cast<size_t>(nh) * ROW_DOUBLES;
+    const double* row = table + static_cast<size_t>(period ? nh % period : nh) * ROW_DOUBLES;
     const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), c1 = static_cast<T>(row[ROW_C1]);
     const T g2 = static_cast<T>(g2d);
     const long long ls = DIR == 0 ? pitch : 1, ps = DIR == 0 ? 1 : pitch;   // strides between lines / along the line

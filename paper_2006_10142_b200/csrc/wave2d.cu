@@ -140,6 +140,7 @@ struct wave2d_s {
     int win_i0 = 0, win_j0 = 0, win_w = 0, win_h = 0;
 
     std::vector<double> table;           // host copy
+    int table_period = 0;                // 0: one row per half-step; 2: constant c and g, two rows serve every step
     double* d_table = nullptr;
     int* d_k = nullptr;
     double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
@@ -225,14 +226,21 @@ void fill_row(double* row, double gamma, double ap, double am, double qv)
 
 void build_table(wave2d_t* h)
 {
-    const int nhalf = 2 * h->M;
+    // Constant c and g (the paper's own runs): all x rows are equal and all y rows are equal, so two rows
+    // serve every step and M is not bounded by the size of the table.
+    bool constant = h->M >= 2;
+    for (size_t i = 1; i < h->c_half.size() && constant; ++i) constant = h->c_half[i] == h->c_half[0];
+    if (h->have_src)
+        for (size_t i = 1; i < h->g_half.size() && constant; ++i) constant = h->g_half[i] == h->g_half[0];
+    h->table_period = constant ? 2 : 0;
+    const int nhalf = constant ? 2 : 2 * h->M;
     h->table.assign(static_cast<size_t>(std::max(nhalf, 1)) * ROW_DOUBLES, 0.0);
     const double t2 = h->tau * h->tau;
     if (h->scheme == 1) {
         // Factorised (2.8): step k -> k+1 (k = t + 1) is sweep 2t (x) and 2t+1 (y), both with
         // gamma = 1:  x: (I - ax+ Dx) V^{k+1} = 2 U^k - (I - ax- Dx) V^{k-1} + tau^2 g_k s,  y: (I - ay+ Dy) U^{k+1} = V^{k+1}
         // (V^j = (I - ay(c^j) Dy) U^j is carried); a_d^+- = tau^2 c^{k+-1} / (2 h_d^2).
-        for (int t = 0; t + 2 <= h->M; ++t) {
+        for (int t = 0; t + 2 <= (constant ? 2 : h->M); ++t) {
             const int k = t + 1;
             const double h1 = h->l / h->N1, h2 = h->l / h->N2;
             const double cp1 = h->c_half[2 * (k + 1)], cm1 = h->c_half[2 * (k - 1)];
@@ -389,7 +397,7 @@ int plan_dir(wave2d_t* h, int d)
     const double tolp = h->dtype == WAVE2D_F64 ? 2e-15 : 1e-8;  // pivots count as stationary within a few ulp
     double rho = 0.0;
     int pconv = 0;   // rows [pconv, n) have stationary pivots (to tol) in every half-step
-    for (int n = d; n < 2 * h->M; n += 2) {
+    for (int n = d; n < (h->table_period ? h->table_period : 2 * h->M); n += 2) {
         const double* row = &h->table[static_cast<size_t>(n) * ROW_DOUBLES];
         if (row[ROW_BETA] == 0.0) continue;   // unused row (scheme 1 has M - 1 steps)
         rho = std::max(rho, row[ROW_RHO]);
@@ -534,7 +542,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     const int sp0 = d == 0 ? h->win_i0 : h->win_j0, snp = d == 0 ? h->win_w : h->win_h;
     if (P.solver == WAVE2D_SOLVER_STREAM) {
         SweepArgs a;
-        a.table = h->d_table; a.d_k = dk; a.n_off = n_off;
+        a.table = h->d_table; a.table_period = h->table_period; a.d_k = dk; a.n_off = n_off;
         a.n = P.n; a.nlines = (P.nlines + P.var->vec - 1) / P.var->vec; a.nbk = P.nbk; a.kb = P.kb;
         a.pieces = h->d_pieces[d]; a.npieces = (int)P.pieces.size(); a.tickets = h->d_tickets;
         a.cta_off = h->d_cta_off[d]; a.nstatic = P.nstatic;
@@ -565,13 +573,13 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     // exact two-pass Thomas
     double* cpv = h->d_piv;
     double* ivv = h->d_piv + std::max(h->n1, h->n2);
-    wave2d_exact_pivots<<<1, 256, 0, h->stream>>>(h->d_table, dk, n_off, P.n, cpv, ivv);
+    wave2d_exact_pivots<<<1, 256, 0, h->stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv);
     const int tb = 128, gb = (P.nlines + tb - 1) / tb;
     const double g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
 #define W2D_EXACT(T, D)                                                                                               \
     do {                                                                                                              \
-        wave2d_exact_forward<T, D><<<gb, tb, 0, h->stream>>>((const T*)prev, (const T*)cur, (T*)out, h->d_table, dk,  \
-                                                             n_off, P.n, P.nlines, h->pitch, cpv, ivv, (const T*)src, \
+        wave2d_exact_forward<T, D><<<gb, tb, 0, h->stream>>>((const T*)prev, (const T*)cur, (T*)out, h->d_table,      \
+                                                             h->table_period, dk, n_off, P.n, P.nlines, h->pitch, cpv, ivv, (const T*)src, \
                                                              sl0, snl, sp0, snp, g2);                                 \
         wave2d_exact_backward<T, D><<<gb, tb, 0, h->stream>>>((T*)out, P.n, P.nlines, h->pitch, cpv);                 \
     } while (0)

@@ -491,3 +491,33 @@ def test_checkpoint_resume_is_bit_identical():
         assert e.value.status == -5
     finally:
         h.close()
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_constant_speed_needs_no_per_step_table(scheme):
+    """c = const, g = const (the paper's own runs): two table rows serve every step, so M = 600 000
+    (a 1.3 GB table otherwise: ERR_UNSUPPORTED) runs; the first 26 levels are compared with the oracle."""
+    N, M, K = 200, 600_000, 26
+    w = W.cfg2(N=N, M=K)
+    tau = w.tau
+    s = W.cfg3(N=N, M=K).s
+    def run_gpu(c_half):
+        h = B.Wave2D(N, N, 1.0, tau, M, "f64")
+        try:
+            if scheme:
+                h.set_option("scheme", 1)
+            h.set_speed(c_half)
+            h.set_source(s, None)                       # g == 1: the time-independent "full grid" source (R11)
+            h.set_initial(w.phi)
+            h.run(K - h.steps_done())
+            return h.get()
+        finally:
+            h.close()
+    u = run_gpu(np.array([1.3]))
+    r = oracle.solve(N, N, 1.0, tau, K, w.phi, None, c_half=np.full(2 * K + 1, 1.3), s=s, g_half=None, scheme=scheme)
+    assert relerr(u, r) <= 1e-10
+    varying = np.full(2 * M + 1, 1.3)
+    varying[7] = 1.31                                   # not constant: needs 2M rows of 2 KB -> refused, not truncated
+    with pytest.raises(B.Wave2DError) as e:
+        run_gpu(varying)
+    assert e.value.status == -5
