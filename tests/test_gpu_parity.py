@@ -521,3 +521,30 @@ def test_constant_speed_needs_no_per_step_table(scheme):
     with pytest.raises(B.Wave2DError) as e:
         run_gpu(varying)
     assert e.value.status == -5
+
+
+@pytest.mark.parametrize("N1,N2", [(2, 2), (2, 9), (9, 2), (3, 3), (4, 5), (17, 16), (18, 33), (33, 18), (34, 34),
+                                   (65, 66), (66, 65), (127, 129), (129, 127), (130, 66), (257, 40), (40, 257)])
+@pytest.mark.parametrize("dtype,scheme", [("f32", 0), ("f64", 1), ("f32", 1)])
+def test_tiny_and_ragged_sizes_fp32_and_scheme1(N1, N2, dtype, scheme):
+    """Sizes straddling one unit / one 32-line (fp32 y sweep: 64-column) panel, odd and even n1 (the vec2f y sweep
+    pairs columns; an odd n1 leaves a zero pad column in the last pair), for fp32 and for scheme 1."""
+    rng = np.random.default_rng(7000 * N1 + 13 * N2 + scheme)
+    M = 7
+    tau = 0.9 / max(N1, N2)
+    shape = (N2 - 1, N1 - 1)
+    phi, psi, s = (rng.uniform(-1, 1, shape) for _ in range(3))
+    c = rng.uniform(0.5, 1.5, 2 * M + 1)
+    g = rng.uniform(-1, 1, 2 * M)
+    w = W.Workload("rand", N1, N2, 1.0, tau, M, dtype, phi, psi, c, s=s, g_half=g)
+    tol = 1e-12 if dtype == "f64" else 2e-5
+    for opts in ({}, {"solver": B.SOLVER_EXACT}):
+        if scheme:
+            u, _ = gpu1(w, **opts)
+            r = ref1(w)
+        else:
+            u, _ = gpu(w, **opts)
+            npdt = np.float32
+            r = oracle.solve(N1, N2, 1.0, tau, M, phi.astype(npdt).astype(float), psi.astype(npdt).astype(float),
+                             c_half=c, s=s.astype(npdt).astype(float), g_half=g)
+        assert relerr(u, r) <= tol, (opts, relerr(u, r))
