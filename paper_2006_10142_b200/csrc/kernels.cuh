@@ -61,6 +61,7 @@ constexpr int ROW_CP = 8, ROW_INVP = 8 + KMAX, ROW_DOUBLES = 8 + 2 * KMAX;
 // streamed, starting NBK units early (carry warm-up) and ending >= NBK units late (carry look-ahead).
 struct Piece {
     int panel, ua, ub, nst;
+    int safe;   // 1: touches only lines the previous sweep finished in its static part (may start before it ends)
 };
 
 struct SweepArgs {
@@ -77,6 +78,10 @@ struct SweepArgs {
     int nstatic;           // pieces [0, nstatic) are dealt out statically, the rest through the ticket counter
     const int* cta_off;    // device: CTA b first works pieces [cta_off[b], cta_off[b+1])
     int* tickets;          // device: one zeroed counter per half-step (indexed like `table`)
+    int* done;             // device: one zeroed counter per half-step: CTAs whose static share is complete and visible
+    int signal;            // 1: the next sweep has safe pieces, so this one publishes `done`
+    int early;             // 1: the previous kernel in the stream is sweep nh - 1 of this handle (see "early start")
+    int prev_grid;         // its grid size
     void* out;             // y sweep: output field (direct coalesced stores)
     long long pitch;       // row pitch in elements
     const void* src;       // compact source window, [p - sp0][line - sl0] (line fastest), or NULL
@@ -231,7 +236,6 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     // Everything above touched only data no earlier kernel writes (the scalar table, the step counter, which
     // changes between graph launches only).  From here on the fields of the previous half-step are read.
     pdl_launch_dependents();
-    pdl_wait();
     int* const ticket = a.tickets + nh;
     int own_next = a.cta_off[blockIdx.x];
     const int own_end = a.cta_off[blockIdx.x + 1], nstatic = a.nstatic;
@@ -242,6 +246,36 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     if (threadIdx.x == 0) s_q[0] = draw();
     __syncthreads();
     const int npieces = a.npieces;
+    // ---- early start.  The previous sweep deals most of its work out statically and finishes the rest in short
+    // drawn pieces; its CTAs end several microseconds apart.  A CTA of this kernel that becomes resident meanwhile
+    // may already work a "safe" piece: one that reads and writes only lines the previous sweep completed in its
+    // static part (the host marks them; a CTA's share is ordered safe-first).  It waits until every CTA of the
+    // previous sweep has published "static share complete and visible" (counter `done`), with a time-out after which
+    // it simply waits for the whole previous kernel like any unsafe piece does (griddepcontrol.wait).
+    bool waited = false;
+    {
+        const bool try_early = a.early != 0 && s_q[0] < npieces && a.pieces[s_q[0]].safe != 0;
+        __shared__ int s_early_ok;
+        if (try_early) {
+            if (threadIdx.x == 0) {
+                const int* flag = a.done + (nh - 1);
+                int ok = 0;
+                for (int spin = 0; spin < 20000 && !ok; ++spin) {
+                    int v;
+                    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+                    ok = v >= a.prev_grid;
+                    if (!ok) __nanosleep(200);
+                }
+                s_early_ok = ok;
+            }
+            __syncthreads();
+            if (s_early_ok) asm volatile("fence.proxy.async;" ::: "memory");   // acquired generic writes -> our TMA reads
+        }
+        if (!try_early || !s_early_ok) {
+            pdl_wait();
+            waited = true;
+        }
+    }
     const int nbk = a.nbk, n = a.n, kb = a.kb, nlines = a.nlines;
     const long long pitch = a.pitch;
     [[maybe_unused]] T* const out_lane = reinterpret_cast<T*>(a.out) + (threadIdx.x & 31);
@@ -288,6 +322,10 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             ++q_ord;
             q_id = s_q[q_ord & (QR - 1)];
             if (q_id < npieces) q_pc = a.pieces[q_id];
+            if (!waited && !(q_id < npieces && q_pc.safe)) {   // the next piece needs the whole previous sweep
+                pdl_wait();
+                waited = true;
+            }
         }
     };
     // Thread 0 draws the producer's next piece as late as possible: in the stage whose produce() call finishes
@@ -404,6 +442,17 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 
     // The stage loop, compiled twice: DEF = false for warps that finish their unit in the same stage,
     // DEF = true for the last few warps, which keep the local x of their unit in registers for one stage.
+    // "static share complete": every warp makes its own stores visible (x sweep: its TMA stores have completed;
+    // y sweep: fence), then after the next CTA barrier thread 0 counts the CTA in `done` (release).
+    const int own_count = own_end - a.cta_off[blockIdx.x];
+    bool signaled = a.signal == 0, signaled_now = false;   // nothing to publish if nobody will look
+    auto publish_static_done = [&]() {
+        if constexpr (DIR == 0) {
+            if (lane == 0) tma_wait_all();
+        }
+        __threadfence();
+        signaled_now = true;
+    };
     auto run_pieces = [&](auto def_c) {
         constexpr bool DEF = decltype(def_c)::value;
         T pend[DEF ? U : 1];
@@ -420,7 +469,18 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             const bool src_line = line >= a.sl0 && line < a.sl0 + a.snl;
             const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
 
+            if (!signaled && ord > own_count) {   // static share and one drawn piece done: its stores have landed
+                publish_static_done();
+                signaled = true;
+            }
             named_bar_sync(1, NW * 32);   // the previous piece is completely finished
+            if (signaled_now) {
+                if (threadIdx.x == 0) {
+                    __threadfence();
+                    atomicAdd(a.done + nh, 1);
+                }
+                signaled_now = false;
+            }
             s_L[(NW + warp) * TL + lane] = T(0);   // "stage -1": zero carries
             if (lane == 0) s_A[NW + warp] = T(0);
 
@@ -564,6 +624,15 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     if (warp >= wdef) run_pieces(std::true_type{});
     else run_pieces(std::false_type{});
 
+    if (!waited) pdl_wait();   // (a CTA whose pieces were all safe) never exit before the previous kernel has
+    if (!signaled) {           // few or no drawn pieces: publish at the end
+        publish_static_done();
+        named_bar_sync(1, NW * 32);
+        if (threadIdx.x == 0) {
+            __threadfence();
+            atomicAdd(a.done + nh, 1);
+        }
+    }
     if constexpr (DIR == 0) {
         if (lane == 0) tma_wait_read<0>();
     }

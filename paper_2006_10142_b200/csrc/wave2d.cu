@@ -118,6 +118,7 @@ struct DirPlan {
     std::vector<Piece> pieces;
     std::vector<int> cta_off;   // CTA b's static share: pieces [cta_off[b], cta_off[b+1]); pieces >= nstatic are drawn
     int nstatic = 0;
+    bool has_safe = false;      // some static piece may start before the previous sweep ends (early start)
 };
 
 }  // namespace
@@ -152,7 +153,8 @@ struct wave2d_s {
     int* d_cta_off[2] = {nullptr, nullptr};
     double opt_static_frac = 0.75, opt_tail_div = 2.0;
     int opt_tail_min = 2;
-    int opt_trace = 0, opt_pdl = 1;
+    int opt_trace = 0, opt_pdl = 1, opt_early = 1;
+    int last_sweep = -1000;               // index of the sweep launched last on the stream (early start needs n - 1)
     unsigned long long* d_trace[2] = {nullptr, nullptr};   // per-CTA trace of the last launch per direction
     cudaGraphExec_t gexec = nullptr;
     int gexec_steps = 0;
@@ -348,6 +350,36 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
     while ((int)P.cta_off.size() < slots + 1) P.cta_off.push_back(P.nstatic);   // CTAs without a static share
 }
 
+// Early start (kernels.cuh): a static piece of direction d is "safe" if everything it reads and writes lies in grid
+// lines that the OTHER direction's sweep completes within its static part, i.e. before the first panel that has a
+// drawn piece.  Positions along a line of d are line indices of the other direction.  Each CTA's share is reordered
+// safe-first, so that a CTA that becomes resident during the previous sweep's tail has something to do.
+// Scheme 0 only (the ring of 3 makes the write set of a safe piece disjoint from what the previous tail still reads).
+void mark_safe_pieces(wave2d_t* h)
+{
+    for (int d = 0; d < 2; ++d) {
+        DirPlan& P = h->plan[d];
+        const DirPlan& O = h->plan[1 - d];
+        for (Piece& pc : P.pieces) pc.safe = 0;
+        P.has_safe = false;
+        if (!h->opt_early || h->scheme != 0 || P.solver != WAVE2D_SOLVER_STREAM || O.solver != WAVE2D_SOLVER_STREAM ||
+            P.nstatic == 0 || O.nstatic == 0 || O.nstatic >= (int)O.pieces.size())
+            continue;
+        const long long limit = (long long)O.pieces[O.nstatic].panel * 32 * O.var->vec;   // first line not surely done
+        const Variant& V = *P.var;
+        for (int i = 0; i < P.nstatic; ++i) {
+            Piece& pc = P.pieces[i];
+            const int gbase = std::max(pc.ua - P.nbk, 0) / V.sub * V.sub;
+            const long long end = (long long)(gbase + pc.nst * V.nw) * V.unit + 16;   // + neighbour points, margin
+            pc.safe = end <= limit ? 1 : 0;
+            P.has_safe = P.has_safe || pc.safe != 0;
+        }
+        for (size_t c = 0; c + 1 < P.cta_off.size(); ++c)   // safe pieces first within a CTA's share
+            std::stable_partition(P.pieces.begin() + P.cta_off[c], P.pieces.begin() + P.cta_off[c + 1],
+                                  [](const Piece& q) { return q.safe != 0; });
+    }
+}
+
 // x sweep load map: the field seen as (128-byte tile row, grid row, tile index along the row); a box of
 // [ntiles][32 rows][128 B] lands in shared memory tile after tile, each 128B-swizzled, and is 32 rows x
 // ntiles * 128 contiguous bytes in global memory.  Elements beyond n1 inside the last tile are the zero pad columns.
@@ -466,6 +498,7 @@ int ensure_plan(wave2d_t* h)
         st = plan_dir(h, d);
         if (st) return st;
     }
+    mark_safe_pieces(h);
     for (int b = 0; b < (h->scheme == 1 ? 4 : 3); ++b) {
         if (h->plan[0].solver == WAVE2D_SOLVER_STREAM) {
             const int U = h->plan[0].var->unit;
@@ -545,6 +578,11 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         a.table = h->d_table; a.table_period = h->table_period; a.d_k = dk; a.n_off = n_off;
         a.n = P.n; a.nlines = (P.nlines + P.var->vec - 1) / P.var->vec; a.nbk = P.nbk; a.kb = P.kb;
         a.pieces = h->d_pieces[d]; a.npieces = (int)P.pieces.size(); a.tickets = h->d_tickets;
+        a.done = h->d_tickets + 2 * h->M + 2;
+        a.early = h->opt_early && h->opt_pdl && h->scheme == 0 && h->last_sweep == n_abs - 1 &&
+                  h->plan[1 - d].solver == WAVE2D_SOLVER_STREAM;
+        a.prev_grid = h->plan[1 - d].grid;
+        a.signal = h->plan[1 - d].has_safe ? 1 : 0;
         a.cta_off = h->d_cta_off[d]; a.nstatic = P.nstatic;
         a.out = out; a.pitch = h->pitch / P.var->vec;   // in units of the kernel's T
         a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
@@ -567,6 +605,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         cfg.attrs = at;
         cfg.numAttrs = h->opt_pdl ? 1 : 0;
         W2D_CUDA(h, cudaLaunchKernelExC(&cfg, P.var->fn, args));
+        h->last_sweep = n_abs;
         h->launches += 1;
         return WAVE2D_OK;
     }
@@ -590,6 +629,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     }
 #undef W2D_EXACT
     W2D_CUDA(h, cudaGetLastError());
+    h->last_sweep = -1000;
     h->launches += 3;
     return WAVE2D_OK;
 }
@@ -600,6 +640,7 @@ int build_graph(wave2d_t* h, int steps)
     cudaGraph_t g = nullptr;
     W2D_CUDA(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
     const long long l0 = h->launches;
+    h->last_sweep = -1000;   // the first sweep of a replay follows the counter kernel, not a sweep
     int st = WAVE2D_OK;
     for (int s = 0; s < steps && st == WAVE2D_OK; ++s) {
         st = launch_half_step(h, 2 * s, 2 * s, true);
@@ -607,6 +648,7 @@ int build_graph(wave2d_t* h, int steps)
     }
     if (st == WAVE2D_OK) wave2d_bump_counter<<<1, 1, 0, h->stream>>>(h->d_k, steps);
     h->launches = l0;   // capture is not execution
+    h->last_sweep = -1000;
     cudaError_t e = cudaStreamEndCapture(h->stream, &g);
     if (st != WAVE2D_OK) {
         if (g) cudaGraphDestroy(g);
@@ -686,9 +728,10 @@ int set_initial_factored(wave2d_t* h, const void* phi, const void* psi, long ld)
                                                             h->pitch, -h->tau);
     W2D_CUDA(h, cudaGetLastError());
     W2D_CUDA(h, cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream));
-    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)2 * h->M + 2) * sizeof(int), h->stream));
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)4 * h->M + 4) * sizeof(int), h->stream));
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_initial = true;
+    h->last_sweep = -1000;
     h->v_ready = false;
     h->k = 1;
     h->ran = false;
@@ -750,7 +793,7 @@ int wave2d_create(wave2d_t** out, int N1, int N2, double l, double tau, int M, i
     int st = WAVE2D_OK;
     for (int b = 0; b < 3 && st == WAVE2D_OK; ++b) st = dev_alloc(h, &h->buf[b], fbytes);
     if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_k), sizeof(int));
-    const size_t tk_bytes = ((size_t)2 * M + 2) * sizeof(int);
+    const size_t tk_bytes = ((size_t)4 * M + 4) * sizeof(int);   // tickets[2M+2] | done[2M+2]
     if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_tickets), tk_bytes);
     if (st == WAVE2D_OK) {
         for (int b = 0; b < 3; ++b) cudaMemsetAsync(h->buf[b], 0, fbytes, h->stream);
@@ -795,6 +838,7 @@ int wave2d_set_stream(wave2d_t* h, void* cuda_stream)
     if (!h) return WAVE2D_ERR_ARG;
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->stream = cuda_stream ? static_cast<cudaStream_t>(cuda_stream) : h->own_stream;
+    h->last_sweep = -1000;
     drop_graph(h);
     return WAVE2D_OK;
 }
@@ -823,6 +867,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
     else if (!strcmp(name, "trace")) h->opt_trace = iv != 0;
     else if (!strcmp(name, "pdl")) h->opt_pdl = iv != 0;
+    else if (!strcmp(name, "early")) h->opt_early = iv != 0;
     else if (!strcmp(name, "tail_min")) { if (iv < 1) return WAVE2D_ERR_ARG; h->opt_tail_min = iv; }
     else if (!strcmp(name, "tail_div")) { if (!(value >= 0.25)) return WAVE2D_ERR_ARG; h->opt_tail_div = value; }
     else if (!strcmp(name, "static_frac")) { if (!(value >= 0.0 && value <= 1.0)) return WAVE2D_ERR_ARG; h->opt_static_frac = value; }
@@ -855,9 +900,10 @@ int wave2d_set_initial(wave2d_t* h, const void* phi, const void* psi, long ld)
                                                             h->pitch, 0.5 * h->tau);
     W2D_CUDA(h, cudaGetLastError());
     W2D_CUDA(h, cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream));
-    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)2 * h->M + 2) * sizeof(int), h->stream));   // work queues
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)4 * h->M + 4) * sizeof(int), h->stream));   // work queues
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_initial = true;
+    h->last_sweep = -1000;
     h->k = 0;
     h->ran = false;
     return WAVE2D_OK;
@@ -871,9 +917,10 @@ int wave2d_set_state(wave2d_t* h, int k, const void* u_prev_half, const void* u,
     int st = copy_in(h, h->buf[(2 * k) % 3], u_prev_half, ld);
     if (st == WAVE2D_OK) st = copy_in(h, h->buf[(2 * k + 1) % 3], u, ld);
     if (st) return st;
-    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)2 * h->M + 2) * sizeof(int), h->stream));
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)4 * h->M + 4) * sizeof(int), h->stream));
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_initial = true;
+    h->last_sweep = -1000;
     h->k = k;
     return WAVE2D_OK;
 }
@@ -968,6 +1015,7 @@ int wave2d_run(wave2d_t* h, int steps)
                 counter_set = true;
             }
             W2D_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
+            h->last_sweep = -1000;
             h->launches += launches_per_step(h) * gs + 1;
             h->k += gs;
             left -= gs;
