@@ -103,6 +103,9 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (units per stage = consumer warps / stages).
  *   "pdl"    1 (default): sweep kernels are launched with programmatic stream serialization, so that a kernel's
  *            prologue overlaps the tail of the previous one (it waits for it before touching the fields).
+ *   "early"  1 (default): early start -- a CTA that becomes resident while the previous sweep is still finishing its
+ *            last drawn pieces begins with a piece of its share that touches only grid lines that sweep completed in
+ *            its static part; needs "pdl".  0: every CTA waits for the whole previous sweep.
  *   "trace"  1: sweep kernels record per-CTA timing (see wave2d_get_trace).  Default 0.
  *   "quota_x", "quota_y"   tuning: length in stages of every piece of work a line is cut into (0 = planned:
  *                          guided self-scheduling, long pieces first, short ones last).

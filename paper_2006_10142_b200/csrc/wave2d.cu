@@ -354,7 +354,9 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
 // lines that the OTHER direction's sweep completes within its static part, i.e. before the first panel that has a
 // drawn piece.  Positions along a line of d are line indices of the other direction.  Each CTA's share is reordered
 // safe-first, so that a CTA that becomes resident during the previous sweep's tail has something to do.
-// Scheme 0 only (the ring of 3 makes the write set of a safe piece disjoint from what the previous tail still reads).
+// Hazards: a safe piece writes only safe lines of a buffer in which the previous sweep's tail still reads at most its
+// own (unsafe) lines -- scheme 0: w_{n+2} overwrites w_{n-1}; scheme 1: U^{k+1} overwrites V^{k-1}, V^{k+2} overwrites U^k,
+// which the y sweep before it never touches.
 void mark_safe_pieces(wave2d_t* h)
 {
     for (int d = 0; d < 2; ++d) {
@@ -362,7 +364,7 @@ void mark_safe_pieces(wave2d_t* h)
         const DirPlan& O = h->plan[1 - d];
         for (Piece& pc : P.pieces) pc.safe = 0;
         P.has_safe = false;
-        if (!h->opt_early || h->scheme != 0 || P.solver != WAVE2D_SOLVER_STREAM || O.solver != WAVE2D_SOLVER_STREAM ||
+        if (!h->opt_early || P.solver != WAVE2D_SOLVER_STREAM || O.solver != WAVE2D_SOLVER_STREAM ||
             P.nstatic == 0 || O.nstatic == 0 || O.nstatic >= (int)O.pieces.size())
             continue;
         const long long limit = (long long)O.pieces[O.nstatic].panel * 32 * O.var->vec;   // first line not surely done
@@ -579,7 +581,7 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         a.n = P.n; a.nlines = (P.nlines + P.var->vec - 1) / P.var->vec; a.nbk = P.nbk; a.kb = P.kb;
         a.pieces = h->d_pieces[d]; a.npieces = (int)P.pieces.size(); a.tickets = h->d_tickets;
         a.done = h->d_tickets + 2 * h->M + 2;
-        a.early = h->opt_early && h->opt_pdl && h->scheme == 0 && h->last_sweep == n_abs - 1 &&
+        a.early = h->opt_early && h->opt_pdl && h->last_sweep == n_abs - 1 &&
                   h->plan[1 - d].solver == WAVE2D_SOLVER_STREAM;
         a.prev_grid = h->plan[1 - d].grid;
         a.signal = h->plan[1 - d].has_safe ? 1 : 0;
