@@ -179,7 +179,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 // Panel sweep: RHS assembly (A1/A3) fused with the line solve (A2/A4), SURVEY.md 8a.
 //   grid  = persistent CTAs (SM count x CTAs/SM); CTA b walks its host-planned pieces.
 //   block = NW warps.  Per stage, warp w owns unit g = gbase + s*NW + w (UT points) of the panel's 32
-//           lines, lane = line.  Thread 0 also feeds the ring of NSTAGE TMA stages.
+//           lines, lane = line.  Lane 0 of a few warps requests the stage's TMA boxes (ring of NSTAGE stages).
 //   stage:  smem -> registers; RHS + local forward; publish L, A; bar (the slot is free: refill it);
 //           carry-in, correct y, local backward; publish head; bar;
 //           warps whose look-ahead heads are all in this stage finish and store their unit now, the last
@@ -493,7 +493,8 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 draw_ahead();   // (thread 0) the ticket's round trip overlaps this stage's first half
                 const unsigned char* st = sm + slot * K::STAGE_BYTES;
                 if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
-                T wp[U], wc[U], wl, wr;
+                [[maybe_unused]] T wp[U], wl, wr;
+                T wc[U];
                 if constexpr (DIR == 0) {
                     const unsigned char* tp = st + tix * 4096;
                     load_unit_x<T, U>(tp, lane, sub, wp);

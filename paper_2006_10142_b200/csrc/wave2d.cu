@@ -680,16 +680,6 @@ long long launches_per_step(const wave2d_t* h)
     return n;
 }
 
-bool is_device_ptr(const void* p)
-{
-    cudaPointerAttributes at;
-    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
-        (void)cudaGetLastError();
-        return false;
-    }
-    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
-}
-
 int copy_in(wave2d_t* h, void* dst, const void* src, long ld)
 {
     W2D_CUDA(h, cudaMemcpy2DAsync(dst, (size_t)h->pitch * h->elem, src, (size_t)ld * h->elem, (size_t)h->n1 * h->elem,
