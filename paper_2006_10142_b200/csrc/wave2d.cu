@@ -605,7 +605,9 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // overlap our prologue with the previous
         at[0].val.programmaticStreamSerializationAllowed = 1;            // kernel's tail (griddepcontrol.wait inside)
         cfg.attrs = at;
-        cfg.numAttrs = h->opt_pdl ? 1 : 0;
+        // Only behind a sweep of our own: a kernel that follows something else (the step-counter kernel at the start
+        // of a graph replay, a copy) reads the step counter before griddepcontrol.wait and must see it final.
+        cfg.numAttrs = h->opt_pdl && h->last_sweep == n_abs - 1 ? 1 : 0;
         W2D_CUDA(h, cudaLaunchKernelExC(&cfg, P.var->fn, args));
         h->last_sweep = n_abs;
         h->launches += 1;
