@@ -418,7 +418,13 @@ int plan_dir(wave2d_t* h, int d)
     P.nlines = d == 0 ? h->n2 : h->n1;
     P.shape = h->opt_shape[d];
     const int one = h->scheme == 1 && d == 1;
-    if (one) P.shape = std::min(P.shape, 1);
+    if (one) {
+        P.shape = std::min(P.shape, 1);
+        // Large grids (>= 128 stages of 4096 points per SM): 16-point units halve the barrier rounds per point and
+        // the longer pieces cost nothing there (config 5: +4.5 %); smaller grids keep 8-point units (shorter tail).
+        const long long work = (long long)((P.nlines + 31) / 32) * ((P.n + 127) / 128);
+        if (h->opt_shape[d] == 0 && h->elem == 8 && work >= 128LL * h->num_sms) P.shape = 1;
+    }
     P.var = find_variant(h->elem, d, P.shape, one);
     if (P.var && P.var->vec == 2 && ((h->have_src && !one) || (h->pitch & 1))) P.var = find_variant(h->elem, d, P.shape + 1, one);
     if (!P.var) {
