@@ -548,3 +548,33 @@ def test_tiny_and_ragged_sizes_fp32_and_scheme1(N1, N2, dtype, scheme):
             r = oracle.solve(N1, N2, 1.0, tau, M, phi.astype(npdt).astype(float), psi.astype(npdt).astype(float),
                              c_half=c, s=s.astype(npdt).astype(float), g_half=g)
         assert relerr(u, r) <= tol, (opts, relerr(u, r))
+
+
+def test_early_start_and_pdl_do_not_change_a_single_bit():
+    """Early start only changes WHEN a piece runs (and the order of a CTA's share), programmatic launch only how
+    kernels are chained: with both off, one off, both on, three runs each way must agree bit for bit on a grid with
+    several pieces per CTA, a source and time-varying c (split scheme) -- and the same for scheme 1."""
+    w = W.cfg2(N=2048, M=26)
+    src = W.cfg3(N=2048, M=26)
+    w.s, w.g_half = src.s, W.ricker(W.half_times(w.tau, 2 * w.M) + 0.058)
+    base, _ = gpu(w, early=0, pdl=0)
+    assert relerr(base, ref(w)) <= 1e-10
+    for opts in ({"early": 1}, {"early": 0}, {"early": 1, "graph": 0}, {"early": 1}, {"early": 1}):
+        u, _ = gpu(w, **opts)
+        assert np.array_equal(u, base), opts
+    base1, _ = gpu1(w, early=0, pdl=0)
+    assert relerr(base1, ref1(w)) <= 1e-10
+    for opts in ({"early": 1}, {"early": 1, "graph": 0}, {"early": 1}):
+        u, _ = gpu1(w, **opts)
+        assert np.array_equal(u, base1), opts
+
+
+def test_factored_scheme_large_tau_falls_back_to_exact_solver():
+    N, M = 160, 10
+    w = W.cfg2(N=N, M=M)
+    w.tau = 16.0 / N
+    w.psi = 0.2 * w.phi
+    r = ref1(w)
+    u, info = gpu1(w)
+    assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
+    assert relerr(u, r) <= 1e-10

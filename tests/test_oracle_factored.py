@@ -162,3 +162,14 @@ def test_anisotropic_grid_uses_h1_in_x_and_h2_in_y():
     assert np.abs(u - amps[M] * shape).max() <= 1e-13
     wrong = modal_amplitudes_factored(N2, N1, 1.0, tau, 1, 2, 1.0, 0.5, np.ones(2 * M + 1), M)
     assert abs(wrong[M] - amps[M]) > 1e-3
+
+
+def test_unconditionally_stable_at_large_time_steps():
+    """the implicit three-level scheme is unconditionally stable; so is its factorised form (per mode the
+    recurrence A_{k+1} = (2 A_k - d A_{k-1}) / d with d >= 1 has |roots| = 1): tau = 64 h for 300 steps stays bounded."""
+    N, M = 32, 300
+    tau = 64.0 / N
+    x = np.arange(1, N) / N
+    phi = np.outer(np.sin(np.pi * x), np.sin(2 * np.pi * x)) + 0.5 * np.outer(np.sin(5 * np.pi * x), np.sin(3 * np.pi * x))
+    u = oracle.solve(N, N, 1.0, tau, M, phi, None, scheme=1)
+    assert np.isfinite(u).all() and np.abs(u).max() <= 1.0 + 1e-9 + np.abs(phi).max()
