@@ -152,7 +152,7 @@ struct wave2d_s {
     int* d_tickets = nullptr;              // one work-queue counter per half-step
     int* d_cta_off[2] = {nullptr, nullptr};
     double opt_static_frac = 0.75, opt_tail_div = 2.0;
-    int opt_tail_min = 2;
+    int opt_tail_min = 0, opt_tail_max = 6;   // tail_min 0: planned from the stage size
     int opt_trace = 0, opt_pdl = 1, opt_early = 1;
     int last_sweep = -1000;               // index of the sweep launched last on the stream (early start needs n - 1)
     unsigned long long* d_trace[2] = {nullptr, nullptr};   // per-CTA trace of the last launch per direction
@@ -295,7 +295,8 @@ int make_tmap(wave2d_t* h, CUtensorMap* tm, void* base, int box0, int box1, int 
 // counter once their own share is done, so that CTAs the memory system serves more slowly get less of it.  The
 // short pieces follow guided self-scheduling (remaining / (2 slots) stages, between 2 and 6).
 // `fixed` > 0 (tests): no static part, every piece `fixed` stages long.
-void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double static_frac, int tail_min, double tail_div)
+void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double static_frac, int tail_min, double tail_div,
+                  int tail_max = 6)
 {
     P.pieces.clear();
     P.cta_off.assign(1, 0);
@@ -328,8 +329,9 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
     if (fixed == 0 && P.nstatic == 0 && total < 4LL * slots) {
         // Small problem (a CTA gets at most a few stages): one wave of equal pieces, at most one per CTA, because a
         // second piece on some CTAs would double the kernel time.  k pieces per line, each st stages.
-        const int k = (int)std::max<long long>(1, std::min<long long>(slots / P.npanels, SL / min_st));
-        const int st = std::max(min_st, (UT + (k - 1) * 2 * P.nbk + k * nw - 1) / (k * nw));
+        const int min_one = std::max(2, (2 * P.nbk + sub) / nw + 1);   // (tail_min is about the drawn tail only)
+        const int k = (int)std::max<long long>(1, std::min<long long>(slots / P.npanels, SL / min_one));
+        const int st = std::max(min_one, (UT + (k - 1) * 2 * P.nbk + k * nw - 1) / (k * nw));
         while (panel < P.npanels) take(st, st - 1);
         P.nstatic = (int)P.pieces.size();   // all static (CTA c owns pieces c, c + slots, ...: here just piece c):
         const int per = (P.nstatic + slots - 1) / slots;   // no ticket is ever drawn
@@ -339,7 +341,7 @@ void build_pieces(DirPlan& P, int nw, int sub, int slots, int fixed, double stat
     double remaining = 0.0;
     if (panel < P.npanels) remaining = (double)(P.npanels - panel) * SL - (double)ua / nw;
     while (panel < P.npanels) {
-        int st = fixed > 0 ? fixed : std::min(6, (int)(remaining / (tail_div * slots)));
+        int st = fixed > 0 ? fixed : std::min(tail_max, (int)(remaining / (tail_div * slots)));
         st = std::max(st, min_st);
         const int ua_before = ua, panel_before = panel;
         take(st, (st + 1) / 2);
@@ -477,7 +479,12 @@ int plan_dir(wave2d_t* h, int d)
     P.total_units = (P.n + U - 1) / U;
     // Persistent grid, one wave; the CTAs draw the pieces from an atomic ticket counter.
     const int slots = per_sm * h->num_sms;
-    build_pieces(P, V.nw, V.sub, slots, h->opt_quota[d], h->opt_static_frac, h->opt_tail_min, h->opt_tail_div);
+    // shortest drawn piece: ~16 K points of work per line panel (4 stages of 4096 points in fp64, 2 of 8192 in fp32):
+    // shorter pieces pay relatively more for their carry warm-up, longer ones lengthen the tail of the kernel
+    const int stage_points = V.nw * V.unit * 32 * V.vec;
+    const int tail_min = h->opt_tail_min > 0 ? h->opt_tail_min : std::min(6, std::max(2, 16384 / stage_points));
+    build_pieces(P, V.nw, V.sub, slots, h->opt_quota[d], h->opt_static_frac, tail_min, h->opt_tail_div,
+                 h->opt_tail_max);
     P.quota = h->opt_quota[d];
     P.grid = slots;
     return WAVE2D_OK;
@@ -868,7 +875,8 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "trace")) h->opt_trace = iv != 0;
     else if (!strcmp(name, "pdl")) h->opt_pdl = iv != 0;
     else if (!strcmp(name, "early")) h->opt_early = iv != 0;
-    else if (!strcmp(name, "tail_min")) { if (iv < 1) return WAVE2D_ERR_ARG; h->opt_tail_min = iv; }
+    else if (!strcmp(name, "tail_max")) { if (iv < 1) return WAVE2D_ERR_ARG; h->opt_tail_max = iv; }
+    else if (!strcmp(name, "tail_min")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_tail_min = iv; }
     else if (!strcmp(name, "tail_div")) { if (!(value >= 0.25)) return WAVE2D_ERR_ARG; h->opt_tail_div = value; }
     else if (!strcmp(name, "static_frac")) { if (!(value >= 0.0 && value <= 1.0)) return WAVE2D_ERR_ARG; h->opt_static_frac = value; }
     else if (!strcmp(name, "quota_x")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[0] = iv; }
@@ -1164,7 +1172,8 @@ int wave2d_host_plan(int n, int nlines, int unit, int units_per_stage, int units
     P.n = n; P.nlines = nlines; P.nbk = nbk;
     P.npanels = (nlines + 31) / 32;
     P.total_units = (n + unit - 1) / unit;
-    build_pieces(P, units_per_stage, units_per_tile, slots, fixed_stages, static_frac, 2, 2.0);
+    const int tail_min = std::min(6, std::max(2, 16384 / (units_per_stage * unit * 32)));   // as plan_dir
+    build_pieces(P, units_per_stage, units_per_tile, slots, fixed_stages, static_frac, tail_min, 2.0);
     *npieces = (int)P.pieces.size();
     *nstatic = P.nstatic;
     if (capacity < *npieces) return WAVE2D_ERR_ARG;
