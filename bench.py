@@ -401,12 +401,14 @@ def run_ours(args):
                      "step_passes": passes, "step_frac": passes * fbytes / step_s / 1e9 / peak,
                      "step_frac6": 6 * fbytes / step_s / 1e9 / peak, "step_frac5": 5 * fbytes / step_s / 1e9 / peak},
     }
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(traffic_file):   # dram bytes per launch from the committed ncu --set full capture
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(traffic_file):   # dram bytes per launch from the committed ncu --set full capture (r1g_summary.md)
         try:
-            t = json.load(open(traffic_file)).get(f"{w.name}:{dom}" + (":scheme1" if sch else ""))
-            if t:
-                line["roofline"]["traffic"] = t
+            key = f"{w.name}:{dom}" + (":scheme1" if sch else "")
+            for ln in open(traffic_file).read().splitlines()[1:]:
+                k, v = ln.rsplit(",", 1)
+                if k == key:
+                    line["roofline"]["traffic"] = int(v)
         except Exception:
             pass
     if rank == 0:
