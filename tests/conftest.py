@@ -13,6 +13,16 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "slow: full-size oracle comparison, opt-in via WAVE2D_FULL_PARITY=1")
 
 
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """Build the C-ABI library and the oracle if they are missing or older than their sources (in-tree, nvcc / gcc):
+    the tests never run against a stale or absent build, and never against anything but libwave2d.so."""
+    from paper_2006_10142_b200 import build as _b
+    from oracle import oracle as _o
+    _b.build()
+    _o.build()
+
+
 def _has_gpu():
     try:
         import torch
