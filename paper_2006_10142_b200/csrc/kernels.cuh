@@ -112,7 +112,7 @@ struct PanelCfg {
     static constexpr int OUT_BYTES = DIR == 0 ? NW * 2 * 32 * RB : 0;   // two store tiles per warp
     static constexpr int BAR_BYTES = ((NSTAGE * 8) + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * KMAX * (int)sizeof(T);
-    static constexpr int XCH_BYTES = (4 * NW * TL + 2 * NW + UT) * (int)sizeof(T);   // L[2NW][32], H[2NW][32], A[2NW], pw[UT]
+    static constexpr int XCH_BYTES = (4 * NW * TL + 4 * NW + UT) * (int)sizeof(T);   // L, H [2NW][32]; A, AH [2NW]; pw[UT]
     static constexpr int SMEM_BYTES = 1024 + NSTAGE * STAGE_BYTES + OUT_BYTES + BAR_BYTES + TAB_BYTES + XCH_BYTES;
     static constexpr int THREADS = 32 * NW;
     static_assert((NW & (NW - 1)) == 0, "NW must be a power of two (ring indexing)");
@@ -206,6 +206,8 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     T* s_H = s_L + RING * TL;        // [RING][32]  first local x of a unit
     T* s_A = s_H + RING * TL;        // [RING]      product of the unit's cp
     T* s_pw = s_A + RING;            // [U]         rho^(e+1)
+    T* s_AH = s_pw + U;              // [RING]      the same product, published with H (read by the carry from the right,
+                                     //             which outlives the stage: s_A is rewritten one barrier earlier)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nh = a.n_off + (a.d_k ? 2 * (*a.d_k) : 0);
@@ -360,7 +362,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     // carry series: value entering unit `ring` from the left (dirn = -1, over L) or from the right (+1, over H)
     // `stat`: all nbk units of the series are whole units with stationary pivots, so every A is rho^U.
     const T pwU = pw_at(U - 1);
-    auto carry = [&](const T* vals_lane, int ring, int dirn, bool stat) -> T {
+    auto carry = [&](const T* vals_lane, const T* fac, int ring, int dirn, bool stat) -> T {
         T c = T(0);
         if (stat) {
             if (nbk > 4) {
@@ -378,21 +380,21 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             for (int j = NBK_MAX; j > 4; --j)
                 if (j <= nbk) {
                     const int idx = (ring + dirn * j) & (RING - 1);
-                    c = fmaT(s_A[idx], c, vals_lane[idx * TL]);
+                    c = fmaT(fac[idx], c, vals_lane[idx * TL]);
                 }
         }
 #pragma unroll
         for (int j = 4; j >= 1; --j)
             if (j <= nbk) {
                 const int idx = (ring + dirn * j) & (RING - 1);
-                c = fmaT(s_A[idx], c, vals_lane[idx * TL]);
+                c = fmaT(fac[idx], c, vals_lane[idx * TL]);
             }
         return c;
     };
 
     // finish unit gp (local x in v[]): add the carry from the right, store
     auto finish = [&](T (&v)[U], int gp, int ring, const Piece& pc) {
-        const T Xin = carry(sH_lane, ring, +1, gp + 1 >= kb && (gp + nbk + 1) * U <= n);   // x at the start of unit gp+1
+        const T Xin = carry(sH_lane, s_AH, ring, +1, gp + 1 >= kb && (gp + nbk + 1) * U <= n);   // x at the start of unit gp+1
         if (gp < pc.ua || gp >= pc.ub) return;    // warp-uniform
         const int pp0 = gp * U;
         const bool full = pp0 + U <= n;
@@ -581,7 +583,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 produce();   // every warp holds its stage data in registers: refill the slot
 
                 // ---- carry from the left, local back substitution
-                const T Yin = carry(sL_lane, ring, -1, g - nbk >= kb && p0 <= n);   // y at the end of unit g-1
+                const T Yin = carry(sL_lane, s_A, ring, -1, g - nbk >= kb && p0 <= n);   // y at the end of unit g-1
 #ifdef W2D_COPY_PROBE
                 if (true) {
                     xl[0] += Yin;
@@ -602,6 +604,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                     for (int e = U - 2; e >= 0; --e) xl[e] = fmaT(cp_at(p0 + e), xl[e + 1], xl[e]);
                 }
                 s_H[ring * TL + lane] = xl[0];
+                if (lane == 0) s_AH[ring] = Aval;
                 named_bar_sync(1, NW * 32);
 
                 // ---- carry from the right, store
@@ -615,6 +618,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             }
             // ---- flush: the deferred units of the last stage see zero heads beyond it
             const int ringf = (pc.nst & 1) * NW + warp;
+            named_bar_sync(1, NW * 32);   // the deferred warps have read the heads of stage nst-2 (same half of the ring)
             s_H[ringf * TL + lane] = T(0);
             named_bar_sync(1, NW * 32);
             if constexpr (DEF) {
