@@ -325,6 +325,7 @@ def run_ours(args):
     sampler.start()
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps between two events on the stream
+    h.run(0)                                # plan + graphs (captured, instantiated, uploaded) before anything is timed
     h.run(Wm)
     h.sync()
     l0 = h.info("launches")
@@ -339,6 +340,7 @@ def run_ours(args):
     tw1 = time.perf_counter()
     ms = max_over_ranks(float(ev0.elapsed_time(ev1)))
     launches = int(h.info("launches") - l0)
+    graph_replays, plain_sweeps = int(h.info("graph_launches")), int(h.info("plain_sweeps"))
     clocks = sampler.stop(tw0, tw1) or {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable"]}
 
     # ---- per-kernel timing of the two sweep kernels, live, CUDA events on the same stream
@@ -399,7 +401,12 @@ def run_ours(args):
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                      "peak_source": peak_src, "bytes_per_launch": sweep_bytes,
                      "ms_per_launch": ms_dom, "share_of_step": share_dom,
-                     "how": "timed region (graph replay, events on the stream) x kernel share of the step",
+                     "how": "method 'share': K-step timed region (graph replays only, CUDA events on the launching "
+                            "stream) / K = step time; x the kernel's share of the step taken from the per-launch "
+                            "events of wave2d_profile_sweeps (sweeps overlap at their boundaries by programmatic "
+                            "launch, so a launch has no separate duration inside the region); 'isolated' below = "
+                            "plain launches with an event pair per kernel; ncu (serialised, cold) in profiles/",
+                     "graph_replays_total": graph_replays, "sweeps_outside_graphs": plain_sweeps,
                      "isolated": {"what": "plain launches, one event pair per kernel (includes a launch gap)",
                                   "ms_x": ms_x, "ms_y": ms_y,
                                   "gbs_x": bytes_x / ms_x / 1e6, "gbs_y": bytes_y / ms_y / 1e6,
@@ -410,7 +417,9 @@ def run_ours(args):
                      "step_frac6": 6 * fbytes / step_s / 1e9 / peak, "step_frac5": 5 * fbytes / step_s / 1e9 / peak},
     }
     traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(traffic_file):   # dram bytes per launch from the committed ncu --set full capture (r1g_summary.md)
+    line["roofline"]["traffic_source"] = "profiles/traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum of one " \
+                                         "committed ncu --set full capture of this kernel (not measured by this run)"
+    if os.path.exists(traffic_file):
         try:
             key = f"{w.name}:{dom}" + (":scheme1" if sch else "")
             for ln in open(traffic_file).read().splitlines()[1:]:

@@ -25,7 +25,7 @@
  *   - Half-level index n = 0,1,2,...: t = n tau/2; the half-step n -> n+1 is implicit in x for even n and
  *     in y for odd n.  c_half[n] = c(n tau/2), g_half[n] = g(n tau/2).
  *   - The handle owns all device memory it allocates (three pitched field buffers, the optional source
- *     field, a per-half-step scalar table) and frees it in wave2d_destroy().
+ *     field, a per-half-step scalar table, the work plan) and frees it in wave2d_destroy().
  *   - One handle is single-threaded; distinct handles are independent.  Work is asynchronous on the
  *     handle's stream unless stated otherwise.
  *
@@ -66,8 +66,7 @@ enum {
 /*
  * Create a solver for the grid of (2.6)-(2.7): N1 x N2 intervals on [0,l]^2, time step tau, at most M
  * steps (T = M tau), dtype WAVE2D_F64 or WAVE2D_F32.  Defaults: c == 1, no source, gamma = 2,
- * kappa = 1/2 (see wave2d_set_option).  Uses the current CUDA device and a non-blocking stream of its own
- * (CUDA Graph capture is not possible on the legacy default stream).
+ * kappa = 1/2 (see wave2d_set_option).  Uses the current CUDA device and a non-blocking stream of its own.
  * Errors: ERR_ARG (N < 2, l <= 0, tau <= 0, M < 0, bad dtype, out == NULL), ERR_ALLOC, ERR_CUDA
  * (no device, or not an sm_100 device), ERR_UNSUPPORTED (a line too long for every solver path).
  */
@@ -97,9 +96,13 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *               ERR_UNSUPPORTED: the ring carries (I - ay Dy) u^{k-1}, not u^{k-1}.  Must be set before
  *               wave2d_set_initial (ERR_ARG afterwards).  Uses a fourth field buffer.
  *   "solver" one of WAVE2D_SOLVER_*.     Default AUTO.
- *   "graph"  1 (default): the step loop is replayed as a CUDA Graph; 0: plain launches.
- *   "graph_steps"  time steps per graph replay (multiple of 3; scheme 1 also needs a multiple of 4, the period
- *            of its ring, else it falls back to plain launches).  Default 12.
+ *   "graph"  1 (default): the step loop is replayed as CUDA Graphs; 0: the same kernel sequence launched directly.
+ *            The loop runs in chunks of 2^i time steps, longest first (20 steps = 16 + 4); one graph per chunk length is
+ *            captured, instantiated and uploaded when the plan is made (first wave2d_run / wave2d_get_info after the
+ *            last set_* call; wave2d_run(h, 0) forces it), never inside a later run call.  The kernels take the buffer
+ *            roles of the time-level ring from the device step counter, so every graph serves every phase of the
+ *            ring and no step of any run call is launched outside a graph.
+ *   "graph_steps"  longest chunk in time steps: 1, 2, 4, 8, 16 or 32 (default 32).
  *   "shape_x", "shape_y"   tuning: kernel shape variant 0..3 (units per stage = consumer warps / stages).
  *   "pdl"    1 (default): sweep kernels are launched with programmatic stream serialization, so that a kernel's
  *            prologue overlaps the tail of the previous one (it waits for it before touching the fields).
@@ -173,6 +176,11 @@ int wave2d_sync(wave2d_t *h);
  *   "upc_*" (units per CTA)  launch geometry
  *   "source_window"          points kept of the source field (its non-zero bounding box)
  *   "launches"               kernels launched by this handle so far (graph nodes count individually)
+ *   "graph_launches"         graph replays issued by wave2d_run so far
+ *   "plain_sweeps"           sweep kernels launched outside a graph so far (0 unless "graph" = 0 or
+ *                            wave2d_profile_sweeps was used)
+ *   "static_*", "safe_*"     pieces dealt out statically / of those, pieces that may start before the previous
+ *                            sweep has ended (early start)
  *   "pitch"                  internal row pitch in elements
  *   "device_bytes"           device memory owned by the handle
  * The plan is (re)computed by this call if needed.  Errors: ERR_ARG.

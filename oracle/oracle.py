@@ -18,7 +18,9 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "wave2d_oracle.c")
-_LIB = os.path.join(_HERE, "liboracle_wave2d.so")
+# WAVE2D_ORACLE_SANITIZE=1: a separate ASan + UBSan build (run python with LD_PRELOAD=$(gcc -print-file-name=libasan.so))
+_SANITIZE = os.environ.get("WAVE2D_ORACLE_SANITIZE") == "1"
+_LIB = os.path.join(_HERE, "liboracle_wave2d_san.so" if _SANITIZE else "liboracle_wave2d.so")
 _lock = threading.Lock()
 _lib = None
 
@@ -29,8 +31,9 @@ def build(force: bool = False) -> str:
     """Compile oracle/wave2d_oracle.c -> oracle/liboracle_wave2d.so (gcc -O2 -fopenmp)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + f".tmp{os.getpid()}"
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if _SANITIZE else ["-O2"]
         subprocess.check_call(
-            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"])
+            ["gcc"] + flags + ["-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 

@@ -10,8 +10,8 @@
  * the loop of Algorithm 1.  Only tests/, __graft_entry__.smoke() and bench.py's
  * cpu_baseline / --impl reference leg may call this file.  It shares no code, header, table or
  * constant with the CUDA path under paper_2006_10142_b200/ and uses a different algorithm
- * (Thomas elimination per line with explicit a,b,c,f arrays; the GPU uses scalar-coefficient
- * scans / cyclic reduction).
+ * (Thomas elimination per line with explicit a,b,c,f arrays; the GPU solves unit-local scalar-pivot
+ * recurrences joined by carry series).
  *
  * Notation:
  *   n1 = N1-1, n2 = N2-1      unknowns per x-line / y-line; h_d = l/N_d

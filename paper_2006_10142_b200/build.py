@@ -39,8 +39,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
            "-shared", "-Xcompiler", "-fPIC", "--cudart", "static",
            "-o", tmp] + [os.path.join(_CSRC, s) for s in _SOURCES]
-    if os.environ.get("W2D_NVCC_DEFINES"):   # e.g. W2D_COPY_PROBE (bandwidth probe build, never shipped)
-        cmd[1:1] = ["-D" + d for d in os.environ["W2D_NVCC_DEFINES"].split(",")]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd), flush=True)

@@ -64,11 +64,40 @@ struct Piece {
     int safe;   // 1: touches only lines the previous sweep finished in its static part (may start before it ends)
 };
 
+// Buffer roles of sweep nh (two sweeps per solve), computed on the device from the step counter so that one
+// captured graph serves every phase of the ring (A6).
+//   ring 3 (scheme 0): reads w_{n-1} = B[n % 3], w_n = B[(n+1) % 3], writes w_{n+1} = B[(n+2) % 3].
+//   ring 4 (scheme 1): t = nh / 2 solves done: U^k = B[t % 4], V^{k-1} = B[(t+1) % 4], V^k = B[(t+2) % 4];
+//             x sweep: "prev" = V^{k-1}, "cur" = U^k, writes V^{k+1} into B[(t+3) % 4];
+//             y sweep: right-hand side V^{k+1} (as "prev" and "cur"), writes U^{k+1} over V^{k-1}.
+struct Roles {
+    int prev, cur, out;
+};
+__host__ __device__ __forceinline__ Roles roles_of(int nh, int ring)
+{
+    if (ring == 3) return Roles{nh % 3, (nh + 1) % 3, (nh + 2) % 3};
+    const int t = nh >> 1;
+    if ((nh & 1) == 0) return Roles{(t + 1) & 3, t & 3, (t + 3) & 3};
+    return Roles{(t + 3) & 3, (t + 3) & 3, (t + 1) & 3};
+}
+
+// TMA descriptors of one sweep direction, one per ring buffer (kernel parameter, __grid_constant__: the kernel
+// picks prev / cur / out by the roles of its half-step).
+struct SweepMaps {
+    CUtensorMap load[4];    // field as the sweep's load box sees it
+    CUtensorMap store[4];   // x sweep: one warp's unit [32 rows][U points]
+    CUtensorMap edge[4];    // x sweep: 16-byte neighbour boxes
+};
+
+constexpr int SLOTS = 64;   // half-steps per chunk of the step loop (work-queue / early-start counters per slot)
+
 struct SweepArgs {
     const double* table;   // device, ROW_DOUBLES per half-step (or per period, see table_period)
     int table_period;      // 0: one row per half-step; p > 0: the rows repeat with period p (constant c and g)
-    const int* d_k;        // device: completed time steps at graph start (NULL: 0)
-    int n_off;             // half-step index = n_off + 2 * (*d_k)
+    const int* d_k;        // device: completed solves at the start of the chunk
+    int n_off;             // half-step index = n_off + 2 * (*d_k); n_off < SLOTS is also the counter slot
+    int ring;              // 3 or 4 field buffers (see roles_of)
+    void* bufs[4];         // the ring (y sweep: direct stores into bufs[out])
     int n;                 // unknowns per line
     int nlines;            // number of lines
     int nbk;               // carry series length in units (<= NW, <= NBK_MAX)
@@ -77,12 +106,11 @@ struct SweepArgs {
     int npieces;           // all pieces
     int nstatic;           // pieces [0, nstatic) are dealt out statically, the rest through the ticket counter
     const int* cta_off;    // device: CTA b first works pieces [cta_off[b], cta_off[b+1])
-    int* tickets;          // device: one zeroed counter per half-step (indexed like `table`)
-    int* done;             // device: one zeroed counter per half-step: CTAs whose static share is complete and visible
+    int* tickets;          // device: one zeroed counter per slot of the chunk (indexed by n_off)
+    int* done;             // device: one zeroed counter per slot: CTAs whose static share is complete and visible
     int signal;            // 1: the next sweep has safe pieces, so this one publishes `done`
     int early;             // 1: the previous kernel in the stream is sweep nh - 1 of this handle (see "early start")
     int prev_grid;         // its grid size
-    void* out;             // y sweep: output field (direct coalesced stores)
     long long pitch;       // row pitch in elements
     const void* src;       // compact source window, [p - sp0][line - sl0] (line fastest), or NULL
     int sl0, snl, sp0, snp;
@@ -187,9 +215,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 // ---------------------------------------------------------------------------------------------------
 template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB, bool ONE = false>
 __global__ void __launch_bounds__(32 * NW, MINB)
-wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_constant__ CUtensorMap tm_cur,
-                   const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_edge,
-                   const SweepArgs a)
+wave2d_sweep_panel(const __grid_constant__ SweepMaps maps, const __grid_constant__ SweepArgs a)
 {
     using K = PanelCfg<T, DIR, UT, NW, NSTAGE, ONE>;
     constexpr int U = UT, TL = K::TL, V = K::V, SUB = K::SUB, NT = K::NT, RING = 2 * NW;
@@ -210,8 +236,13 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                                      //             which outlives the stage: s_A is rewritten one barrier earlier)
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nh = a.n_off + (a.d_k ? 2 * (*a.d_k) : 0);
+    const int nh = a.n_off + 2 * (*a.d_k);
     const double* row = a.table + static_cast<size_t>(a.table_period ? nh % a.table_period : nh) * ROW_DOUBLES;
+    const Roles R = roles_of(nh, a.ring);   // descriptor addresses are formed where they are used (three ints live, not four pointers)
+#define tm_prev (&maps.load[R.prev])
+#define tm_cur (&maps.load[R.cur])
+#define tm_out (&maps.store[R.out])
+#define tm_edge (&maps.edge[R.prev])
 
     for (int i = threadIdx.x; i < KMAX; i += K::THREADS) {
         s_cp[i] = static_cast<T>(row[ROW_CP + i]);
@@ -225,8 +256,8 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 #pragma unroll
         for (int s = 0; s < NSTAGE; ++s) mbar_init(bar32 + 8 * s, 1);
         mbar_fence_init();
-        tma_prefetch_desc(&tm_prev);
-        tma_prefetch_desc(&tm_cur);
+        tma_prefetch_desc(tm_prev);
+        tma_prefetch_desc(tm_cur);
     }
     __syncthreads();
 
@@ -238,7 +269,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     // Everything above touched only data no earlier kernel writes (the scalar table, the step counter, which
     // changes between graph launches only).  From here on the fields of the previous half-step are read.
     pdl_launch_dependents();
-    int* const ticket = a.tickets + nh;
+    int* const ticket = a.tickets + a.n_off;
     int own_next = a.cta_off[blockIdx.x];
     const int own_end = a.cta_off[blockIdx.x + 1], nstatic = a.nstatic;
     auto draw = [&]() -> int {   // thread 0: the next piece of this CTA: its own share first, then the queue
@@ -260,7 +291,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
         __shared__ int s_early_ok;
         if (try_early) {
             if (threadIdx.x == 0) {
-                const int* flag = a.done + (nh - 1);
+                const int* flag = a.done + (a.n_off - 1);
                 int ok = 0;
                 for (int spin = 0; spin < 20000 && !ok; ++spin) {
                     int v;
@@ -280,7 +311,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
     }
     const int nbk = a.nbk, n = a.n, kb = a.kb, nlines = a.nlines;
     const long long pitch = a.pitch;
-    [[maybe_unused]] T* const out_lane = reinterpret_cast<T*>(a.out) + (threadIdx.x & 31);
+    [[maybe_unused]] T* const out_lane = reinterpret_cast<T*>(a.bufs[R.out]) + (threadIdx.x & 31);
     unsigned long long t_start = 0;
     if (a.trace && threadIdx.x == 0) t_start = globaltimer_ns();
 
@@ -302,19 +333,19 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             if (warp == 0) mbar_arrive_expect_tx(full, K::STAGE_BYTES);
             if constexpr (DIR == 0) {
                 // fields: one 3D box each, [NT tiles][32 rows][128 B] = 1 KB contiguous per row in global memory
-                if (warp == 0) tma_load_3d(dst, &tm_prev, 0, line0, g0 / SUB, full);
-                if (warp == NW / 2) tma_load_3d(dst + K::FIELD_BYTES, &tm_cur, 0, line0, g0 / SUB, full);
+                if (warp == 0) tma_load_3d(dst, tm_prev, 0, line0, g0 / SUB, full);
+                if (warp == NW / 2) tma_load_3d(dst + K::FIELD_BYTES, tm_cur, 0, line0, g0 / SUB, full);
                 if (warp == NW / 4)
-                    tma_load_2d(dst + 2 * K::FIELD_BYTES, &tm_edge, g0 * U - V, line0, full);
+                    tma_load_2d(dst + 2 * K::FIELD_BYTES, tm_edge, g0 * U - V, line0, full);
                 if (warp == 3 * NW / 4)
-                    tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, &tm_edge, (g0 + NW) * U, line0, full);
+                    tma_load_2d(dst + 2 * K::FIELD_BYTES + K::EDGE_BYTES, tm_edge, (g0 + NW) * U, line0, full);
             } else {
                 constexpr int VEC = std::is_same<T, vec2f>::value ? 2 : 1;   // tensor-map columns per lane
                 if constexpr (ONE) {
-                    if (warp == 0) tma_load_2d(dst, &tm_cur, line0 * VEC, g0 * U, full);
+                    if (warp == 0) tma_load_2d(dst, tm_cur, line0 * VEC, g0 * U, full);
                 } else {
-                    if (warp == 0) tma_load_2d(dst, &tm_prev, line0 * VEC, g0 * U - 1, full);
-                    if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, &tm_cur, line0 * VEC, g0 * U - 1, full);
+                    if (warp == 0) tma_load_2d(dst, tm_prev, line0 * VEC, g0 * U - 1, full);
+                    if (warp == NW / 2) tma_load_2d(dst + K::FIELD_BYTES, tm_cur, line0 * VEC, g0 * U - 1, full);
                 }
             }
         }
@@ -398,11 +429,6 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
         if (gp < pc.ua || gp >= pc.ub) return;    // warp-uniform
         const int pp0 = gp * U;
         const bool full = pp0 + U <= n;
-#ifdef W2D_COPY_PROBE
-        if (true) {
-            v[0] += Xin;
-        } else
-#endif
         if (gp >= kb && full) {
 #pragma unroll
             for (int e = 0; e < U; ++e) v[e] = fmaT(pw_at(U - 1 - e), Xin, v[e]);
@@ -421,7 +447,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             fence_async_smem();
             __syncwarp();
             if (lane == 0) {
-                tma_store_2d(&tm_out, pp0, pc.panel * TL, smem_u32(my_out));
+                tma_store_2d(tm_out, pp0, pc.panel * TL, smem_u32(my_out));
                 tma_commit();
             }
             my_out = my_out == my_out0 ? my_out0 + 32 * K::RB : my_out0;
@@ -479,7 +505,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             if (signaled_now) {
                 if (threadIdx.x == 0) {
                     __threadfence();
-                    atomicAdd(a.done + nh, 1);
+                    atomicAdd(a.done + a.n_off, 1);
                 }
                 signaled_now = false;
             }
@@ -524,14 +550,6 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
                 // ---- RHS + local forward elimination
                 const bool fast = g >= kb && p0 + U <= n;   // stationary pivots, whole unit inside the line
                 T Aval;
-#ifdef W2D_COPY_PROBE   // bandwidth probe (not the method): same data movement and barriers, no solve
-                if (true) {
-#pragma unroll
-                    for (int e = 0; e < U; ++e) xl[e] = wp[e] + wc[e];
-                    xl[0] += wl + wr;
-                    Aval = T(0);
-                } else
-#endif
                 if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
 #pragma unroll
                     for (int e = 0; e < U; ++e) {
@@ -584,11 +602,6 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
 
                 // ---- carry from the left, local back substitution
                 const T Yin = carry(sL_lane, s_A, ring, -1, g - nbk >= kb && p0 <= n);   // y at the end of unit g-1
-#ifdef W2D_COPY_PROBE
-                if (true) {
-                    xl[0] += Yin;
-                } else
-#endif
                 if (fast) {
                     xl[U - 1] = fmaT(pw_at(U - 1), Yin, xl[U - 1]);
 #pragma unroll
@@ -620,6 +633,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             const int ringf = (pc.nst & 1) * NW + warp;
             named_bar_sync(1, NW * 32);   // the deferred warps have read the heads of stage nst-2 (same half of the ring)
             s_H[ringf * TL + lane] = T(0);
+            if (lane == 0) s_AH[ringf] = T(0);   // (a one-stage piece never wrote this half: keep 0 * AH finite)
             named_bar_sync(1, NW * 32);
             if constexpr (DEF) {
                 if (pc.nst > 0) finish(pend, gbase + (pc.nst - 1) * NW + warp, ringf ^ NW, pc);
@@ -635,7 +649,7 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
         named_bar_sync(1, NW * 32);
         if (threadIdx.x == 0) {
             __threadfence();
-            atomicAdd(a.done + nh, 1);
+            atomicAdd(a.done + a.n_off, 1);
         }
     }
     if constexpr (DIR == 0) {
@@ -651,6 +665,10 @@ wave2d_sweep_panel(const __grid_constant__ CUtensorMap tm_prev, const __grid_con
             t[3] = static_cast<unsigned long long>(q_ord);
         }
     }
+#undef tm_prev
+#undef tm_cur
+#undef tm_out
+#undef tm_edge
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -664,7 +682,7 @@ __global__ void wave2d_exact_pivots(const double* table, int period, const int* 
                                     double* ivv)
 {
     __shared__ int s_conv;
-    const int nh = n_off + (d_k ? 2 * (*d_k) : 0);
+    const int nh = n_off + 2 * (*d_k);
     const double* row = table + static_cast<size_t>(period ? nh % period : nh) * ROW_DOUBLES;
     const double ap = row[ROW_AP], beta = row[ROW_BETA];
     if (threadIdx.x == 0) {
@@ -691,15 +709,24 @@ __global__ void wave2d_exact_pivots(const double* table, int period, const int* 
     }
 }
 
+struct FieldSet {   // the ring of field buffers; roles by roles_of(nh, ring)
+    void* b[4];
+    int ring;
+};
+
 template <typename T, int DIR>
-__global__ void wave2d_exact_forward(const T* __restrict__ wprev, const T* __restrict__ wcur, T* __restrict__ out,
-                                     const double* table, int period, const int* d_k, int n_off, int n, int nlines,
-                                     long long pitch, const double* __restrict__ cpv, const double* __restrict__ ivv,
-                                     const T* __restrict__ src, int sl0, int snl, int sp0, int snp, double g2d)
+__global__ void wave2d_exact_forward(const FieldSet fs, const double* table, int period, const int* d_k, int n_off,
+                                     int n, int nlines, long long pitch, const double* __restrict__ cpv,
+                                     const double* __restrict__ ivv, const T* __restrict__ src, int sl0, int snl, int sp0,
+                                     int snp, double g2d)
 {
     const int line = blockIdx.x * blockDim.x + threadIdx.x;
     if (line >= nlines) return;
-    const int nh = n_off + (d_k ? 2 * (*d_k) : 0);
+    const int nh = n_off + 2 * (*d_k);
+    const Roles R = roles_of(nh, fs.ring);
+    const T* __restrict__ wprev = static_cast<const T*>(fs.b[R.prev]);
+    const T* __restrict__ wcur = static_cast<const T*>(fs.b[R.cur]);
+    T* __restrict__ out = static_cast<T*>(fs.b[R.out]);
     const double* row = table + static_cast<size_t>(period ? nh % period : nh) * ROW_DOUBLES;
     const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), c1 = static_cast<T>(row[ROW_C1]);
     const T g2 = static_cast<T>(g2d);
@@ -721,11 +748,12 @@ __global__ void wave2d_exact_forward(const T* __restrict__ wprev, const T* __res
 }
 
 template <typename T, int DIR>
-__global__ void wave2d_exact_backward(T* __restrict__ out, int n, int nlines, long long pitch,
+__global__ void wave2d_exact_backward(const FieldSet fs, const int* d_k, int n_off, int n, int nlines, long long pitch,
                                       const double* __restrict__ cpv)
 {
     const int line = blockIdx.x * blockDim.x + threadIdx.x;
     if (line >= nlines) return;
+    T* __restrict__ out = static_cast<T*>(fs.b[roles_of(n_off + 2 * (*d_k), fs.ring).out]);
     const long long ls = DIR == 0 ? pitch : 1, ps = DIR == 0 ? 1 : pitch;
     T* o = out + line * ls;
     T x = T(0);
@@ -765,6 +793,12 @@ __global__ void wave2d_transpose_small(T* __restrict__ dst, const T* __restrict_
     if (c < cols && r < rows) dst[static_cast<size_t>(c) * rows + r] = src[static_cast<size_t>(r) * cols + c];
 }
 
-__global__ void wave2d_bump_counter(int* d_k, int by) { *d_k += by; }
+// End of a chunk of the step loop: count its solves and zero the work-queue / early-start counters it used.
+// Launched without programmatic serialization: every sweep of the chunk has completed.
+__global__ void wave2d_end_chunk(int* d_k, int by, int* counters)
+{
+    counters[threadIdx.x] = 0;   // blockDim.x == 2 * SLOTS: tickets | done
+    if (threadIdx.x == 0) *d_k += by;
+}
 
 }  // namespace w2d

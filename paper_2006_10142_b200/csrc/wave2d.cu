@@ -109,6 +109,10 @@ EncodeTiledFn encode_tiled()
     return fn;
 }
 
+constexpr int MAX_CHUNK = SLOTS / 2;   // time steps in the longest chunk of the step loop (32)
+constexpr int NCHUNK = 6;              // chunk lengths 1, 2, 4, 8, 16, 32
+static_assert((1 << (NCHUNK - 1)) == MAX_CHUNK, "chunk lengths are the powers of two up to MAX_CHUNK");
+
 struct DirPlan {
     int solver = WAVE2D_SOLVER_STREAM;   // STREAM or EXACT after planning
     int nbk = 1, kb = 0, halo = 0, shape = 0;
@@ -126,7 +130,7 @@ struct DirPlan {
 struct wave2d_s {
     int N1, N2, n1, n2, M, dtype, elem;
     double l, tau, gamma = 2.0, kappa = 0.5;
-    int opt_solver = WAVE2D_SOLVER_AUTO, opt_graph = 1, opt_graph_steps = 12, opt_shape[2] = {0, 0};
+    int opt_solver = WAVE2D_SOLVER_AUTO, opt_graph = 1, opt_graph_steps = MAX_CHUNK, opt_shape[2] = {0, 0};
     int opt_quota[2] = {0, 0};
     cudaStream_t own_stream = nullptr, stream = nullptr;
     int num_sms = 0;
@@ -143,25 +147,26 @@ struct wave2d_s {
     std::vector<double> table;           // host copy
     int table_period = 0;                // 0: one row per half-step; 2: constant c and g, two rows serve every step
     double* d_table = nullptr;
+    size_t table_bytes = 0, pieces_bytes[2] = {0, 0}, cta_off_bytes[2] = {0, 0}, trace_bytes[2] = {0, 0};
     int* d_k = nullptr;
     double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
     bool plan_ok = false;
     DirPlan plan[2];
-    CUtensorMap tm_load[2][4], tm_store[4], tm_edge[4];   // [dir][buffer]; x: load tile, store tile, 16-byte edge box
+    SweepMaps maps[2];                   // per direction: TMA descriptors of every ring buffer
     Piece* d_pieces[2] = {nullptr, nullptr};
-    int* d_tickets = nullptr;              // one work-queue counter per half-step
+    int* d_tickets = nullptr;              // tickets[SLOTS] | done[SLOTS]: per slot of a chunk, zeroed by wave2d_end_chunk
     int* d_cta_off[2] = {nullptr, nullptr};
     double opt_static_frac = 0.75, opt_tail_div = 2.0;
     int opt_tail_min = 0, opt_tail_max = 6;   // tail_min 0: planned from the stage size
     int opt_trace = 0, opt_pdl = 1, opt_early = 1;
-    int last_sweep = -1000;               // index of the sweep launched last on the stream (early start needs n - 1)
     unsigned long long* d_trace[2] = {nullptr, nullptr};   // per-CTA trace of the last launch per direction
-    cudaGraphExec_t gexec = nullptr;
-    int gexec_steps = 0;
+    cudaGraphExec_t gexec[NCHUNK] = {};   // gexec[i]: a chunk of 2^i time steps (built with the plan)
 
     bool have_initial = false, ran = false;
     int k = 0;                           // completed steps
-    long long launches = 0;
+    long long launches = 0;              // kernels launched (graph nodes count individually)
+    long long graph_launches = 0;        // cudaGraphLaunch calls
+    long long plain_sweeps = 0;          // sweep kernels launched outside a graph
     size_t device_bytes = 0;
     std::string err;
 };
@@ -191,11 +196,19 @@ int dev_alloc(wave2d_t* h, void** p, size_t bytes)
     return WAVE2D_OK;
 }
 
+void dev_free(wave2d_t* h, void* p, size_t bytes)
+{
+    if (!p) return;
+    cudaFree(p);
+    h->device_bytes -= bytes;
+}
+
 void drop_graph(wave2d_t* h)
 {
-    if (h->gexec) cudaGraphExecDestroy(h->gexec);
-    h->gexec = nullptr;
-    h->gexec_steps = 0;
+    for (cudaGraphExec_t& g : h->gexec) {
+        if (g) cudaGraphExecDestroy(g);
+        g = nullptr;
+    }
 }
 
 void invalidate_plan(wave2d_t* h)
@@ -490,16 +503,15 @@ int plan_dir(wave2d_t* h, int d)
     return WAVE2D_OK;
 }
 
+int build_graphs(wave2d_t* h);
+
 int ensure_plan(wave2d_t* h)
 {
     if (h->plan_ok) return WAVE2D_OK;
     drop_graph(h);
     build_table(h);
-    if (h->d_table) {
-        cudaFree(h->d_table);
-        h->device_bytes -= 0;   // accounted once below
-        h->d_table = nullptr;
-    }
+    dev_free(h, h->d_table, h->table_bytes);
+    h->d_table = nullptr;
     const size_t tbytes = h->table.size() * sizeof(double);
     if (tbytes > (size_t)1 << 30) {
         h->err = "per-half-step table would exceed 1 GiB (M too large)";
@@ -507,6 +519,7 @@ int ensure_plan(wave2d_t* h)
     }
     int st = dev_alloc(h, reinterpret_cast<void**>(&h->d_table), tbytes);
     if (st) return st;
+    h->table_bytes = tbytes;
     W2D_CUDA(h, cudaMemcpyAsync(h->d_table, h->table.data(), tbytes, cudaMemcpyHostToDevice, h->stream));
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     for (int d = 0; d < 2; ++d) {
@@ -514,24 +527,25 @@ int ensure_plan(wave2d_t* h)
         if (st) return st;
     }
     mark_safe_pieces(h);
+    memset(h->maps, 0, sizeof h->maps);
     for (int b = 0; b < (h->scheme == 1 ? 4 : 3); ++b) {
         if (h->plan[0].solver == WAVE2D_SOLVER_STREAM) {
             const int U = h->plan[0].var->unit;
-            st = make_tmap_x3(h, &h->tm_load[0][b], h->buf[b], h->plan[0].var->nw / h->plan[0].var->sub);
-            if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_store[b], h->buf[b], U, 32, U * h->elem);   // one warp's unit
-            if (st == WAVE2D_OK) st = make_tmap(h, &h->tm_edge[b], h->buf[b], 16 / h->elem, 32, 0);
+            st = make_tmap_x3(h, &h->maps[0].load[b], h->buf[b], h->plan[0].var->nw / h->plan[0].var->sub);
+            if (st == WAVE2D_OK) st = make_tmap(h, &h->maps[0].store[b], h->buf[b], U, 32, U * h->elem);   // one warp's unit
+            if (st == WAVE2D_OK) st = make_tmap(h, &h->maps[0].edge[b], h->buf[b], 16 / h->elem, 32, 0);
             if (st) return st;
         }
         if (h->plan[1].solver == WAVE2D_SOLVER_STREAM) {
             const Variant& V = *h->plan[1].var;
-            st = make_tmap(h, &h->tm_load[1][b], h->buf[b], 32 * V.vec, V.unit * V.nw + (V.one ? 0 : 2), 0);
+            st = make_tmap(h, &h->maps[1].load[b], h->buf[b], 32 * V.vec, V.unit * V.nw + (V.one ? 0 : 2), 0);
             if (st) return st;
         }
     }
     for (int d = 0; d < 2; ++d) {
-        cudaFree(h->d_pieces[d]);
-        cudaFree(h->d_cta_off[d]);
-        cudaFree(h->d_trace[d]);
+        dev_free(h, h->d_pieces[d], h->pieces_bytes[d]);
+        dev_free(h, h->d_cta_off[d], h->cta_off_bytes[d]);
+        dev_free(h, h->d_trace[d], h->trace_bytes[d]);
         h->d_pieces[d] = nullptr;
         h->d_cta_off[d] = nullptr;
         h->d_trace[d] = nullptr;
@@ -539,15 +553,20 @@ int ensure_plan(wave2d_t* h)
         if (P.solver != WAVE2D_SOLVER_STREAM) continue;
         const size_t pb = std::max<size_t>(1, P.pieces.size()) * sizeof(Piece), ob = P.cta_off.size() * sizeof(int);
         st = dev_alloc(h, reinterpret_cast<void**>(&h->d_pieces[d]), pb);
-        if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_cta_off[d]), ob);
         if (st) return st;
+        h->pieces_bytes[d] = pb;
+        st = dev_alloc(h, reinterpret_cast<void**>(&h->d_cta_off[d]), ob);
+        if (st) return st;
+        h->cta_off_bytes[d] = ob;
         W2D_CUDA(h, cudaMemcpy(h->d_cta_off[d], P.cta_off.data(), ob, cudaMemcpyHostToDevice));
         if (!P.pieces.empty())
             W2D_CUDA(h, cudaMemcpy(h->d_pieces[d], P.pieces.data(), P.pieces.size() * sizeof(Piece), cudaMemcpyHostToDevice));
         if (h->opt_trace) {
-            st = dev_alloc(h, reinterpret_cast<void**>(&h->d_trace[d]), (size_t)P.grid * 16 * sizeof(unsigned long long));
+            const size_t tb = (size_t)P.grid * 16 * sizeof(unsigned long long);
+            st = dev_alloc(h, reinterpret_cast<void**>(&h->d_trace[d]), tb);
             if (st) return st;
-            W2D_CUDA(h, cudaMemset(h->d_trace[d], 0, (size_t)P.grid * 16 * sizeof(unsigned long long)));
+            h->trace_bytes[d] = tb;
+            W2D_CUDA(h, cudaMemset(h->d_trace[d], 0, tb));
         }
     }
     if ((h->plan[0].solver == WAVE2D_SOLVER_EXACT || h->plan[1].solver == WAVE2D_SOLVER_EXACT) && !h->d_piv) {
@@ -555,89 +574,81 @@ int ensure_plan(wave2d_t* h)
         if (st) return st;
     }
     h->plan_ok = true;
+    // The step loop's graphs are part of the plan: captured, instantiated and uploaded here, never inside a run call
+    // that may be timed (wave2d_run(h, 0) forces the plan).
+    if (h->opt_graph) {
+        st = build_graphs(h);
+        if (st) {
+            h->plan_ok = false;
+            return st;
+        }
+    }
     return WAVE2D_OK;
 }
 
-// Buffer roles of sweep n_abs (two sweeps per time step).
-//   scheme 0: ring of 3 (A6): reads w_{n-1} = B[n % 3], w_n = B[(n+1) % 3], writes w_{n+1} = B[(n+2) % 3].
-//   scheme 1: ring of 4, t = n_abs / 2 solves done: U^k = B[t % 4], V^{k-1} = B[(t+1) % 4], V^k = B[(t+2) % 4];
-//             x sweep: "prev" = V^{k-1}, "cur" = U^k, writes V^{k+1} into B[(t+3) % 4];
-//             y sweep: right-hand side V^{k+1} (as "prev" and "cur": 2 V - V), writes U^{k+1} over V^{k-1}.
-struct Roles {
-    int prev, cur, out;
-};
-Roles roles(const wave2d_t* h, int n_abs)
+FieldSet field_set(const wave2d_t* h)
 {
-    if (h->scheme == 0) return Roles{n_abs % 3, (n_abs + 1) % 3, (n_abs + 2) % 3};
-    const int t = n_abs >> 1;
-    if ((n_abs & 1) == 0) return Roles{(t + 1) & 3, t & 3, (t + 3) & 3};
-    return Roles{(t + 3) & 3, (t + 3) & 3, (t + 1) & 3};
+    FieldSet fs;
+    for (int b = 0; b < 4; ++b) fs.b[b] = h->buf[b];
+    fs.ring = h->scheme == 1 ? 4 : 3;
+    return fs;
 }
 
-// One half-step n -> n+1.  With use_counter the kernels read the step count from d_k (graph replay) and
-// n_off is relative to it; otherwise n_off is the absolute half-step index.
-int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
+// One half-step: sweep n_off of the current chunk (the kernels add twice the device step counter; the direction is
+// the parity of n_off, the buffer roles follow on the device).  after_own: the previous kernel on `stream` is sweep
+// n_off - 1 of this chunk, so this one may be chained to it by programmatic dependent launch (and start early).
+int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own)
 {
-    const int d = n_abs & 1;
+    const int d = n_off & 1;
     const DirPlan& P = h->plan[d];
-    const Roles R = roles(h, n_abs);
-    void* prev = h->buf[R.prev];
-    void* cur = h->buf[R.cur];
-    void* out = h->buf[R.out];
-    const int* dk = use_counter ? h->d_k : nullptr;
+    const int* dk = h->d_k;
     const void* src = h->have_src && !(h->scheme == 1 && d == 1) ? h->src_dev[d] : nullptr;   // scheme 1: f enters in x only
     const int sl0 = d == 0 ? h->win_j0 : h->win_i0, snl = d == 0 ? h->win_h : h->win_w;
     const int sp0 = d == 0 ? h->win_i0 : h->win_j0, snp = d == 0 ? h->win_w : h->win_h;
     if (P.solver == WAVE2D_SOLVER_STREAM) {
         SweepArgs a;
         a.table = h->d_table; a.table_period = h->table_period; a.d_k = dk; a.n_off = n_off;
+        a.ring = h->scheme == 1 ? 4 : 3;
+        for (int b = 0; b < 4; ++b) a.bufs[b] = h->buf[b];
         a.n = P.n; a.nlines = (P.nlines + P.var->vec - 1) / P.var->vec; a.nbk = P.nbk; a.kb = P.kb;
         a.pieces = h->d_pieces[d]; a.npieces = (int)P.pieces.size(); a.tickets = h->d_tickets;
-        a.done = h->d_tickets + 2 * h->M + 2;
-        a.early = h->opt_early && h->opt_pdl && h->last_sweep == n_abs - 1 &&
-                  h->plan[1 - d].solver == WAVE2D_SOLVER_STREAM;
+        a.done = h->d_tickets + SLOTS;
+        a.early = h->opt_early && h->opt_pdl && after_own && h->plan[1 - d].solver == WAVE2D_SOLVER_STREAM;
         a.prev_grid = h->plan[1 - d].grid;
         a.signal = h->plan[1 - d].has_safe ? 1 : 0;
         a.cta_off = h->d_cta_off[d]; a.nstatic = P.nstatic;
-        a.out = out; a.pitch = h->pitch / P.var->vec;   // in units of the kernel's T
+        a.pitch = h->pitch / P.var->vec;   // in units of the kernel's T
         a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
         a.g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
         a.trace = h->opt_trace ? h->d_trace[d] : nullptr;
-        CUtensorMap* tp = &h->tm_load[d][R.prev];
-        CUtensorMap* tc = &h->tm_load[d][R.cur];
-        CUtensorMap* to = &h->tm_store[R.out];               // x sweep: TMA store box; unused by the y sweep
-        CUtensorMap* te = &h->tm_edge[R.prev];               // x sweep: neighbours of a stage in "prev"
-        if (h->plan[0].solver != WAVE2D_SOLVER_STREAM) { to = tp; te = tp; }   // y sweep alone: placeholders
-        void* args[5] = {tp, tc, to, te, &a};
+        void* args[2] = {&h->maps[d], &a};
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(P.grid);
         cfg.blockDim = dim3(P.var->threads);
         cfg.dynamicSmemBytes = P.var->smem;
-        cfg.stream = h->stream;
+        cfg.stream = stream;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // overlap our prologue with the previous
         at[0].val.programmaticStreamSerializationAllowed = 1;            // kernel's tail (griddepcontrol.wait inside)
         cfg.attrs = at;
-        // Only behind a sweep of our own: a kernel that follows something else (the step-counter kernel at the start
-        // of a graph replay, a copy) reads the step counter before griddepcontrol.wait and must see it final.
-        cfg.numAttrs = h->opt_pdl && h->last_sweep == n_abs - 1 ? 1 : 0;
+        // Only behind a sweep of the same chunk: the first sweep of a chunk follows wave2d_end_chunk (or a copy) and
+        // reads the step counter before griddepcontrol.wait, so it must see it final.
+        cfg.numAttrs = h->opt_pdl && after_own ? 1 : 0;
         W2D_CUDA(h, cudaLaunchKernelExC(&cfg, P.var->fn, args));
-        h->last_sweep = n_abs;
-        h->launches += 1;
         return WAVE2D_OK;
     }
     // exact two-pass Thomas
     double* cpv = h->d_piv;
     double* ivv = h->d_piv + std::max(h->n1, h->n2);
-    wave2d_exact_pivots<<<1, 256, 0, h->stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv);
+    const FieldSet fs = field_set(h);
+    wave2d_exact_pivots<<<1, 256, 0, stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv);
     const int tb = 128, gb = (P.nlines + tb - 1) / tb;
     const double g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
 #define W2D_EXACT(T, D)                                                                                               \
     do {                                                                                                              \
-        wave2d_exact_forward<T, D><<<gb, tb, 0, h->stream>>>((const T*)prev, (const T*)cur, (T*)out, h->d_table,      \
-                                                             h->table_period, dk, n_off, P.n, P.nlines, h->pitch, cpv, ivv, (const T*)src, \
-                                                             sl0, snl, sp0, snp, g2);                                 \
-        wave2d_exact_backward<T, D><<<gb, tb, 0, h->stream>>>((T*)out, P.n, P.nlines, h->pitch, cpv);                 \
+        wave2d_exact_forward<T, D><<<gb, tb, 0, stream>>>(fs, h->d_table, h->table_period, dk, n_off, P.n, P.nlines,  \
+                                                          h->pitch, cpv, ivv, (const T*)src, sl0, snl, sp0, snp, g2); \
+        wave2d_exact_backward<T, D><<<gb, tb, 0, stream>>>(fs, dk, n_off, P.n, P.nlines, h->pitch, cpv);              \
     } while (0)
     if (h->dtype == WAVE2D_F64) {
         if (d == 0) W2D_EXACT(double, 0); else W2D_EXACT(double, 1);
@@ -646,53 +657,65 @@ int launch_half_step(wave2d_t* h, int n_abs, int n_off, bool use_counter)
     }
 #undef W2D_EXACT
     W2D_CUDA(h, cudaGetLastError());
-    h->last_sweep = -1000;
-    h->launches += 3;
     return WAVE2D_OK;
 }
 
-int build_graph(wave2d_t* h, int steps)
+int kernels_per_sweep(const wave2d_t* h, int d) { return h->plan[d].solver == WAVE2D_SOLVER_STREAM ? 1 : 3; }
+
+// A chunk of the step loop (A7): `steps` time steps = sweeps n_off = 0 .. 2 steps - 1 relative to the device step
+// counter, then wave2d_end_chunk, which counts them and re-zeroes the counters they used.  The same sequence is
+// either captured into a graph (once, with the plan) or launched directly (option graph = 0).
+int launch_chunk(wave2d_t* h, cudaStream_t stream, int steps)
 {
-    drop_graph(h);
-    cudaGraph_t g = nullptr;
-    W2D_CUDA(h, cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
-    const long long l0 = h->launches;
-    h->last_sweep = -1000;   // the first sweep of a replay follows the counter kernel, not a sweep
     int st = WAVE2D_OK;
     for (int s = 0; s < steps && st == WAVE2D_OK; ++s) {
-        st = launch_half_step(h, 2 * s, 2 * s, true);
-        if (st == WAVE2D_OK) st = launch_half_step(h, 2 * s + 1, 2 * s + 1, true);
+        st = launch_half_step(h, stream, 2 * s, s > 0 && kernels_per_sweep(h, 1) == 1);
+        if (st == WAVE2D_OK) st = launch_half_step(h, stream, 2 * s + 1, kernels_per_sweep(h, 0) == 1);
     }
-    if (st == WAVE2D_OK) wave2d_bump_counter<<<1, 1, 0, h->stream>>>(h->d_k, steps);
-    h->launches = l0;   // capture is not execution
-    h->last_sweep = -1000;
-    cudaError_t e = cudaStreamEndCapture(h->stream, &g);
-    if (st != WAVE2D_OK) {
-        if (g) cudaGraphDestroy(g);
-        return st;
-    }
-    if (e != cudaSuccess) {
-        h->err = std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e);
-        (void)cudaGetLastError();
-        return WAVE2D_ERR_CUDA;
-    }
-    e = cudaGraphInstantiate(&h->gexec, g, 0);
-    cudaGraphDestroy(g);
-    if (e != cudaSuccess) {
-        h->gexec = nullptr;
-        h->err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e);
-        (void)cudaGetLastError();
-        return WAVE2D_ERR_CUDA;
-    }
-    h->gexec_steps = steps;
+    if (st) return st;
+    wave2d_end_chunk<<<1, 2 * SLOTS, 0, stream>>>(h->d_k, steps, h->d_tickets);
+    W2D_CUDA(h, cudaGetLastError());
     return WAVE2D_OK;
 }
 
-long long launches_per_step(const wave2d_t* h)
+long long kernels_per_chunk(const wave2d_t* h, int steps)
 {
-    long long n = 0;
-    for (int d = 0; d < 2; ++d) n += h->plan[d].solver == WAVE2D_SOLVER_STREAM ? 1 : 3;
-    return n;
+    return (long long)steps * (kernels_per_sweep(h, 0) + kernels_per_sweep(h, 1)) + 1;
+}
+
+// Graphs of 1, 2, 4, ... opt_graph_steps time steps: any step count is a short sequence of replays, at any phase of
+// the buffer ring (the kernels derive the roles from the device step counter), with no plain launch left over.
+// Captured on the handle's own stream (capture needs a non-legacy stream; the executables launch into any stream).
+int build_graphs(wave2d_t* h)
+{
+    drop_graph(h);
+    for (int i = 0; i < NCHUNK && (1 << i) <= h->opt_graph_steps; ++i) {
+        cudaGraph_t g = nullptr;
+        W2D_CUDA(h, cudaStreamBeginCapture(h->own_stream, cudaStreamCaptureModeThreadLocal));
+        const int st = launch_chunk(h, h->own_stream, 1 << i);
+        const cudaError_t e = cudaStreamEndCapture(h->own_stream, &g);
+        if (st != WAVE2D_OK) {
+            if (g) cudaGraphDestroy(g);
+            (void)cudaGetLastError();
+            return st;
+        }
+        if (e != cudaSuccess) {
+            h->err = std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e);
+            (void)cudaGetLastError();
+            return WAVE2D_ERR_CUDA;
+        }
+        const cudaError_t ei = cudaGraphInstantiate(&h->gexec[i], g, 0);
+        cudaGraphDestroy(g);
+        if (ei != cudaSuccess) {
+            h->gexec[i] = nullptr;
+            h->err = std::string("cudaGraphInstantiate: ") + cudaGetErrorString(ei);
+            (void)cudaGetLastError();
+            return WAVE2D_ERR_CUDA;
+        }
+        W2D_CUDA(h, cudaGraphUpload(h->gexec[i], h->own_stream));   // first replay pays no upload
+    }
+    W2D_CUDA(h, cudaStreamSynchronize(h->own_stream));
+    return WAVE2D_OK;
 }
 
 int copy_in(wave2d_t* h, void* dst, const void* src, long ld)
@@ -712,9 +735,6 @@ int copy_out(wave2d_t* h, void* dst, long ld, const void* src)
     return WAVE2D_OK;
 }
 
-// solves done so far: the device step counter and the table / ring index are counted in these
-int solves_done(const wave2d_t* h) { return h->scheme == 1 ? h->k - 1 : h->k; }
-int ring_period(const wave2d_t* h) { return h->scheme == 1 ? 4 : 3; }
 
 // Scheme 1 start, (2.9) as printed: U^0 = phi -> buf[3], U^1 = phi + tau psi -> buf[0]; the state
 // is time level k = 1.  V^0, V^1 follow at the first run (they need the final speed samples).
@@ -735,10 +755,9 @@ int set_initial_factored(wave2d_t* h, const void* phi, const void* psi, long ld)
                                                             h->pitch, -h->tau);
     W2D_CUDA(h, cudaGetLastError());
     W2D_CUDA(h, cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream));
-    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)4 * h->M + 4) * sizeof(int), h->stream));
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, (size_t)2 * SLOTS * sizeof(int), h->stream));
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_initial = true;
-    h->last_sweep = -1000;
     h->v_ready = false;
     h->k = 1;
     h->ran = false;
@@ -800,7 +819,7 @@ int wave2d_create(wave2d_t** out, int N1, int N2, double l, double tau, int M, i
     int st = WAVE2D_OK;
     for (int b = 0; b < 3 && st == WAVE2D_OK; ++b) st = dev_alloc(h, &h->buf[b], fbytes);
     if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_k), sizeof(int));
-    const size_t tk_bytes = ((size_t)4 * M + 4) * sizeof(int);   // tickets[2M+2] | done[2M+2]
+    const size_t tk_bytes = (size_t)2 * SLOTS * sizeof(int);   // tickets[SLOTS] | done[SLOTS]
     if (st == WAVE2D_OK) st = dev_alloc(h, reinterpret_cast<void**>(&h->d_tickets), tk_bytes);
     if (st == WAVE2D_OK) {
         for (int b = 0; b < 3; ++b) cudaMemsetAsync(h->buf[b], 0, fbytes, h->stream);
@@ -845,9 +864,7 @@ int wave2d_set_stream(wave2d_t* h, void* cuda_stream)
     if (!h) return WAVE2D_ERR_ARG;
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->stream = cuda_stream ? static_cast<cudaStream_t>(cuda_stream) : h->own_stream;
-    h->last_sweep = -1000;
-    drop_graph(h);
-    return WAVE2D_OK;
+    return WAVE2D_OK;   // the graphs of the plan launch into any stream
 }
 
 int wave2d_set_option(wave2d_t* h, const char* name, double value)
@@ -869,7 +886,10 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     }
     else if (!strcmp(name, "solver")) { if (iv < 0 || iv > 2) return WAVE2D_ERR_ARG; h->opt_solver = iv; }
     else if (!strcmp(name, "graph")) h->opt_graph = iv != 0;
-    else if (!strcmp(name, "graph_steps")) { if (iv < 3 || iv % 3) return WAVE2D_ERR_ARG; h->opt_graph_steps = iv; }
+    else if (!strcmp(name, "graph_steps")) {
+        if (iv < 1 || iv > MAX_CHUNK || (iv & (iv - 1))) return WAVE2D_ERR_ARG;   // 1, 2, 4, ..., MAX_CHUNK
+        h->opt_graph_steps = iv;
+    }
     else if (!strcmp(name, "shape_x")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[0] = iv; }
     else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
     else if (!strcmp(name, "trace")) h->opt_trace = iv != 0;
@@ -908,10 +928,9 @@ int wave2d_set_initial(wave2d_t* h, const void* phi, const void* psi, long ld)
                                                             h->pitch, 0.5 * h->tau);
     W2D_CUDA(h, cudaGetLastError());
     W2D_CUDA(h, cudaMemsetAsync(h->d_k, 0, sizeof(int), h->stream));
-    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)4 * h->M + 4) * sizeof(int), h->stream));   // work queues
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, (size_t)2 * SLOTS * sizeof(int), h->stream));   // work queues
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_initial = true;
-    h->last_sweep = -1000;
     h->k = 0;
     h->ran = false;
     return WAVE2D_OK;
@@ -925,10 +944,10 @@ int wave2d_set_state(wave2d_t* h, int k, const void* u_prev_half, const void* u,
     int st = copy_in(h, h->buf[(2 * k) % 3], u_prev_half, ld);
     if (st == WAVE2D_OK) st = copy_in(h, h->buf[(2 * k + 1) % 3], u, ld);
     if (st) return st;
-    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, ((size_t)4 * h->M + 4) * sizeof(int), h->stream));
+    W2D_CUDA(h, cudaMemsetAsync(h->d_tickets, 0, (size_t)2 * SLOTS * sizeof(int), h->stream));
+    W2D_CUDA(h, cudaMemcpyAsync(h->d_k, &k, sizeof(int), cudaMemcpyHostToDevice, h->stream));   // synchronised below
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_initial = true;
-    h->last_sweep = -1000;
     h->k = k;
     return WAVE2D_OK;
 }
@@ -998,43 +1017,31 @@ int wave2d_run(wave2d_t* h, int steps)
     if (!h || steps < 0) return WAVE2D_ERR_ARG;
     if (!h->have_initial) return WAVE2D_ERR_STATE;
     if ((long long)h->k + steps > h->M) return WAVE2D_ERR_RANGE;
-    int st = ensure_plan(h);
+    int st = ensure_plan(h);   // also builds the graphs: wave2d_run(h, 0) prepares everything
     if (st) return st;
     if (steps > 0) h->ran = true;
     if (steps > 0 && h->scheme == 1 && !h->v_ready) {
         st = init_factored_v(h);
         if (st) return st;
     }
-    const int period = ring_period(h);
-    const bool can_graph = h->opt_graph && h->stream != nullptr && h->stream != cudaStreamLegacy &&
-                           h->stream != cudaStreamPerThread;
+    // Algorithm 1's loop in chunks of 2^i steps, longest first; each chunk is one graph replay
+    // (or, with graph = 0, the same kernel sequence launched directly).
     int left = steps;
-    bool counter_set = false;
     while (left > 0) {
-        const int gs = h->opt_graph_steps;
-        const int t = solves_done(h);
-        if (can_graph && t % period == 0 && gs % period == 0 && left >= gs) {
-            if (!h->gexec || h->gexec_steps != gs) {
-                st = build_graph(h, gs);
-                if (st) return st;
-            }
-            if (!counter_set) {
-                W2D_CUDA(h, cudaMemcpyAsync(h->d_k, &t, sizeof(int), cudaMemcpyHostToDevice, h->stream));
-                counter_set = true;
-            }
-            W2D_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
-            h->last_sweep = -1000;
-            h->launches += launches_per_step(h) * gs + 1;
-            h->k += gs;
-            left -= gs;
+        int i = 0;
+        while (i + 1 < NCHUNK && (2 << i) <= left && (2 << i) <= h->opt_graph_steps) ++i;
+        const int cs = 1 << i;
+        if (h->opt_graph) {
+            W2D_CUDA(h, cudaGraphLaunch(h->gexec[i], h->stream));
+            h->graph_launches += 1;
         } else {
-            st = launch_half_step(h, 2 * t, 2 * t, false);
-            if (st == WAVE2D_OK) st = launch_half_step(h, 2 * t + 1, 2 * t + 1, false);
+            st = launch_chunk(h, h->stream, cs);
             if (st) return st;
-            h->k += 1;
-            left -= 1;
-            counter_set = false;
+            h->plain_sweeps += 2 * cs;
         }
+        h->launches += kernels_per_chunk(h, cs);
+        h->k += cs;
+        left -= cs;
     }
     return WAVE2D_OK;
 }
@@ -1076,6 +1083,8 @@ int wave2d_get_info(wave2d_t* h, const char* name, double* value)
     if (!strcmp(name, "pitch")) { *value = (double)h->pitch; return WAVE2D_OK; }
     if (!strcmp(name, "device_bytes")) { *value = (double)h->device_bytes; return WAVE2D_OK; }
     if (!strcmp(name, "launches")) { *value = (double)h->launches; return WAVE2D_OK; }
+    if (!strcmp(name, "graph_launches")) { *value = (double)h->graph_launches; return WAVE2D_OK; }
+    if (!strcmp(name, "plain_sweeps")) { *value = (double)h->plain_sweeps; return WAVE2D_OK; }
     if (!strcmp(name, "source_window")) { *value = h->have_src ? (double)h->win_w * h->win_h : 0.0; return WAVE2D_OK; }
     int st = ensure_plan(h);
     if (st) return st;
@@ -1097,6 +1106,12 @@ int wave2d_get_info(wave2d_t* h, const char* name, double* value)
     else if (key == "unit") *value = stream ? P.var->unit : 0;
     else if (key == "upc") *value = stream ? P.quota * P.var->nw : 0;
     else if (key == "quota") *value = stream ? P.quota : 0;
+    else if (key == "static") *value = stream ? P.nstatic : 0;
+    else if (key == "safe") {
+        int c = 0;
+        for (const Piece& pc : P.pieces) c += pc.safe != 0;
+        *value = c;
+    }
     else return WAVE2D_ERR_ARG;
     return WAVE2D_OK;
 }
@@ -1109,17 +1124,24 @@ int wave2d_profile_sweeps(wave2d_t* h, int steps, double* ms_x, double* ms_y)
     int st = ensure_plan(h);
     if (st) return st;
     h->ran = true;
+    if (h->scheme == 1 && !h->v_ready) {
+        st = init_factored_v(h);
+        if (st) return st;
+    }
     std::vector<cudaEvent_t> ev((size_t)3 * steps);
     for (auto& e : ev) W2D_CUDA(h, cudaEventCreate(&e));
-    for (int s = 0; s < steps; ++s) {
+    for (int s = 0; s < steps; ++s) {   // chunks of one step, an event around each sweep
         W2D_CUDA(h, cudaEventRecord(ev[3 * s], h->stream));
-        const int t = solves_done(h);
-        st = launch_half_step(h, 2 * t, 2 * t, false);
+        st = launch_half_step(h, h->stream, 0, false);
         if (st) return st;
         W2D_CUDA(h, cudaEventRecord(ev[3 * s + 1], h->stream));
-        st = launch_half_step(h, 2 * t + 1, 2 * t + 1, false);
+        st = launch_half_step(h, h->stream, 1, kernels_per_sweep(h, 0) == 1);
         if (st) return st;
         W2D_CUDA(h, cudaEventRecord(ev[3 * s + 2], h->stream));
+        wave2d_end_chunk<<<1, 2 * SLOTS, 0, h->stream>>>(h->d_k, 1, h->d_tickets);
+        W2D_CUDA(h, cudaGetLastError());
+        h->launches += kernels_per_chunk(h, 1);
+        h->plain_sweeps += 2;
         h->k += 1;
     }
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));

@@ -10,7 +10,6 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on the B200 box)")
-    config.addinivalue_line("markers", "slow: full-size oracle comparison, opt-in via WAVE2D_FULL_PARITY=1")
 
 
 @pytest.fixture(scope="session", autouse=True)

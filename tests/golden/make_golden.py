@@ -6,13 +6,9 @@ cfg1_modal.txt : config 1 of BASELINE.json (N1=N2=128, tau=h/2, M=100, c=1, phi 
                  amplitude of the (1,1) mode of u^M, obtained by projecting the oracle's full 2D result
                  onto the mode.  Checked in tests/test_oracle_pins.py against the independent scalar modal
                  recurrence (SURVEY.md 8c pin 3) and the PDE closed form of north_star.
-oracle_checksums.txt : max|u| and a few sampled values of the oracle on small scaled copies of the five
-                 workloads -- detects silent drift of the oracle's arithmetic.
 """
 import os
 import sys
-
-import numpy as np
 
 ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 sys.path.insert(0, ROOT)
@@ -28,15 +24,6 @@ def run(w, steps=None):
                         steps=steps)
 
 
-def small_cases():
-    return [("cfg1", W.cfg1()), ("cfg2_N96_M40", W.cfg2(N=96, M=40)), ("cfg3_N128_M60", W.cfg3(N=128, M=60)),
-            ("cfg4_N160x40_M30", W.cfg4(N1=160, N2=40, M=30)), ("cfg5_N192_M20", W.cfg5(N=192, M=20))]
-
-
-def sample_points(w):
-    return [(w.n2 // 2, w.n1 // 2), (w.n2 // 3, (2 * w.n1) // 3), (0, 0), (w.n2 - 1, w.n1 - 2)]
-
-
 def main():
     w = W.cfg1()
     u = run(w)
@@ -45,12 +32,6 @@ def main():
         f.write("# config 1 (BASELINE.json configs[0]): (1,1)-mode amplitude of u^100, oracle 2D run projected on the mode\n")
         f.write("# written by tests/golden/make_golden.py (calls oracle/ only)\n")
         f.write(f"{amp:.17e}\n")
-    with open(os.path.join(HERE, "oracle_checksums.txt"), "w") as f:
-        f.write("# name  max|u|  u[samples...]   written by tests/golden/make_golden.py (calls oracle/ only)\n")
-        for name, w in small_cases():
-            u = run(w)
-            vals = " ".join(f"{u[j, i]:.17e}" for j, i in sample_points(w))
-            f.write(f"{name} {np.abs(u).max():.17e} {vals}\n")
     print("cfg1 amplitude", amp)
 
 

@@ -165,6 +165,62 @@ def test_run_in_pieces_equals_one_run_and_reset_is_reproducible():
     o.close()
 
 
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_every_run_call_replays_graphs_at_any_ring_phase(scheme):
+    """A7: the graphs are built with the plan, the kernels take the buffer roles from the device step counter, so
+    run(5); run(20) (the driver's bench pattern: warm-up 5, then 20 timed steps at ring phase 5 mod 3) issues graph
+    replays only -- no sweep kernel outside a graph, no capture inside a run call -- and is bit-identical to run(25)
+    and to plain launches (graph = 0)."""
+    w = W.cfg2(N=700, M=60)
+    src = W.cfg3(N=700, M=60)
+    w.s, w.g_half = src.s, W.ricker(W.half_times(w.tau, 2 * w.M) + 0.058)
+
+    def handle(**opts):
+        h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, "f64")
+        if scheme:
+            h.set_option("scheme", 1)
+        for k, v in opts.items():
+            h.set_option(k, v)
+        h.set_speed(w.c_half)
+        h.set_source(w.s, w.g_half)
+        h.set_initial(w.phi)
+        return h
+
+    h = handle()
+    try:
+        h.run(0)                                     # plans, captures, instantiates, uploads
+        assert h.info("launches") == 0 and h.info("graph_launches") == 0
+        h.run(5)                                     # 4 + 1
+        assert h.info("graph_launches") == 2
+        h.run(20)                                    # 16 + 4
+        assert h.info("graph_launches") == 4 and h.info("plain_sweeps") == 0
+        assert h.info("launches") == 2 * 25 + 4 + (2 if scheme else 0)   # two sweeps per step, one counter kernel per chunk
+                                                                          # (scheme 1: + the two start kernels)
+        a = h.get()
+        for part in (1, 1, 1, 2, 3, 7, 13):          # every phase of the ring, every chunk length below 16
+            h.run(part)
+        assert h.info("plain_sweeps") == 0
+        a2 = h.get()
+    finally:
+        h.close()
+    K2 = 25 + 28
+    for opts, K, want in (({}, 25, a), ({"graph": 0}, 25, a), ({"graph_steps": 4}, 25, a), ({}, K2, a2),
+                          ({"graph": 0, "pdl": 0}, K2, a2)):
+        h = handle(**opts)
+        try:
+            h.run(K)                                 # K solves in one call
+            u = h.get()
+            if opts.get("graph") == 0:
+                assert h.info("graph_launches") == 0 and h.info("plain_sweeps") > 0
+        finally:
+            h.close()
+        assert np.array_equal(u, want), (opts, K)
+    if scheme == 0:
+        assert relerr(a2, ref(w, steps=K2)) <= 1e-10
+    else:
+        assert relerr(a2, ref1(w, K=K2 + 1)) <= 1e-10          # set_initial stands at level 1: K2 solves reach K2 + 1
+
+
 def test_device_pointers_strided_inputs_and_user_stream():
     import torch
     w = W.cfg4(N1=200, N2=120, M=15)
@@ -550,6 +606,29 @@ def test_tiny_and_ragged_sizes_fp32_and_scheme1(N1, N2, dtype, scheme):
         assert relerr(u, r) <= tol, (opts, relerr(u, r))
 
 
+def test_early_start_engages_and_changes_no_bit():
+    """At 3000^2 both sweeps deal out a static share AND draw a tail, so the planner marks safe pieces (at
+    2048^2 and below it marks none and the early-start protocol was never exercised bitwise).  Early start on / off
+    and programmatic launch on / off must agree bit for bit, repeatedly, for both schemes."""
+    w = W.cfg2(N=3000, M=14)
+    src = W.cfg3(N=3000, M=14)
+    w.s, w.g_half = src.s, W.ricker(W.half_times(w.tau, 2 * w.M) + 0.058)
+    base, info = gpu_info(w, ("safe_x", "safe_y", "static_x", "static_y", "chunks_x", "chunks_y"), early=0, pdl=0)
+    assert relerr(base, ref(w)) <= 1e-10
+    _, info = gpu_info(w, ("safe_x", "safe_y", "static_x", "static_y"), early=1)
+    assert info["safe_x"] > 0 and info["safe_y"] > 0, info
+    assert info["static_x"] < info["chunks_x"] and info["static_y"] < info["chunks_y"]   # a drawn tail exists
+    for opts in ({"early": 1}, {"early": 0}, {"early": 1, "graph": 0}, {"early": 1}, {"early": 1, "graph_steps": 2},
+                 {"early": 1}):
+        u, _ = gpu(w, **opts)
+        assert np.array_equal(u, base), opts
+    base1, _ = gpu1(w, early=0, pdl=0)
+    assert relerr(base1, ref1(w)) <= 1e-10
+    for opts in ({"early": 1}, {"early": 1, "graph": 0}, {"early": 1}):
+        u, _ = gpu1(w, **opts)
+        assert np.array_equal(u, base1), opts
+
+
 def test_early_start_and_pdl_do_not_change_a_single_bit():
     """Early start only changes WHEN a piece runs (and the order of a CTA's share), programmatic launch only how
     kernels are chained: with both off, one off, both on, three runs each way must agree bit for bit on a grid with
@@ -584,12 +663,13 @@ def test_two_handles_on_two_streams_run_concurrently():
     """Two independent simulations, each with persistent one-CTA-per-SM kernels, early start and its own graph, queued
     on two streams at once: no deadlock, and each result equals its solo run bit for bit."""
     import torch
-    wa = W.cfg2(N=1500, M=36)
+    wa = W.cfg2(N=2700, M=36)                   # static share + drawn tail: early start engaged (safe pieces > 0)
     wb = W.cfg4(N1=1800, N2=900, M=36)
-    solo_a, _ = gpu(wa)
+    solo_a, ia = gpu_info(wa, ("safe_x", "safe_y"))
     solo_b, _ = gpu(wb)
+    assert ia["safe_x"] > 0 and ia["safe_y"] > 0
     sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
-    for it in range(60):   # sharing the SMs shifts every timing inside a CTA: this loop exposed a shared-memory race
+    for it in range(40):   # sharing the SMs shifts every timing inside a CTA: this loop exposed a shared-memory race
         ha, hb = B.from_workload(wa), B.from_workload(wb)   # (7 % of iterations) that no single-handle run ever showed
         try:
             ha.set_stream(sa)
