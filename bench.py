@@ -397,7 +397,9 @@ def run_ours(args):
                 "steps_per_call": Ke, "seconds_per_call": e2e_s,
                 "what": "wave2d_set_initial(pinned host phi) + wave2d_run(steps_per_call) + wave2d_get(pinned host u), "
                         "wall clock incl. both copies; bytes are per call / steps_per_call"},
-        "roofline": {"bound": "hbm", "kernel": f"wave2d_sweep_panel<{w.dtype}, dir={dom}>", "achieved": achieved,
+        "roofline": {"bound": "hbm", "kernel": (f"wave2d_sweep_panel<{w.dtype}, dir={dom}>" if geom["solver_x"] != 3 else
+                                                f"wave2d_line_steps<{w.dtype}> (both half-steps of every step in one "
+                                                "launch; each sweep is given half of it)"), "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                      "peak_source": peak_src, "bytes_per_launch": sweep_bytes,
                      "ms_per_launch": ms_dom, "share_of_step": share_dom,

@@ -58,9 +58,14 @@ enum {
 
 /* Solver selection for wave2d_set_option(h, "solver", v). */
 enum {
-    WAVE2D_SOLVER_AUTO = 0,     /* streamed kernels where the decay bound rho^H <= tol allows, else EXACT */
+    WAVE2D_SOLVER_AUTO = 0,     /* LINE on small grids; else streamed kernels where the decay bound
+                                 * rho^H <= tol allows, else EXACT                                        */
     WAVE2D_SOLVER_EXACT = 1,    /* untruncated two-pass elimination through HBM (any tau/h)              */
-    WAVE2D_SOLVER_STREAM = 2    /* force the streamed kernels; ERR_UNSUPPORTED if the bound fails        */
+    WAVE2D_SOLVER_STREAM = 2,   /* force the streamed kernels; ERR_UNSUPPORTED if the bound fails        */
+    WAVE2D_SOLVER_LINE = 3      /* small grids (at most 256 unknowns per line in both directions): the whole step
+                                 * loop in one launch of one thread-block cluster, every line solved whole and
+                                 * exactly on chip by a warp-shuffle scan (any tau/h); AUTO picks it when the grid
+                                 * fits; forcing it on a larger grid gives ERR_UNSUPPORTED                        */
 };
 
 /*
@@ -167,7 +172,7 @@ int wave2d_sync(wave2d_t *h);
 
 /*
  * Introspection for benchmarks and tests.  name:
- *   "solver_x", "solver_y"   solver path in use per direction (WAVE2D_SOLVER_EXACT / _STREAM), after planning
+ *   "solver_x", "solver_y"   solver path in use per direction (WAVE2D_SOLVER_EXACT / _STREAM / _LINE), after planning
  *   "halo_x", "halo_y"       look-ahead H (points) with rho^H <= 1e-17 (fp64) / 1e-8 (fp32)
  *   "rho_x", "rho_y"         largest decay ratio rho over all half-steps
  *   "nbk_*"                  carry series length in units (halo = nbk * unit)

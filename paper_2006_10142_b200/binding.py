@@ -15,7 +15,7 @@ _LIBNAME = "libwave2d.so"
 _lib = None
 
 F64, F32 = 0, 1
-SOLVER_AUTO, SOLVER_EXACT, SOLVER_STREAM = 0, 1, 2
+SOLVER_AUTO, SOLVER_EXACT, SOLVER_STREAM, SOLVER_LINE = 0, 1, 2, 3
 
 EXPORTS = [
     "wave2d_create", "wave2d_destroy", "wave2d_set_stream", "wave2d_set_option", "wave2d_set_initial",

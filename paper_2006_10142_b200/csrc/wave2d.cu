@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "line.cuh"
 
 using namespace w2d;
 
@@ -152,6 +153,9 @@ struct wave2d_s {
     double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
     bool plan_ok = false;
     DirPlan plan[2];
+    bool line_mode = false;              // small grid: the step loop runs in wave2d_line_steps (line.cuh)
+    const void* line_fn = nullptr;
+    int line_unit = 0, line_ctas = 0, line_smem = 0;
     SweepMaps maps[2];                   // per direction: TMA descriptors of every ring buffer
     Piece* d_pieces[2] = {nullptr, nullptr};
     int* d_tickets = nullptr;              // tickets[SLOTS] | done[SLOTS]: per slot of a chunk, zeroed by wave2d_end_chunk
@@ -167,6 +171,7 @@ struct wave2d_s {
     long long launches = 0;              // kernels launched (graph nodes count individually)
     long long graph_launches = 0;        // cudaGraphLaunch calls
     long long plain_sweeps = 0;          // sweep kernels launched outside a graph
+    long long line_launches = 0;         // launches of the small-grid step kernel
     size_t device_bytes = 0;
     std::string err;
 };
@@ -505,6 +510,76 @@ int plan_dir(wave2d_t* h, int d)
 
 int build_graphs(wave2d_t* h);
 
+// ---- small grids: one cluster, one launch for the whole step loop (line.cuh) --------------------------------
+constexpr int LINE_WARPS = 16;   // warps per CTA of the small-grid kernel
+
+template <typename T, int U>
+const void* line_kernel() { return reinterpret_cast<const void*>(&wave2d_line_steps<T, U, LINE_WARPS>); }
+
+int plan_line(wave2d_t* h)
+{
+    h->line_mode = false;
+    const int nmax = std::max(h->n1, h->n2);
+    const bool fits = nmax <= 32 * 8;
+    if (h->opt_solver == WAVE2D_SOLVER_LINE && !fits) {
+        h->err = "solver LINE: more than 256 unknowns per line";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    if (!fits || (h->opt_solver != WAVE2D_SOLVER_AUTO && h->opt_solver != WAVE2D_SOLVER_LINE)) return WAVE2D_OK;
+    const int U = nmax <= 32 * 4 ? 4 : 8;
+    h->line_unit = U;
+    if (h->dtype == WAVE2D_F64) h->line_fn = U == 4 ? line_kernel<double, 4>() : line_kernel<double, 8>();
+    else h->line_fn = U == 4 ? line_kernel<float, 4>() : line_kernel<float, 8>();
+    h->line_smem = 2 * 16 * (32 * U + 1) * h->elem;
+    W2D_CUDA(h, cudaFuncSetAttribute(h->line_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->line_smem));
+    // one CTA per 16 rows of the x half-step / per 16-column strip of the y half-step, at most one portable cluster
+    const int want = std::max((h->n2 + LINE_WARPS - 1) / LINE_WARPS, (h->n1 + 15) / 16);
+    h->line_ctas = std::max(1, std::min(8, want));
+    for (int d = 0; d < 2; ++d) {
+        DirPlan& P = h->plan[d];
+        P = DirPlan();
+        P.solver = WAVE2D_SOLVER_LINE;
+        P.n = d == 0 ? h->n1 : h->n2;
+        P.nlines = d == 0 ? h->n2 : h->n1;
+        P.grid = h->line_ctas;
+        for (int n = d; n < (h->table_period ? h->table_period : 2 * h->M); n += 2)
+            P.rho = std::max(P.rho, h->table[static_cast<size_t>(n) * ROW_DOUBLES + ROW_RHO]);
+    }
+    h->line_mode = true;
+    return WAVE2D_OK;
+}
+
+// All `steps` time steps in one launch (the kernel advances the device step counter itself).
+int launch_line_steps(wave2d_t* h, int steps)
+{
+    LineArgs a;
+    a.table = h->d_table; a.table_period = h->table_period; a.d_k = h->d_k; a.nsteps = steps;
+    a.ring = h->scheme == 1 ? 4 : 3; a.one_y = h->scheme == 1 ? 1 : 0;
+    for (int b = 0; b < 4; ++b) a.bufs[b] = h->buf[b];
+    a.n1 = h->n1; a.n2 = h->n2; a.pitch = h->pitch;
+    a.src[0] = h->have_src ? h->src_dev[0] : nullptr;
+    a.src[1] = h->have_src && h->scheme == 0 ? h->src_dev[1] : nullptr;   // scheme 1: f enters in x only
+    a.win_i0 = h->win_i0; a.win_j0 = h->win_j0; a.win_w = h->win_w; a.win_h = h->win_h;
+    a.g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
+    void* args[1] = {&a};
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(h->line_ctas);
+    cfg.blockDim = dim3(32 * LINE_WARPS);
+    cfg.dynamicSmemBytes = h->line_smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = h->line_ctas;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    W2D_CUDA(h, cudaLaunchKernelExC(&cfg, h->line_fn, args));
+    h->launches += 1;
+    h->line_launches += 1;
+    return WAVE2D_OK;
+}
+
 int ensure_plan(wave2d_t* h)
 {
     if (h->plan_ok) return WAVE2D_OK;
@@ -522,6 +597,12 @@ int ensure_plan(wave2d_t* h)
     h->table_bytes = tbytes;
     W2D_CUDA(h, cudaMemcpyAsync(h->d_table, h->table.data(), tbytes, cudaMemcpyHostToDevice, h->stream));
     W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    st = plan_line(h);
+    if (st) return st;
+    if (h->line_mode) {
+        h->plan_ok = true;
+        return WAVE2D_OK;
+    }
     for (int d = 0; d < 2; ++d) {
         st = plan_dir(h, d);
         if (st) return st;
@@ -884,7 +965,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
         }
         h->scheme = iv;
     }
-    else if (!strcmp(name, "solver")) { if (iv < 0 || iv > 2) return WAVE2D_ERR_ARG; h->opt_solver = iv; }
+    else if (!strcmp(name, "solver")) { if (iv < 0 || iv > 3) return WAVE2D_ERR_ARG; h->opt_solver = iv; }
     else if (!strcmp(name, "graph")) h->opt_graph = iv != 0;
     else if (!strcmp(name, "graph_steps")) {
         if (iv < 1 || iv > MAX_CHUNK || (iv & (iv - 1))) return WAVE2D_ERR_ARG;   // 1, 2, 4, ..., MAX_CHUNK
@@ -1024,6 +1105,14 @@ int wave2d_run(wave2d_t* h, int steps)
         st = init_factored_v(h);
         if (st) return st;
     }
+    if (h->line_mode) {   // small grid: Algorithm 1's whole loop in one launch of one cluster
+        if (steps > 0) {
+            st = launch_line_steps(h, steps);
+            if (st) return st;
+            h->k += steps;
+        }
+        return WAVE2D_OK;
+    }
     // Algorithm 1's loop in chunks of 2^i steps, longest first; each chunk is one graph replay
     // (or, with graph = 0, the same kernel sequence launched directly).
     int left = steps;
@@ -1085,6 +1174,7 @@ int wave2d_get_info(wave2d_t* h, const char* name, double* value)
     if (!strcmp(name, "launches")) { *value = (double)h->launches; return WAVE2D_OK; }
     if (!strcmp(name, "graph_launches")) { *value = (double)h->graph_launches; return WAVE2D_OK; }
     if (!strcmp(name, "plain_sweeps")) { *value = (double)h->plain_sweeps; return WAVE2D_OK; }
+    if (!strcmp(name, "line_launches")) { *value = (double)h->line_launches; return WAVE2D_OK; }
     if (!strcmp(name, "source_window")) { *value = h->have_src ? (double)h->win_w * h->win_h : 0.0; return WAVE2D_OK; }
     int st = ensure_plan(h);
     if (st) return st;
@@ -1093,6 +1183,20 @@ int wave2d_get_info(wave2d_t* h, const char* name, double* value)
     const DirPlan& P = h->plan[name[len - 1] == 'y'];
     const std::string key(name, len - 2);
     const bool stream = P.solver == WAVE2D_SOLVER_STREAM;
+    if (P.solver == WAVE2D_SOLVER_LINE) {
+        if (key == "solver") *value = P.solver;
+        else if (key == "rho") *value = P.rho;
+        else if (key == "grid") *value = h->line_ctas;
+        else if (key == "threads") *value = 32 * LINE_WARPS;
+        else if (key == "smem") *value = h->line_smem;
+        else if (key == "unit") *value = h->line_unit;
+        else if (key == "ctas_per_sm") *value = 1;
+        else if (key == "chunks") *value = 1;
+        else if (key == "halo" || key == "nbk" || key == "kb" || key == "upc" || key == "quota" || key == "static" ||
+                 key == "safe") *value = 0;
+        else return WAVE2D_ERR_ARG;
+        return WAVE2D_OK;
+    }
     if (key == "solver") *value = P.solver;
     else if (key == "halo") *value = P.halo;
     else if (key == "rho") *value = P.rho;
@@ -1127,6 +1231,23 @@ int wave2d_profile_sweeps(wave2d_t* h, int steps, double* ms_x, double* ms_y)
     if (h->scheme == 1 && !h->v_ready) {
         st = init_factored_v(h);
         if (st) return st;
+    }
+    if (h->line_mode) {   // one kernel runs both half-steps of every step: the launch is timed, each sweep gets half
+        cudaEvent_t e0, e1;
+        W2D_CUDA(h, cudaEventCreate(&e0));
+        W2D_CUDA(h, cudaEventCreate(&e1));
+        W2D_CUDA(h, cudaEventRecord(e0, h->stream));
+        st = launch_line_steps(h, steps);
+        if (st) return st;
+        W2D_CUDA(h, cudaEventRecord(e1, h->stream));
+        W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+        float ms = 0.f;
+        W2D_CUDA(h, cudaEventElapsedTime(&ms, e0, e1));
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+        h->k += steps;
+        *ms_x = *ms_y = 0.5 * ms / steps;
+        return WAVE2D_OK;
     }
     std::vector<cudaEvent_t> ev((size_t)3 * steps);
     for (auto& e : ev) W2D_CUDA(h, cudaEventCreate(&e));

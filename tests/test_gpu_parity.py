@@ -63,21 +63,26 @@ def small_cases():
     ]
 
 
+_ST = {"solver": B.SOLVER_STREAM}
+
+
 @pytest.mark.parametrize("name,w", small_cases(), ids=[c[0] for c in small_cases()])
-@pytest.mark.parametrize("opts", [{}, {"solver": B.SOLVER_EXACT}, {"graph": 0}, {"quota_x": 3, "quota_y": 3},
-                                  {"shape_x": 1, "shape_y": 1, "quota_x": 4, "quota_y": 5},
-                                  {"shape_x": 2, "shape_y": 3}, {"shape_x": 3, "shape_y": 2}],
-                         ids=["default", "exact", "nograph", "quota3", "shapes1_cut", "shapes23", "shapes32"])
+@pytest.mark.parametrize("opts", [{}, _ST, {"solver": B.SOLVER_EXACT}, {"graph": 0, **_ST},
+                                  {"quota_x": 3, "quota_y": 3, **_ST},
+                                  {"shape_x": 1, "shape_y": 1, "quota_x": 4, "quota_y": 5, **_ST},
+                                  {"shape_x": 2, "shape_y": 3, **_ST}, {"shape_x": 3, "shape_y": 2, **_ST}],
+                         ids=["default", "stream", "exact", "nograph", "quota3", "shapes1_cut", "shapes23", "shapes32"])
 def test_small_workloads_match_oracle(name, w, opts):
     r = ref(w)
     u, info = gpu(w, **opts)
     assert np.isfinite(u).all()
     assert relerr(u, r) <= TOL[w.dtype]
-    assert info["launches"] >= 2 * w.M          # the CUDA kernels ran: >= 2 sweeps per step
-    if opts.get("solver") == B.SOLVER_EXACT:
-        assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
-    elif "solver" not in opts:
-        assert info["solver_x"] == B.SOLVER_STREAM and info["solver_y"] == B.SOLVER_STREAM
+    want = opts.get("solver", B.SOLVER_LINE if max(w.n1, w.n2) <= 256 else B.SOLVER_STREAM)   # AUTO: small grids -> LINE
+    assert info["solver_x"] == want and info["solver_y"] == want
+    if want == B.SOLVER_LINE:
+        assert info["launches"] == 1            # Algorithm 1's whole loop in one launch
+    else:
+        assert info["launches"] >= 2 * w.M      # the CUDA kernels ran: >= 2 sweeps per step
 
 
 @pytest.mark.parametrize("N1,N2", [(2, 2), (2, 9), (9, 2), (3, 3), (4, 5), (16, 17), (17, 16), (18, 33), (33, 18),
@@ -94,7 +99,7 @@ def test_tiny_and_ragged_sizes(N1, N2):
     g = rng.uniform(-1, 1, 2 * M)
     w = W.Workload("rand", N1, N2, 1.0, tau, M, "f64", phi, psi, c, s=s, g_half=g)
     r = ref(w)
-    for opts in ({}, {"solver": B.SOLVER_EXACT}):
+    for opts in ({}, {"solver": B.SOLVER_STREAM}, {"solver": B.SOLVER_EXACT}):   # {}: the small-grid kernel (LINE)
         u, _ = gpu(w, **opts)
         assert relerr(u, r) <= 1e-12, (opts, relerr(u, r))
 
@@ -110,18 +115,23 @@ def test_literal_constants_gamma1_kappa1():
     assert relerr(u, ref(w)) > 1e-3   # and it differs from the default reading
 
 
-def test_large_tau_falls_back_to_exact_solver():
-    """tau = 16 h: rho = 0.88, the decay bound needs ~300 points of look-ahead -> AUTO picks EXACT."""
-    N, M = 160, 12
+@pytest.mark.parametrize("N", [160, 300])
+def test_large_tau_falls_back_to_exact_solver(N):
+    """tau = 16 h: rho = 0.88, the decay bound needs ~300 points of look-ahead: the streamed kernels refuse, AUTO
+    picks the small-grid kernel (exact for any tau) at N = 160 and the EXACT path at N = 300."""
+    M = 12
     w = W.cfg2(N=N, M=M)
     w.tau = 16.0 / N
     r = ref(w)
     u, info = gpu(w)
-    assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
+    want = B.SOLVER_LINE if N <= 257 else B.SOLVER_EXACT
+    assert info["solver_x"] == want and info["solver_y"] == want
     assert relerr(u, r) <= 1e-10
     with pytest.raises(B.Wave2DError) as e:
         gpu(w, solver=B.SOLVER_STREAM)
     assert e.value.status == -5
+    u, info = gpu(w, solver=B.SOLVER_EXACT)
+    assert info["solver_x"] == B.SOLVER_EXACT and relerr(u, r) <= 1e-10
 
 
 @pytest.mark.parametrize("ratio,H", [(2.3, 47), (3.0, 60)])
@@ -429,14 +439,18 @@ def factored_cases():
 
 
 @pytest.mark.parametrize("name,w", factored_cases(), ids=[c[0] for c in factored_cases()])
-@pytest.mark.parametrize("opts", [{}, {"solver": B.SOLVER_EXACT}, {"graph": 0}, {"quota_x": 3, "quota_y": 3}],
-                         ids=["default", "exact", "nograph", "quota3"])
+@pytest.mark.parametrize("opts", [{}, _ST, {"solver": B.SOLVER_EXACT}, {"graph": 0, **_ST},
+                                  {"quota_x": 3, "quota_y": 3, **_ST}],
+                         ids=["default", "stream", "exact", "nograph", "quota3"])
 def test_factored_scheme_matches_oracle(name, w, opts):
     r = ref1(w)
     u, info = gpu1(w, **opts)
     assert np.isfinite(u).all()
     assert relerr(u, r) <= TOL[w.dtype]
-    assert info["launches"] >= 2 * (w.M - 1)
+    if info["solver_x"] == B.SOLVER_LINE:
+        assert info["launches"] == 3            # the two start kernels + one launch for every step
+    else:
+        assert info["launches"] >= 2 * (w.M - 1)
 
 
 def test_factored_scheme_levels_one_by_one_and_modal():
@@ -594,7 +608,7 @@ def test_tiny_and_ragged_sizes_fp32_and_scheme1(N1, N2, dtype, scheme):
     g = rng.uniform(-1, 1, 2 * M)
     w = W.Workload("rand", N1, N2, 1.0, tau, M, dtype, phi, psi, c, s=s, g_half=g)
     tol = 1e-12 if dtype == "f64" else 2e-5
-    for opts in ({}, {"solver": B.SOLVER_EXACT}):
+    for opts in ({}, {"solver": B.SOLVER_STREAM}, {"solver": B.SOLVER_EXACT}):
         if scheme:
             u, _ = gpu1(w, **opts)
             r = ref1(w)
@@ -648,14 +662,16 @@ def test_early_start_and_pdl_do_not_change_a_single_bit():
         assert np.array_equal(u, base1), opts
 
 
-def test_factored_scheme_large_tau_falls_back_to_exact_solver():
-    N, M = 160, 10
+@pytest.mark.parametrize("N", [160, 300])
+def test_factored_scheme_large_tau_falls_back_to_exact_solver(N):
+    M = 10
     w = W.cfg2(N=N, M=M)
     w.tau = 16.0 / N
     w.psi = 0.2 * w.phi
     r = ref1(w)
     u, info = gpu1(w)
-    assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
+    want = B.SOLVER_LINE if N <= 257 else B.SOLVER_EXACT
+    assert info["solver_x"] == want and info["solver_y"] == want
     assert relerr(u, r) <= 1e-10
 
 
@@ -682,3 +698,73 @@ def test_two_handles_on_two_streams_run_concurrently():
             ha.close()
             hb.close()
         assert np.array_equal(ua, solo_a) and np.array_equal(ub, solo_b), it
+
+
+# ---- the small-grid kernel (solver LINE): one cluster, one launch for the whole step loop, exact warp-scan solves ----
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 31, 32, 33, 126, 127, 128, 129, 200, 255, 256])
+@pytest.mark.parametrize("alpha", [0.5, 50.0, 128.0])
+def test_line_kernel_sizes_and_any_tau(n, alpha):
+    """SURVEY.md 8c pin 7: n in {1, 2, 3, 126..129, ...} and alpha = tau^2 c / (2 h^2) in {0.5, 50, 128} (tau up to 16 h,
+    rho = 0.88, where a truncated solver fails: tiny n with large alpha gave 1.7e-1 in the survey's probe).  The warp
+    scan truncates nothing, so every case matches the Thomas oracle to rounding.  Asymmetric grid: n x (n + 3)."""
+    N1, N2 = n + 1, min(n + 4, 257)
+    M = 6
+    rng = np.random.default_rng(31 * n + int(alpha))
+    tau = np.sqrt(2.0 * alpha) / N1                      # alpha_x = tau^2 / (2 h1^2) with c = 1
+    shape = (N2 - 1, N1 - 1)
+    phi, psi, s = (rng.uniform(-1, 1, shape) for _ in range(3))
+    c = rng.uniform(0.8, 1.0, 2 * M + 1)
+    g = rng.uniform(-1, 1, 2 * M)
+    # fp32 away from the configs' alpha <= 1: the systems' condition number (gamma + 4 alpha) / gamma bounds the rounding
+    # of each solve, ~ cond * 6e-8 per half-step
+    tol32 = max(1e-4, 12 * (2.0 + 4.0 * alpha * (N2 / N1) ** 2) / 2.0 * 6e-8 * 4)
+    for dtype, tol in (("f64", 1e-11), ("f32", tol32)):
+        w = W.Workload("rand", N1, N2, 1.0, tau, M, dtype, phi, psi, c, s=s, g_half=g)
+        npdt = np.float64 if dtype == "f64" else np.float32
+        cast = lambda a: a.astype(npdt).astype(np.float64)
+        r = oracle.solve(N1, N2, 1.0, tau, M, cast(phi), cast(psi), c_half=c, s=cast(s), g_half=g)
+        u, info = gpu(w)
+        assert info["solver_x"] == B.SOLVER_LINE and info["solver_y"] == B.SOLVER_LINE and info["launches"] == 1
+        assert relerr(u, r) <= tol, (dtype, relerr(u, r))
+        r1 = oracle.solve(N1, N2, 1.0, tau, M, cast(phi), cast(psi), c_half=c, s=cast(s), g_half=g, scheme=1)
+        u1, info = gpu1(w)
+        assert info["solver_x"] == B.SOLVER_LINE
+        assert relerr(u1, r1) <= tol, (dtype, "scheme 1", relerr(u1, r1))
+
+
+def test_line_kernel_run_in_pieces_checkpoint_and_limits():
+    w = W.cfg2(N=256, M=40)
+    src = W.cfg3(N=256, M=40)
+    w.s, w.g_half = src.s, W.ricker(W.half_times(w.tau, 2 * w.M) + 0.058)
+    h = B.from_workload(w)
+    try:
+        h.run(w.M)
+        a = h.get()
+        assert h.info("line_launches") == 1 and h.info("graph_launches") == 0 and h.info("plain_sweeps") == 0
+        h.set_initial(w.phi)
+        for part in (1, 2, 0, 7, 13, 17):
+            h.run(part)
+        assert h.steps_done() == w.M
+        b = h.get()
+        h.set_initial(w.phi)
+        h.run(11)
+        prev, cur = h.get_prev(), h.get()
+    finally:
+        h.close()
+    assert np.array_equal(a, b)                     # one launch of 40 steps == six launches
+    assert relerr(a, ref(w)) <= 1e-10
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+    try:
+        h.set_speed(w.c_half)
+        h.set_source(w.s, w.g_half)
+        h.set_state(11, prev, cur)
+        h.run(w.M - 11)
+        assert np.array_equal(h.get(), a)           # resume from a checkpoint: the device step counter follows set_state
+    finally:
+        h.close()
+    u, info = gpu(w, solver=B.SOLVER_STREAM)         # the streamed kernels on the same grid agree to rounding
+    assert info["solver_x"] == B.SOLVER_STREAM and relerr(u, a) <= 1e-12
+    big = W.cfg2(N=258, M=2)
+    with pytest.raises(B.Wave2DError) as e:
+        gpu(big, solver=B.SOLVER_LINE)
+    assert e.value.status == -5
