@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--scheme", type=int, default=0, choices=[0, 1],
                     help="0: the paper's split scheme (2.11)-(2.12) (default, the north_star path); "
                          "1: factorised unsplit scheme (2.8), 5 field passes per step (SURVEY.md 8f NEXT-2)")
+    ap.add_argument("--tau-factor", type=float, default=1.0,
+                    help="off-config: multiply the workload's tau (16: alpha = 128, the exact whole-line solvers run)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps per end-to-end iteration (default: --steps)")
@@ -299,6 +301,9 @@ def run_ours(args):
     K, Wm = args.steps, args.warmup
     PROF = 12                                             # per-kernel timing pass (plain launches + events)
     w = load_workload(args.workload, Wm + K + PROF + 2)
+    if args.tau_factor != 1.0:
+        w.tau *= args.tau_factor
+        w.name += f" with tau x {args.tau_factor:g} (off-config)"
     sch = args.scheme
     npdt = np.float64 if w.dtype == "f64" else np.float32
     esz = 8 if w.dtype == "f64" else 4
@@ -397,7 +402,8 @@ def run_ours(args):
                 "steps_per_call": Ke, "seconds_per_call": e2e_s,
                 "what": "wave2d_set_initial(pinned host phi) + wave2d_run(steps_per_call) + wave2d_get(pinned host u), "
                         "wall clock incl. both copies; bytes are per call / steps_per_call"},
-        "roofline": {"bound": "hbm", "kernel": (f"wave2d_sweep_panel<{w.dtype}, dir={dom}>" if geom["solver_x"] != 3 else
+        "roofline": {"bound": "hbm", "kernel": (f"wave2d_exact_{dom}<{w.dtype}>" if geom["solver_x"] == 1 else
+                                                f"wave2d_sweep_panel<{w.dtype}, dir={dom}>" if geom["solver_x"] != 3 else
                                                 f"wave2d_line_steps<{w.dtype}> (both half-steps of every step in one "
                                                 "launch; each sweep is given half of it)"), "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,

@@ -58,6 +58,10 @@ def lib() -> C.CDLL:
             L.oracle_wave2d_set_initial.argtypes = [C.c_void_p, _dp, _dp, C.c_long]
             L.oracle_wave2d_set_speed.argtypes = [C.c_void_p, _dp, C.c_int]
             L.oracle_wave2d_set_source.argtypes = [C.c_void_p, _dp, C.c_long, _dp, C.c_int]
+            L.oracle_wave2d_set_speed_field.argtypes = [C.c_void_p, _dp, C.c_long]
+            L.oracle_half_step_var.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                               C.c_double, _dp, _dp, _dp, _dp, _dp]
+            L.oracle_half_step_var.restype = None
             L.oracle_wave2d_run.argtypes = [C.c_void_p, C.c_int]
             L.oracle_wave2d_get.argtypes = [C.c_void_p, _dp, C.c_long]
             L.oracle_wave2d_get_prev.argtypes = [C.c_void_p, _dp, C.c_long]
@@ -101,6 +105,18 @@ def half_step(direction: int, ap: float, am: float, gamma: float, q: float, w_pr
     n2, n1 = w_prev.shape
     out = np.empty_like(w_prev)
     lib().oracle_half_step(n1, n2, int(direction), ap, am, gamma, q, _p(w_prev), _p(w_cur), _p(s), _p(out))
+    return out
+
+
+def half_step_var(direction: int, ap: float, am: float, gamma: float, q: float, cs, w_prev, w_cur, s=None) -> np.ndarray:
+    """One half-step with the spatial speed factor cs (oracle_half_step_var); arrays of shape (n2, n1)."""
+    w_prev = _f64(w_prev)
+    w_cur = _f64(w_cur, w_prev.shape)
+    cs = _f64(cs, w_prev.shape)
+    s = _f64(s, w_prev.shape) if s is not None else None
+    n2, n1 = w_prev.shape
+    out = np.empty_like(w_prev)
+    lib().oracle_half_step_var(n1, n2, int(direction), ap, am, gamma, q, _p(cs), _p(w_prev), _p(w_cur), _p(s), _p(out))
     return out
 
 
@@ -156,6 +172,13 @@ class Wave2DOracle:
         c_half = _f64(np.atleast_1d(c_half))
         _check(lib().oracle_wave2d_set_speed(self._h, _p(c_half), c_half.shape[0]), "set_speed")
 
+    def set_speed_field(self, cs):
+        if cs is None:
+            _check(lib().oracle_wave2d_set_speed_field(self._h, None, 0), "set_speed_field")
+            return
+        cs = _f64(cs, (self.n2, self.n1))
+        _check(lib().oracle_wave2d_set_speed_field(self._h, _p(cs), self.n1), "set_speed_field")
+
     def set_source(self, s, g_half=None):
         if s is None:
             _check(lib().oracle_wave2d_set_source(self._h, None, 0, None, 0), "set_source")
@@ -185,7 +208,7 @@ class Wave2DOracle:
 
 
 def solve(N1, N2, l, tau, M, phi, psi=None, c_half=None, s=None, g_half=None, steps=None,
-          gamma=None, kappa=None, scheme=0) -> np.ndarray:
+          gamma=None, kappa=None, scheme=0, cs=None) -> np.ndarray:
     """Convenience: advance to time level `steps` (default M) and return u^steps.
     scheme 1 (factorised (2.8)): set_initial already stands at level 1, so steps - 1 solves are run."""
     o = Wave2DOracle(N1, N2, l, tau, M)
@@ -198,6 +221,8 @@ def solve(N1, N2, l, tau, M, phi, psi=None, c_half=None, s=None, g_half=None, st
             o.set_option("kappa", kappa)
         if c_half is not None:
             o.set_speed(c_half)
+        if cs is not None:
+            o.set_speed_field(cs)
         if s is not None:
             o.set_source(s, g_half)
         o.set_initial(phi, psi)

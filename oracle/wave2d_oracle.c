@@ -36,6 +36,9 @@
  * A second scheme (option "scheme" = 1, oracle_factored_step below) is the factorised form of the unsplit
  * scheme (2.8); it has its own pins (tests/test_oracle_factored.py).
  *
+ * A variable speed c(t) cs(x,y) (oracle_half_step_var) has its pins in
+ * tests/test_oracle_varspeed.py.
+ *
  * Parity pins (tests/test_oracle_*.py): dense LU of the Kronecker system on tiny grids, the exact
  * discrete modal recurrence, the PDE standing wave (observed order 1), forced response, tridiagonal
  * residuals, linearity / reflection invariants.  Nothing here is "parity unpinned".
@@ -118,6 +121,55 @@ void oracle_half_step(int n1, int n2, int dir, double ap, double am, double gamm
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * Variable speed (reading R16).  Algorithm 1 computes the tridiagonal elements
+ * a_i, b_i, c_i, f_i point by point; with a speed c(t) cs(x,y) -- separable like the source
+ * f = g(t) s(x,y) of PAPER.md:33 -- the weights of (2.11)/(2.12) are taken at the point p of the equation:
+ *
+ *   gamma (x_p - 2 w_n[p] + w_{n-1}[p])
+ *      - ap cs[p] (x_{p+1} - 2 x_p + x_{p-1}) - am cs[p] (w_{n-1}[p+1] - 2 w_{n-1}[p] + w_{n-1}[p-1])
+ *      = kappa tau^2 g_n s[p]
+ *
+ * i.e.  a_p = c_p = -ap cs[p],  b_p = gamma + 2 ap cs[p]  (a non-Toeplitz, non-symmetric, strictly diagonally
+ * dominant system per line).  ap, am, q as in oracle_half_step; cs: n2 x n1, every value > 0.
+ * ---------------------------------------------------------------------------------------------- */
+void oracle_half_step_var(int n1, int n2, int dir, double ap, double am, double gamma, double q, const double *cs,
+                          const double *w_prev, const double *w_cur, const double *s, double *w_next)
+{
+    const int nlines = dir == 0 ? n2 : n1;
+    const int n = dir == 0 ? n1 : n2;
+    const long step = dir == 0 ? 1 : n1;
+    const long lstep = dir == 0 ? n1 : 1;
+
+#pragma omp parallel
+    {
+        double *a = (double *)malloc(sizeof(double) * 7 * (size_t)(n > 0 ? n : 1));
+        double *b = a + n, *c = b + n, *f = c + n, *x = f + n, *cp = x + n, *fp = cp + n;
+#pragma omp for schedule(static)
+        for (int line = 0; line < nlines; ++line) {
+            const double *wp = w_prev + line * lstep;
+            const double *wc = w_cur + line * lstep;
+            const double *cl = cs + line * lstep;
+            const double *sp = s ? s + line * lstep : NULL;
+            for (int p = 0; p < n; ++p) {
+                double wm = p > 0 ? wp[(p - 1) * step] : 0.0;     /* zero Dirichlet ghost, (2.10) */
+                double wq = p < n - 1 ? wp[(p + 1) * step] : 0.0;
+                double w0 = wp[p * step];
+                double app = ap * cl[p * step], amp = am * cl[p * step];
+                a[p] = -app;
+                b[p] = gamma + 2.0 * app;
+                c[p] = -app;
+                f[p] = gamma * (2.0 * wc[p * step] - w0) + amp * (wm - 2.0 * w0 + wq);
+                if (sp) f[p] += q * sp[p * step];
+            }
+            oracle_thomas(n, a, b, c, f, x, cp, fp);
+            double *wn = w_next + line * lstep;
+            for (int p = 0; p < n; ++p) wn[p * step] = x[p];
+        }
+        free(a);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------
  * Scheme 1: the factorised form of the UNSPLIT three-level scheme (2.8).
  * (2.8) times tau^2 reads, with a_d^+- = tau^2 c^{k+-1} / (2 h_d^2) and D_d the undivided second difference
  * along d with zero Dirichlet ghosts (2.10),
@@ -188,6 +240,7 @@ typedef struct oracle_wave2d_s {
     double *c_half;   /* 2M+1 samples c(n tau/2)                                   */
     double *g_half;   /* 2M samples g(n tau/2), or NULL meaning g == 1             */
     double *s;        /* n2 x n1 source shape, or NULL (no source)                 */
+    double *cs;       /* n2 x n1 spatial speed factor, or NULL (c = c(t) only)     */
     double *w[3];     /* w[0] = w_{n-1}, w[1] = w_n, w[2] = scratch for w_{n+1}     */
     int have_initial; /* set_initial called                                        */
     int n_done;       /* half-steps taken so far (scheme 1: 2 x the time level k)  */
@@ -215,7 +268,7 @@ int oracle_wave2d_create(oracle_wave2d_t **out, int N1, int N2, double l, double
 void oracle_wave2d_destroy(oracle_wave2d_t *h)
 {
     if (!h) return;
-    free(h->c_half); free(h->g_half); free(h->s);
+    free(h->c_half); free(h->g_half); free(h->s); free(h->cs);
     for (int k = 0; k < 3; ++k) free(h->w[k]);
     free(h);
 }
@@ -268,6 +321,24 @@ int oracle_wave2d_set_speed(oracle_wave2d_t *h, const double *c_half, int count)
     return ORACLE_OK;
 }
 
+/* Spatial speed factor: c(t,x,y) = c_half[n] * cs(x,y) (reading R16); cs NULL returns to c = c(t).  Scheme 0 only. */
+int oracle_wave2d_set_speed_field(oracle_wave2d_t *h, const double *cs, long ld)
+{
+    if (!h) return ORACLE_ERR_ARG;
+    if (h->n_done > (h->scheme == 1 ? 2 : 0)) return ORACLE_ERR_STATE;
+    free(h->cs); h->cs = NULL;
+    if (!cs) return ORACLE_OK;
+    if (ld < h->n1 || h->scheme == 1) return ORACLE_ERR_ARG;
+    for (int j = 0; j < h->n2; ++j)
+        for (int i = 0; i < h->n1; ++i)
+            if (!(cs[(long)j * ld + i] > 0.0)) return ORACLE_ERR_ARG;   /* PAPER.md:31, positive speed */
+    h->cs = (double *)malloc(sizeof(double) * (size_t)h->n1 * (size_t)h->n2);
+    if (!h->cs) return ORACLE_ERR_ALLOC;
+    for (int j = 0; j < h->n2; ++j)
+        memcpy(h->cs + (size_t)j * h->n1, cs + (long)j * ld, sizeof(double) * (size_t)h->n1);
+    return ORACLE_OK;
+}
+
 /* f(t,x,y) = g(t) s(x,y); g_half[n] = g(n tau/2), n = 0..2M-1; g_half NULL means g == 1; s NULL clears. */
 int oracle_wave2d_set_source(oracle_wave2d_t *h, const double *s, long ld, const double *g_half, int count)
 {
@@ -294,6 +365,7 @@ int oracle_wave2d_run(oracle_wave2d_t *h, int steps)
     if (!h || steps < 0) return ORACLE_ERR_ARG;
     if (!h->have_initial) return ORACLE_ERR_STATE;
     if (h->n_done / 2 + steps > h->M) return ORACLE_ERR_RANGE;
+    if (h->scheme == 1 && h->cs) return ORACLE_ERR_ARG;
     if (h->scheme == 1) {   /* (2.8) factorised: level k -> k+1 needs c^{k-1}, c^{k+1}, g^k (integer levels) */
         for (int it = 0; it < steps; ++it) {
             const int k = h->n_done / 2;
@@ -318,7 +390,8 @@ int oracle_wave2d_run(oracle_wave2d_t *h, int steps)
         const double am = t2 * h->c_half[n > 0 ? n - 1 : 0] / (2.0 * hd * hd);   /* reading A5 */
         const double g = h->g_half ? h->g_half[n] : 1.0;                        /* reading A8 */
         const double q = h->kappa * t2 * g;
-        oracle_half_step(h->n1, h->n2, dir, ap, am, h->gamma, q, h->w[0], h->w[1], h->s, h->w[2]);
+        if (h->cs) oracle_half_step_var(h->n1, h->n2, dir, ap, am, h->gamma, q, h->cs, h->w[0], h->w[1], h->s, h->w[2]);
+        else oracle_half_step(h->n1, h->n2, dir, ap, am, h->gamma, q, h->w[0], h->w[1], h->s, h->w[2]);
         /* (w_prev, w_cur) <- (w_cur, w_next): "swap(u,Ux); swap(U0,Uy)" done one half-level at a time */
         double *old = h->w[0];
         h->w[0] = h->w[1]; h->w[1] = h->w[2]; h->w[2] = old;

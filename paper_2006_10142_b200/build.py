@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libwave2d.so")
 _SOURCES = ["wave2d.cu"]
-_DEPS = ["wave2d.cu", "kernels.cuh", "line.cuh", "ptx.cuh", os.path.join("..", "..", "include", "wave2d.h")]
+_DEPS = ["wave2d.cu", "kernels.cuh", "exact.cuh", "line.cuh", "ptx.cuh", os.path.join("..", "..", "include", "wave2d.h")]
 
 
 def nvcc_path() -> str:

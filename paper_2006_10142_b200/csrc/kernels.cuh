@@ -671,97 +671,10 @@ wave2d_sweep_panel(const __grid_constant__ SweepMaps maps, const __grid_constant
 #undef tm_edge
 }
 
-// ---------------------------------------------------------------------------------------------------
-// Exact path (any tau/h): plain Thomas elimination with the half-step's own pivots, one thread per
-// line, two passes through HBM (forward writes y into `out`, backward turns it into x in place).
-// Used when rho^H cannot be made negligible within the look-ahead the streamed kernel supports, or
-// on request (WAVE2D_SOLVER_EXACT).  DIR 1 is coalesced; DIR 0 walks rows and is slow but correct.
-// ---------------------------------------------------------------------------------------------------
-// cpv[p], ivv[p], p < n: one thread block; thread 0 runs the pivot recurrence until it is stationary.
-__global__ void wave2d_exact_pivots(const double* table, int period, const int* d_k, int n_off, int n, double* cpv,
-                                    double* ivv)
-{
-    __shared__ int s_conv;
-    const int nh = n_off + 2 * (*d_k);
-    const double* row = table + static_cast<size_t>(period ? nh % period : nh) * ROW_DOUBLES;
-    const double ap = row[ROW_AP], beta = row[ROW_BETA];
-    if (threadIdx.x == 0) {
-        double cp = 0.0;
-        int p = 0;
-        for (; p < n; ++p) {
-            const double iv = 1.0 / (beta - ap * cp);
-            const double cn = ap * iv;
-            cpv[p] = cn;
-            ivv[p] = iv;
-            if (cn == cp) { ++p; break; }
-            cp = cn;
-        }
-        s_conv = p;
-    }
-    __syncthreads();
-    const int pc = s_conv;
-    if (pc < n) {
-        const double cp = cpv[pc - 1], iv = ivv[pc - 1];
-        for (int p = pc + threadIdx.x; p < n; p += blockDim.x) {
-            cpv[p] = cp;
-            ivv[p] = iv;
-        }
-    }
-}
-
 struct FieldSet {   // the ring of field buffers; roles by roles_of(nh, ring)
     void* b[4];
     int ring;
 };
-
-template <typename T, int DIR>
-__global__ void wave2d_exact_forward(const FieldSet fs, const double* table, int period, const int* d_k, int n_off,
-                                     int n, int nlines, long long pitch, const double* __restrict__ cpv,
-                                     const double* __restrict__ ivv, const T* __restrict__ src, int sl0, int snl, int sp0,
-                                     int snp, double g2d)
-{
-    const int line = blockIdx.x * blockDim.x + threadIdx.x;
-    if (line >= nlines) return;
-    const int nh = n_off + 2 * (*d_k);
-    const Roles R = roles_of(nh, fs.ring);
-    const T* __restrict__ wprev = static_cast<const T*>(fs.b[R.prev]);
-    const T* __restrict__ wcur = static_cast<const T*>(fs.b[R.cur]);
-    T* __restrict__ out = static_cast<T*>(fs.b[R.out]);
-    const double* row = table + static_cast<size_t>(period ? nh % period : nh) * ROW_DOUBLES;
-    const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), c1 = static_cast<T>(row[ROW_C1]);
-    const T g2 = static_cast<T>(g2d);
-    const long long ls = DIR == 0 ? pitch : 1, ps = DIR == 0 ? 1 : pitch;   // strides between lines / along the line
-    const T* wp = wprev + line * ls;
-    const T* wc = wcur + line * ls;
-    T* o = out + line * ls;
-    const bool src_line = src != nullptr && line >= sl0 && line < sl0 + snl;
-    T left = T(0), mid = n > 0 ? wp[0] : T(0), fy = T(0);
-    for (int p = 0; p < n; ++p) {
-        const T right = p + 1 < n ? wp[(p + 1) * ps] : T(0);
-        T r = fma(g2, wc[p * ps], fma(am, left + right, c1 * mid));
-        if (src_line && p >= sp0 && p < sp0 + snp) r = fma(q, src[static_cast<size_t>(p - sp0) * snl + (line - sl0)], r);
-        fy = fma(static_cast<T>(cpv[p]), fy, r * static_cast<T>(ivv[p]));
-        o[p * ps] = fy;
-        left = mid;
-        mid = right;
-    }
-}
-
-template <typename T, int DIR>
-__global__ void wave2d_exact_backward(const FieldSet fs, const int* d_k, int n_off, int n, int nlines, long long pitch,
-                                      const double* __restrict__ cpv)
-{
-    const int line = blockIdx.x * blockDim.x + threadIdx.x;
-    if (line >= nlines) return;
-    T* __restrict__ out = static_cast<T*>(fs.b[roles_of(n_off + 2 * (*d_k), fs.ring).out]);
-    const long long ls = DIR == 0 ? pitch : 1, ps = DIR == 0 ? 1 : pitch;
-    T* o = out + line * ls;
-    T x = T(0);
-    for (int p = n - 1; p >= 0; --p) {
-        x = fma(static_cast<T>(cpv[p]), x, o[p * ps]);
-        o[p * ps] = x;
-    }
-}
 
 // ---- A-init (PAPER.md:68-69 (2.9)): w_{-1} = phi - (tau/2) psi -----------------
 template <typename T>

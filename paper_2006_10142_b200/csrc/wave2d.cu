@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "exact.cuh"
 #include "line.cuh"
 
 using namespace w2d;
@@ -124,6 +125,9 @@ struct DirPlan {
     std::vector<int> cta_off;   // CTA b's static share: pieces [cta_off[b], cta_off[b+1]); pieces >= nstatic are drawn
     int nstatic = 0;
     bool has_safe = false;      // some static piece may start before the previous sweep ends (early start)
+    // exact path (exact.cuh)
+    const void* ex_fn = nullptr;
+    int ex_wpc = 0, ex_nseg = 0, ex_sc = 0, ex_smem = 0;
 };
 
 }  // namespace
@@ -430,6 +434,54 @@ int make_tmap_x3(wave2d_t* h, CUtensorMap* tm, void* base, int ntiles)
     return WAVE2D_OK;
 }
 
+// Exact path (exact.cuh): a group of wpc warps per line, segments of wpc * 32 * 8 points.
+//   x: rows; nseg > 1 parks y of the whole line in shared memory (needs the full CTA per line).
+//   y: strips of sc columns, the widest that fits the shared-memory budget, all rows of the strip on chip.
+int plan_exact(wave2d_t* h, int d)
+{
+    DirPlan& P = h->plan[d];
+    const int units = (P.n + EX_U - 1) / EX_U;
+    int wpc = 1;
+    while (wpc < EX_NW && wpc * 32 < units) wpc *= 2;        // power of two, so that it divides EX_NW
+    const int nseg = (units + wpc * 32 - 1) / (wpc * 32);
+    const size_t budget = 200 * 1024;
+    P.ex_wpc = wpc;
+    if (d == 0) {
+        P.ex_nseg = nseg;
+        P.ex_sc = 0;
+        // nseg > 1: the parked line; else the two prefetch slots of (2 NV + 1) 16-byte cells per thread
+        const size_t smem = nseg > 1 ? (size_t)nseg * wpc * 32 * EX_U * h->elem
+                                     : (size_t)2 * (2 * (EX_U * h->elem / 16) + 1) * EX_NT * 16;
+        if (smem > budget) {
+            h->err = "exact solver: an x line of more than 25600 fp64 unknowns does not fit shared memory";
+            return WAVE2D_ERR_UNSUPPORTED;
+        }
+        P.ex_smem = (int)smem;
+        P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double>)
+                                         : reinterpret_cast<const void*>(&wave2d_exact_x<float>);
+        const int passes = (P.nlines + EX_NW / wpc - 1) / (EX_NW / wpc);
+        P.grid = std::max(1, std::min(passes, 4 * h->num_sms));
+    } else {
+        const size_t col = (size_t)units * (EX_U + 1) * h->elem;   // one column of the strip
+        int sc = 16;
+        while (sc > 1 && sc * col > budget) sc /= 2;
+        if (sc * col > budget) {
+            h->err = "exact solver: a y line of more than 22700 fp64 unknowns does not fit shared memory";
+            return WAVE2D_ERR_UNSUPPORTED;
+        }
+        while (sc > 1 && (P.nlines + sc - 1) / sc < h->num_sms) sc /= 2;   // small grids: more, narrower strips
+        P.ex_sc = sc;
+        P.ex_nseg = nseg;
+        P.ex_smem = (int)(sc * col);
+        P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double>)
+                                         : reinterpret_cast<const void*>(&wave2d_exact_y<float>);
+        const int strips = (P.nlines + sc - 1) / sc;
+        P.grid = std::max(1, std::min(strips, 4 * h->num_sms));
+    }
+    W2D_CUDA(h, cudaFuncSetAttribute(P.ex_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
+    return WAVE2D_OK;
+}
+
 int plan_dir(wave2d_t* h, int d)
 {
     DirPlan& P = h->plan[d];
@@ -475,7 +527,7 @@ int plan_dir(wave2d_t* h, int d)
     const bool fits = nbk <= std::min(NBK_MAX, V.nw) && pconv <= KMAX;
     if (h->opt_solver == WAVE2D_SOLVER_EXACT || (h->opt_solver == WAVE2D_SOLVER_AUTO && !fits)) {
         P.solver = WAVE2D_SOLVER_EXACT;
-        return WAVE2D_OK;
+        return plan_exact(h, d);
     }
     if (!fits) {
         h->err = "streamed solver: decay bound rho^H <= tol needs a longer carry series than supported";
@@ -651,7 +703,7 @@ int ensure_plan(wave2d_t* h)
         }
     }
     if ((h->plan[0].solver == WAVE2D_SOLVER_EXACT || h->plan[1].solver == WAVE2D_SOLVER_EXACT) && !h->d_piv) {
-        st = dev_alloc(h, reinterpret_cast<void**>(&h->d_piv), sizeof(double) * 2 * (size_t)std::max(h->n1, h->n2));
+        st = dev_alloc(h, reinterpret_cast<void**>(&h->d_piv), sizeof(double) * (2 * (size_t)std::max(h->n1, h->n2) + 1));
         if (st) return st;
     }
     h->plan_ok = true;
@@ -718,30 +770,31 @@ int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own
         W2D_CUDA(h, cudaLaunchKernelExC(&cfg, P.var->fn, args));
         return WAVE2D_OK;
     }
-    // exact two-pass Thomas
+    // exact path: pivots of this half-step, then the whole-line solver of the direction (exact.cuh)
     double* cpv = h->d_piv;
     double* ivv = h->d_piv + std::max(h->n1, h->n2);
-    const FieldSet fs = field_set(h);
-    wave2d_exact_pivots<<<1, 256, 0, stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv);
-    const int tb = 128, gb = (P.nlines + tb - 1) / tb;
-    const double g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
-#define W2D_EXACT(T, D)                                                                                               \
-    do {                                                                                                              \
-        wave2d_exact_forward<T, D><<<gb, tb, 0, stream>>>(fs, h->d_table, h->table_period, dk, n_off, P.n, P.nlines,  \
-                                                          h->pitch, cpv, ivv, (const T*)src, sl0, snl, sp0, snp, g2); \
-        wave2d_exact_backward<T, D><<<gb, tb, 0, stream>>>(fs, dk, n_off, P.n, P.nlines, h->pitch, cpv);              \
-    } while (0)
-    if (h->dtype == WAVE2D_F64) {
-        if (d == 0) W2D_EXACT(double, 0); else W2D_EXACT(double, 1);
-    } else {
-        if (d == 0) W2D_EXACT(float, 0); else W2D_EXACT(float, 1);
-    }
-#undef W2D_EXACT
-    W2D_CUDA(h, cudaGetLastError());
+    int* conv = reinterpret_cast<int*>(h->d_piv + 2 * (size_t)std::max(h->n1, h->n2));
+    wave2d_exact_pivots<<<1, 256, 0, stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv, conv);
+    ExactArgs a;
+    a.conv = conv;
+    a.fs = field_set(h);
+    a.table = h->d_table; a.period = h->table_period; a.d_k = dk; a.n_off = n_off;
+    a.n = P.n; a.nlines = P.nlines; a.pitch = h->pitch; a.cpv = cpv; a.ivv = ivv;
+    a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
+    a.g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
+    a.one = h->scheme == 1 && d == 1;
+    a.wpc = P.ex_wpc; a.nseg = P.ex_nseg; a.sc = P.ex_sc;
+    void* args[1] = {&a};
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(P.grid);
+    cfg.blockDim = dim3(EX_NT);
+    cfg.dynamicSmemBytes = P.ex_smem;
+    cfg.stream = stream;
+    W2D_CUDA(h, cudaLaunchKernelExC(&cfg, P.ex_fn, args));
     return WAVE2D_OK;
 }
 
-int kernels_per_sweep(const wave2d_t* h, int d) { return h->plan[d].solver == WAVE2D_SOLVER_STREAM ? 1 : 3; }
+int kernels_per_sweep(const wave2d_t* h, int d) { return h->plan[d].solver == WAVE2D_SOLVER_STREAM ? 1 : 2; }
 
 // A chunk of the step loop (A7): `steps` time steps = sweeps n_off = 0 .. 2 steps - 1 relative to the device step
 // counter, then wave2d_end_chunk, which counts them and re-zeroes the counters they used.  The same sequence is
@@ -1203,11 +1256,12 @@ int wave2d_get_info(wave2d_t* h, const char* name, double* value)
     else if (key == "chunks") *value = stream ? (double)P.pieces.size() : 1;
     else if (key == "nbk") *value = stream ? P.nbk : 0;
     else if (key == "kb") *value = stream ? P.kb : 0;
-    else if (key == "grid") *value = stream ? P.grid : (P.nlines + 127) / 128;
+    else if (key == "grid") *value = P.grid;
     else if (key == "ctas_per_sm") *value = stream ? P.ctas_per_sm : 0;
-    else if (key == "smem") *value = stream ? P.var->smem : 0;
-    else if (key == "threads") *value = stream ? P.var->threads : 128;
-    else if (key == "unit") *value = stream ? P.var->unit : 0;
+    else if (key == "smem") *value = stream ? P.var->smem : P.ex_smem;
+    else if (key == "threads") *value = stream ? P.var->threads : EX_NT;
+    else if (key == "unit") *value = stream ? P.var->unit : EX_U;
+    else if (key == "strip") *value = stream ? 0 : P.ex_sc;
     else if (key == "upc") *value = stream ? P.quota * P.var->nw : 0;
     else if (key == "quota") *value = stream ? P.quota : 0;
     else if (key == "static") *value = stream ? P.nstatic : 0;
