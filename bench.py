@@ -54,6 +54,9 @@ def parse_args():
                          "1: factorised unsplit scheme (2.8), 5 field passes per step (SURVEY.md 8f NEXT-2)")
     ap.add_argument("--tau-factor", type=float, default=1.0,
                     help="off-config: multiply the workload's tau (16: alpha = 128, the exact whole-line solvers run)")
+    ap.add_argument("--speed-field", action="store_true",
+                    help="off-config (SURVEY.md 8f NEXT-4): c(t) cs(x,y) with a smooth seeded positive field cs; the "
+                         "variable-coefficient solvers run, 4 field passes per sweep")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps per end-to-end iteration (default: --steps)")
@@ -320,6 +323,12 @@ def run_ours(args):
     if sch:
         h.set_option("scheme", sch)      # factorised (2.8): set_initial stands at level 1, every run step is a solve
     h.set_speed(w.c_half)
+    if args.speed_field:
+        yy = np.linspace(0.0, 1.0, w.n2)[:, None]
+        xx = np.linspace(0.0, 1.0, w.n1)[None, :]
+        cs = 1.0 + 0.4 * np.sin(2 * np.pi * xx) * np.cos(np.pi * yy) + 0.3 * xx - 0.2 * yy
+        h.set_speed_field(cs.astype(npdt))
+        w.name += " with speed field cs(x,y) (off-config)"
     if w.s is not None:
         h.set_source(w.s.astype(npdt, copy=False), w.g_half)
     h.set_initial(phi_pin)
@@ -374,8 +383,10 @@ def run_ours(args):
     dom = "x" if ms_x >= ms_y else "y"
     # algorithmic bytes per launch: read 2 fields, write 1; scheme 1's y sweep reads 1, writes 1
     bytes_x, bytes_y = 3 * fbytes, (2 if sch else 3) * fbytes
+    if args.speed_field:                      # + the speed field in every sweep
+        bytes_x, bytes_y = 4 * fbytes, 4 * fbytes
     sweep_bytes = bytes_x if dom == "x" else bytes_y
-    passes = 5 if sch else 6
+    passes = 8 if args.speed_field else 5 if sch else 6
     step_s = ms * 1e-3 / K
     # The timed region is K steps = K launches of each sweep kernel back to back (graph replay), timed by the two
     # events above.  The dominant kernel's average launch duration in that region is its share of the step (from

@@ -148,6 +148,17 @@ int wave2d_set_state(wave2d_t *h, int k, const void *u_prev_half, const void *u,
 int wave2d_set_speed(wave2d_t *h, const double *c_half, int count);
 
 /*
+ * Spatially varying speed: c(t,x,y) = c_half[n] * cs(x,y), separable like the source below.
+ * cs: interior array, every value > 0 (else ERR_ARG); NULL returns to c = c(t).  Algorithm 1 computes the tridiagonal
+ * elements a_i, b_i, c_i point by point: the weights of (2.11)/(2.12) are taken at the point of the
+ * equation, a_p = tau^2 c_{n+1} cs_p / (2 h_d^2).  The systems are then no longer Toeplitz: every line computes its own
+ * elimination pivots (a scan of linear-fractional maps, csrc/exact.cuh) inside the whole-line solvers, which read one
+ * more field per sweep (32 instead of 24 bytes per point in fp64).  Split scheme only (scheme 1: ERR_UNSUPPORTED), lines
+ * of at most 4096 unknowns (ERR_UNSUPPORTED at the first run otherwise), solver AUTO or EXACT.  Before the first run.
+ */
+int wave2d_set_speed_field(wave2d_t *h, const void *cs, long ld);
+
+/*
  * Source f(t,x,y) = g(t) s(x,y).  s: interior array (NULL clears the source);
  * g_half[n] = g(n tau/2), n = 0..2M-1 (count >= 2M), or NULL for g == 1 (a time-independent full-grid
  * source).  Half-step n uses g_half[n]: f^k in (2.11), f^{k+1/2} in (2.12).

@@ -20,7 +20,7 @@ SOLVER_AUTO, SOLVER_EXACT, SOLVER_STREAM, SOLVER_LINE = 0, 1, 2, 3
 EXPORTS = [
     "wave2d_create", "wave2d_destroy", "wave2d_set_stream", "wave2d_set_option", "wave2d_set_initial",
     "wave2d_set_state",
-    "wave2d_set_speed", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
+    "wave2d_set_speed", "wave2d_set_speed_field", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
     "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
     "wave2d_host_scalars", "wave2d_host_plan", "wave2d_strerror", "wave2d_last_error",
 ]
@@ -56,6 +56,7 @@ def load_library() -> C.CDLL:
     L.wave2d_set_state.argtypes = [vp, C.c_int, vp, vp, C.c_long]
     L.wave2d_set_speed.argtypes = [vp, dp, C.c_int]
     L.wave2d_set_source.argtypes = [vp, vp, C.c_long, dp, C.c_int]
+    L.wave2d_set_speed_field.argtypes = [vp, vp, C.c_long]
     L.wave2d_run.argtypes = [vp, C.c_int]
     L.wave2d_get.argtypes = [vp, vp, C.c_long]
     L.wave2d_get_prev.argtypes = [vp, vp, C.c_long]
@@ -171,6 +172,11 @@ class Wave2D:
         c = np.ascontiguousarray(np.atleast_1d(c_half), dtype=np.float64)
         self._check(self._L.wave2d_set_speed(self._h, c.ctypes.data_as(C.POINTER(C.c_double)), c.shape[0]),
                     "wave2d_set_speed")
+
+    def set_speed_field(self, cs):
+        keep = []
+        p, ld = self._field(cs, keep)
+        self._check(self._L.wave2d_set_speed_field(self._h, p, ld), "wave2d_set_speed_field")
 
     def set_source(self, s, g_half=None):
         keep = []

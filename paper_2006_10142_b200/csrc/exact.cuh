@@ -270,6 +270,112 @@ __device__ __forceinline__ T group_backward(bool fast, T (&y)[U], const T (&cp)[
                 : group_backward_impl<T, U, false>(y, cp, S, xin, wpc, gw, lane, sB, sH);
 }
 
+// ---- variable speed: the pivots of a non-Toeplitz line -------------------------------------------
+// With c(t) cs(x,y) the system of a line is  -a_p x_{p-1} + (gamma + 2 a_p) x_p - a_p x_{p+1} = r_p,  a_p = ap cs_p
+// (Algorithm 1's a_i, b_i, c_i "per point"), and the elimination pivots follow the NONLINEAR recurrence
+//      cp_p = a_p / (b_p - a_p cp_{p-1}),    inv_p = 1 / (b_p - a_p cp_{p-1}),      b_p = gamma + 2 a_p.
+// It is a linear-fractional map of cp_{p-1}, so maps compose as 2x2 matrices: with cp = N / D,
+//      (N, D) <- (a_p D, b_p D - a_p N).
+// A thread multiplies the maps of its U points, the products are scanned over the line exactly like the carries
+// (normalised to [[A, B], [C, 1]] after every product: the maps are projective, and C B' + 1 >= 3/4 by diagonal
+// dominance), and the exclusive prefix applied to the value entering the segment gives every thread its cp_{p0-1}.
+template <typename T>
+struct Mob {
+    T A, B, C;   // [[A, B], [C, 1]]
+};
+template <typename T>
+__device__ __forceinline__ T rcpT(T x) { return T(1) / x; }
+// `later` after `earlier`
+template <typename T>
+__device__ __forceinline__ Mob<T> mob_after(const Mob<T>& later, const Mob<T>& earlier)
+{
+    const T d = rcpT(fmaT(later.C, earlier.B, T(1)));
+    Mob<T> r;
+    r.A = fmaT(later.A, earlier.A, later.B * earlier.C) * d;
+    r.B = fmaT(later.A, earlier.B, later.B) * d;
+    r.C = fmaT(later.C, earlier.A, earlier.C) * d;
+    return r;
+}
+template <typename T>
+__device__ __forceinline__ T mob_apply(const Mob<T>& m, T c) { return fmaT(m.A, c, m.B) * rcpT(fmaT(m.C, c, T(1))); }
+
+// a[]: this thread's a_p (0 beyond the line).  cin: cp just before the segment.  Fills cp[], iv[]; returns cp at the end
+// of the segment.  sM: the group's slice [3][wpc] of a CTA array (one CTA barrier inside; every thread must call).
+template <typename T, int U>
+__device__ __forceinline__ T group_pivots(const T (&a)[U], T gamma, T (&cp)[U], T (&iv)[U], T cin, int wpc, int gw,
+                                          int lane, T* sMA, T* sMB, T* sMC)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    // the unit's map: rows (n0, n1), (d0, d1) of N and D as linear forms of the (N, D) entering the unit
+    T n0 = T(1), n1 = T(0), d0 = T(0), d1 = T(1);
+#pragma unroll
+    for (int e = 0; e < U; ++e) {
+        const T b = fmaT(T(2), a[e], gamma);
+        const T m0 = a[e] * d0, m1 = a[e] * d1;
+        d0 = fmaT(b, d0, -(a[e] * n0));
+        d1 = fmaT(b, d1, -(a[e] * n1));
+        n0 = m0;
+        n1 = m1;
+        if ((e & 3) == 3) {                      // keep the entries in range (fp32: b^8 may not fit)
+            const T sc = rcpT(d1);
+            n0 *= sc; n1 *= sc; d0 *= sc; d1 = T(1);
+        }
+    }
+    Mob<T> m{n0, n1, d0};                        // (d1 == 1 after the last normalisation: U is a multiple of 4)
+    static_assert(U % 4 == 0, "the unit map is normalised every 4 points");
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {           // inclusive scan over the lanes
+        Mob<T> o;
+        o.A = __shfl_up_sync(FULL, m.A, d);
+        o.B = __shfl_up_sync(FULL, m.B, d);
+        o.C = __shfl_up_sync(FULL, m.C, d);
+        if (lane >= d) m = mob_after(m, o);
+    }
+    if (lane == 31) {
+        sMA[gw] = m.A;
+        sMB[gw] = m.B;
+        sMC[gw] = m.C;
+    }
+    named_bar_sync(1, EX_NT);
+    Mob<T> g;
+    g.A = lane < wpc ? sMA[lane] : T(1);
+    g.B = lane < wpc ? sMB[lane] : T(0);
+    g.C = lane < wpc ? sMC[lane] : T(0);
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {           // inclusive scan over the warps of the group (identity beyond wpc)
+        Mob<T> o;
+        o.A = __shfl_up_sync(FULL, g.A, d);
+        o.B = __shfl_up_sync(FULL, g.B, d);
+        o.C = __shfl_up_sync(FULL, g.C, d);
+        if (lane >= d) g = mob_after(g, o);
+    }
+    const int gp = gw > 0 ? gw - 1 : 0;
+    Mob<T> pw;                                   // everything before this warp
+    pw.A = __shfl_sync(FULL, g.A, gp);
+    pw.B = __shfl_sync(FULL, g.B, gp);
+    pw.C = __shfl_sync(FULL, g.C, gp);
+    const T cw = gw == 0 ? cin : mob_apply(pw, cin);
+    Mob<T> all;
+    all.A = __shfl_sync(FULL, g.A, wpc - 1);
+    all.B = __shfl_sync(FULL, g.B, wpc - 1);
+    all.C = __shfl_sync(FULL, g.C, wpc - 1);
+    const T cout = mob_apply(all, cin);
+    Mob<T> pl;                                   // the lanes before this one
+    pl.A = __shfl_up_sync(FULL, m.A, 1);
+    pl.B = __shfl_up_sync(FULL, m.B, 1);
+    pl.C = __shfl_up_sync(FULL, m.C, 1);
+    T c = lane == 0 ? cw : mob_apply(pl, cw);    // cp_{p0 - 1}
+#pragma unroll
+    for (int e = 0; e < U; ++e) {
+        const T b = fmaT(T(2), a[e], gamma);
+        const T v = rcpT(fmaT(-a[e], c, b));
+        c = a[e] * v;
+        cp[e] = c;
+        iv[e] = v;
+    }
+    return cout;
+}
+
 struct ExactArgs {
     FieldSet fs;
     const double* table;
@@ -288,6 +394,8 @@ struct ExactArgs {
     int wpc;               // warps per line (group size); EX_NW / wpc lines per CTA pass
     int nseg;              // x: segments of wpc * 32 * U points per line (nseg > 1 only with wpc == EX_NW)
     int sc;                // y: columns per strip
+    const void* cs;        // VAR kernels: spatial speed factor (pitched like a field, pad 0)
+    double gamma;          // VAR kernels: the time-quotient constant (b_p = gamma + 2 a_p)
 };
 
 template <typename T>
@@ -327,7 +435,8 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 //   nseg == 1: two prefetch slots of EX_NT * (2 NV + 1) 16-byte cells -- while a pass is solved, every thread's own
 //              points of the next pass's row (and the two neighbour values of a warp) are already on their way;
 //   nseg  > 1: the parked line, nseg * wpc * 32 * U values (no prefetch: the line itself fills shared memory).
-template <typename T>
+// VAR: variable speed -- one more field (cs) per row, the pivots come from group_pivots, no stationary fast path.
+template <typename T, bool VAR>
 __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ ExactArgs a)
 {
     constexpr int U = EX_U, V = 16 / (int)sizeof(T), NV = U / V;
@@ -337,6 +446,7 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
     // aggregates of the block-wide scans, double-buffered: consecutive forward (or backward) calls alternate, so a warp
     // that runs ahead into the next call never overwrites what a slower warp still reads (one barrier per call)
     __shared__ T s_agg[2][4][EX_NW];
+    __shared__ T s_mob[VAR ? 2 : 1][3][EX_NW];   // aggregates of the pivot scan (VAR), double-buffered likewise
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wpc = a.wpc, group = warp / wpc, gw = warp % wpc, ngroups = EX_NW / wpc;
@@ -345,13 +455,16 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
     const T* const prev = static_cast<const T*>(a.fs.b[R.prev]);
     const T* const cur = static_cast<const T*>(a.fs.b[R.cur]);
     T* const out = static_cast<T*>(a.fs.b[R.out]);
+    [[maybe_unused]] const T* const csf = static_cast<const T*>(a.cs);
     const double* row = a.table + static_cast<size_t>(a.period ? nh % a.period : nh) * ROW_DOUBLES;
     const T am = static_cast<T>(row[ROW_AM]), q = static_cast<T>(row[ROW_Q]), c1 = static_cast<T>(row[ROW_C1]);
+    [[maybe_unused]] const T ap = static_cast<T>(row[ROW_AP]), gam = static_cast<T>(a.gamma);
     const T g2 = static_cast<T>(a.g2);
     const bool one = a.one != 0;
     const int n = a.n, seg_pts = wpc * 32 * U;
     const T* const src = static_cast<const T*>(a.src);
     int pf = 0, pb = 0;   // buffer parity of the next forward / backward call
+    [[maybe_unused]] int pp = 0;
 
     auto pivots = [&](int p0, T (&cp)[U], T (&iv)[U]) {
 #pragma unroll
@@ -363,10 +476,11 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
     };
     Stat<T, U> S;
     S.init(row[ROW_RHO], row[ROW_INV], lane);
-    const int pc = *a.conv;                       // pivots are the fixed point from here on
+    const int pc = VAR ? 0x7fffffff : *a.conv;    // pivots are the fixed point from here on (never, with a variable speed)
 
-    // prefetch (nseg == 1): cell c of slot s of this thread; cells [0, NV): prev, [NV, 2 NV): cur, 2 NV: neighbour of the warp
-    constexpr int CELLS = 2 * NV + 1;
+    // prefetch (nseg == 1): cell c of slot s of this thread; cells [0, NV): prev, [NV, 2 NV): cur, (VAR: [2 NV, 3 NV): cs,)
+    // last: neighbour of the warp
+    constexpr int CELLS = (VAR ? 3 : 2) * NV + 1;
     const bool pre = a.nseg == 1;
     auto cell = [&](int slot, int c) -> unsigned char* {
         return ex_smem + ((static_cast<size_t>(slot) * CELLS + c) * EX_NT + threadIdx.x) * 16;
@@ -380,9 +494,10 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
             for (int c = 0; c < NV; ++c) {
                 if (!one) cp_async16(cell(slot, c), prev + rn + c * V);
                 cp_async16(cell(slot, NV + c), cur + rn + c * V);
+                if constexpr (VAR) cp_async16(cell(slot, 2 * NV + c), csf + rn + c * V);
             }
-            if (!one && lane == 0 && q0 > 0) cp_async_small<sizeof(T)>(cell(slot, 2 * NV), prev + rn - 1);
-            if (!one && lane == 31 && q0 + U < a.pitch) cp_async_small<sizeof(T)>(cell(slot, 2 * NV), prev + rn + U);
+            if (!one && lane == 0 && q0 > 0) cp_async_small<sizeof(T)>(cell(slot, CELLS - 1), prev + rn - 1);
+            if (!one && lane == 31 && q0 + U < a.pitch) cp_async_small<sizeof(T)>(cell(slot, CELLS - 1), prev + rn + U);
         }
         cp_async_commit();
     };
@@ -400,10 +515,11 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
             const int p0 = s * seg_pts + (gw * 32 + lane) * U;
             const int w0 = s * seg_pts + gw * 32 * U;                  // first point of this warp
             const bool fast = live && w0 >= pc && w0 + 32 * U <= n;     // 32 whole stationary units (warp-uniform)
-            if (!fast) pivots(p0, cp, iv);
+            if (!VAR && !fast) pivots(p0, cp, iv);
             T wp[U], wc[U];
+            [[maybe_unused]] T wa[U];                   // VAR: cs, then a_p = ap cs_p
 #pragma unroll
-            for (int e = 0; e < U; ++e) wp[e] = wc[e] = T(0);
+            for (int e = 0; e < U; ++e) wp[e] = wc[e] = wa[e] = T(0);
             const bool inrow = live && p0 < a.pitch;   // (pad columns inside the pitch are zero)
             T edge = T(0);                              // lane 0: the point before the warp's first, lane 31: after its last
             if (pre) {
@@ -414,15 +530,17 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
                     for (int c = 0; c < NV; ++c) {
                         if (!one) ld16(reinterpret_cast<const T*>(cell(it & 1, c)), wp + c * V);
                         ld16(reinterpret_cast<const T*>(cell(it & 1, NV + c)), wc + c * V);
+                        if constexpr (VAR) ld16(reinterpret_cast<const T*>(cell(it & 1, 2 * NV + c)), wa + c * V);
                     }
                     if (!one && ((lane == 0 && p0 > 0) || (lane == 31 && p0 + U < a.pitch)))
-                        edge = *reinterpret_cast<const T*>(cell(it & 1, 2 * NV));
+                        edge = *reinterpret_cast<const T*>(cell(it & 1, CELLS - 1));
                 }
             } else if (inrow) {
 #pragma unroll
                 for (int c = 0; c < NV; ++c) {
                     if (!one) ld16(prev + ro + p0 + c * V, wp + c * V);
                     ld16(cur + ro + p0 + c * V, wc + c * V);
+                    if constexpr (VAR) ld16(csf + ro + p0 + c * V, wa + c * V);
                 }
                 if (!one && lane == 0 && p0 > 0) edge = prev[ro + p0 - 1];
                 if (!one && lane == 31 && p0 + U < a.pitch) edge = prev[ro + p0 + U];
@@ -437,7 +555,12 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
 #pragma unroll
                 for (int e = 0; e < U; ++e) {     // A1: right-hand side of (2.11)
                     const T left = e == 0 ? wl : wp[e - 1], right = e == U - 1 ? wr : wp[e + 1];
-                    y[e] = fmaT(g2, wc[e], fmaT(am, left + right, c1 * wp[e]));
+                    if constexpr (VAR) {           // am_p = am cs_p at the point of the equation
+                        const T amp = am * wa[e];
+                        y[e] = fmaT(g2, wc[e], fmaT(amp, left + right, -fmaT(T(2), amp, gam) * wp[e]));
+                    } else {
+                        y[e] = fmaT(g2, wc[e], fmaT(am, left + right, c1 * wp[e]));
+                    }
                 }
                 if (src_row && p0 < a.sp0 + a.snp && p0 + U > a.sp0) {
 #pragma unroll
@@ -446,6 +569,13 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
                         if (ps >= 0 && ps < a.snp) y[e] = fmaT(q, src[static_cast<size_t>(ps) * a.snl + (j - a.sl0)], y[e]);
                     }
                 }
+            }
+            if constexpr (VAR) {                   // this line's own pivots (host: nseg == 1 with a variable speed)
+#pragma unroll
+                for (int e = 0; e < U; ++e) wa[e] = p0 + e < n ? ap * wa[e] : T(0);
+                group_pivots<T, U>(wa, gam, cp, iv, T(0), wpc, gw, lane, &s_mob[pp][0][group * wpc],
+                                   &s_mob[pp][1][group * wpc], &s_mob[pp][2][group * wpc]);
+                pp ^= 1;
             }
             carry = group_forward<T, U>(fast, y, cp, iv, S, carry, wpc, gw, lane, &s_agg[pf][0][group * wpc],
                                         &s_agg[pf][1][group * wpc]);
@@ -479,13 +609,15 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
 // ---- y half-step: (A3 + A4) exact ------------------------------------------------------------------------------
 // A strip: columns [c0, c0 + sc) over all n rows.  Shared memory: strip[sc][units * (U + 1)] (a unit of U rows is U + 1
 // apart: a warp reading one row offset of 32 consecutive units touches 32 distinct bank pairs).
-template <typename T>
+// VAR: a second strip holds a_p = ap cs_p (the solve needs it along the column), so strips are half as wide.
+template <typename T, bool VAR>
 __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ ExactArgs a)
 {
     constexpr int U = EX_U, V = 16 / (int)sizeof(T);
     extern __shared__ __align__(16) unsigned char ex_smem[];
     T* const strip = reinterpret_cast<T*>(ex_smem);
     __shared__ T s_agg[2][4][EX_NW];   // double-buffered like in wave2d_exact_x
+    __shared__ T s_mob[VAR ? 2 : 1][3][EX_NW];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wpc = a.wpc, group = warp / wpc, gw = warp % wpc, ngroups = EX_NW / wpc;
@@ -503,9 +635,13 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
     const int seg_units = wpc * 32, nseg = (units + seg_units - 1) / seg_units;
     const T* const src = static_cast<const T*>(a.src);
     int pf = 0, pb = 0;
+    [[maybe_unused]] int pp = 0;
     Stat<T, U> S;
     S.init(row[ROW_RHO], row[ROW_INV], lane);
-    const int pc = *a.conv;
+    const int pc = VAR ? 0x7fffffff : *a.conv;
+    [[maybe_unused]] const T* const csf = static_cast<const T*>(a.cs);
+    [[maybe_unused]] const T ap = static_cast<T>(row[ROW_AP]), gam = static_cast<T>(a.gamma);
+    [[maybe_unused]] T* const strip_a = strip + static_cast<size_t>(sc) * cpitch;   // VAR: a_p, same layout
     const int ve = sc < V ? sc : V;                  // elements a loader thread moves per access
     const int kcn = sc / ve;                         // accesses per strip row
 
@@ -517,14 +653,20 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
         const int total = n * kcn;
         for (int i0 = threadIdx.x; i0 < total; i0 += EX_NT * UN) {
             T vc[UN][V], vm[UN][V], vu[UN][V], vd[UN][V];
+            [[maybe_unused]] T vs[UN][V];
 #pragma unroll
             for (int k = 0; k < UN; ++k) {
 #pragma unroll
-                for (int e = 0; e < V; ++e) vc[k][e] = vm[k][e] = vu[k][e] = vd[k][e] = T(0);
+                for (int e = 0; e < V; ++e) vc[k][e] = vm[k][e] = vu[k][e] = vd[k][e] = vs[k][e] = T(0);
                 const int idx = i0 + k * EX_NT;
                 if (idx < total) {
                     const int r = idx / kcn, kc = idx % kcn;
                     const long long o = static_cast<long long>(r) * a.pitch + c0 + kc * ve;   // inside the pitch (pad columns are zero)
+                    if constexpr (VAR) {
+                        if (ve == V) ld16(csf + o, vs[k]);
+                        else
+                            for (int e = 0; e < ve; ++e) vs[k][e] = csf[o + e];
+                    }
                     if (ve == V) {
                         ld16(cur + o, vc[k]);
                         if (!one) {
@@ -554,7 +696,14 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
                     for (int e = 0; e < V; ++e) {
                         if (e < ve) {
                             const int col = c0 + kc * ve + e;
-                            T rv = one ? vc[k][e] : fmaT(g2, vc[k][e], fmaT(am, vu[k][e] + vd[k][e], c1 * vm[k][e]));
+                            T rv;
+                            if constexpr (VAR) {   // am_p = am cs_p at the point of the equation
+                                const T amp = am * vs[k][e];
+                                rv = fmaT(g2, vc[k][e], fmaT(amp, vu[k][e] + vd[k][e], -fmaT(T(2), amp, gam) * vm[k][e]));
+                                strip_a[(kc * ve + e) * cpitch + r + r / U] = ap * vs[k][e];
+                            } else {
+                                rv = one ? vc[k][e] : fmaT(g2, vc[k][e], fmaT(am, vu[k][e] + vd[k][e], c1 * vm[k][e]));
+                            }
                             if (src_r && col >= a.sl0 && col < a.sl0 + a.snl)
                                 rv = fmaT(q, src[static_cast<size_t>(r - a.sp0) * a.snl + (col - a.sl0)], rv);
                             strip[(kc * ve + e) * cpitch + r + r / U] = rv;
@@ -578,11 +727,20 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
 #pragma unroll
                 for (int e = 0; e < U; ++e) {
                     const bool in = live && p0 + e < n;
-                    if (!fast) {
+                    if (!VAR && !fast) {
                         cp[e] = p0 + e < n ? static_cast<T>(a.cpv[p0 + e]) : T(0);
                         iv[e] = p0 + e < n ? static_cast<T>(a.ivv[p0 + e]) : T(0);
                     }
                     y[e] = in ? line[u * (U + 1) + e] : T(0);
+                }
+                if constexpr (VAR) {               // this column's own pivots (host: nseg == 1 with a variable speed)
+                    T wa[U];
+#pragma unroll
+                    for (int e = 0; e < U; ++e)
+                        wa[e] = live && p0 + e < n ? strip_a[static_cast<size_t>(col) * cpitch + u * (U + 1) + e] : T(0);
+                    group_pivots<T, U>(wa, gam, cp, iv, T(0), wpc, gw, lane, &s_mob[pp][0][group * wpc],
+                                       &s_mob[pp][1][group * wpc], &s_mob[pp][2][group * wpc]);
+                    pp ^= 1;
                 }
                 carry = group_forward<T, U>(fast, y, cp, iv, S, carry, wpc, gw, lane, &s_agg[pf][0][group * wpc],
                                             &s_agg[pf][1][group * wpc]);

@@ -145,6 +145,8 @@ struct wave2d_s {
     bool v_ready = false;                // scheme 1: V^0, V^1 computed from U^0, U^1 (needs the final c samples)
     void* buf[4] = {nullptr, nullptr, nullptr, nullptr};   // scheme 0 uses 3
     std::vector<double> c_half, g_half;  // g_half empty: g == 1
+    bool have_cs = false;                // spatial speed factor set (wave2d_set_speed_field): variable-coefficient solvers
+    void* d_cs = nullptr;                // pitched like a field, pad 0
     bool have_src = false;
     void* src_dev[2] = {nullptr, nullptr};    // [0]: x sweep (transposed window), [1]: y sweep (natural window)
     int win_i0 = 0, win_j0 = 0, win_w = 0, win_h = 0;
@@ -444,25 +446,34 @@ int plan_exact(wave2d_t* h, int d)
     int wpc = 1;
     while (wpc < EX_NW && wpc * 32 < units) wpc *= 2;        // power of two, so that it divides EX_NW
     const int nseg = (units + wpc * 32 - 1) / (wpc * 32);
-    const size_t budget = 200 * 1024;
+    const bool var = h->have_cs;
+    if (var && nseg > 1) {
+        h->err = "variable speed: lines of more than 4096 unknowns are not supported yet";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    const size_t budget = (var ? 224 : 200) * 1024;
     P.ex_wpc = wpc;
     if (d == 0) {
         P.ex_nseg = nseg;
         P.ex_sc = 0;
-        // nseg > 1: the parked line; else the two prefetch slots of (2 NV + 1) 16-byte cells per thread
+        // nseg > 1: the parked line; else the two prefetch slots of (2 NV + 1) 16-byte cells per thread (3 NV + 1 with cs)
         const size_t smem = nseg > 1 ? (size_t)nseg * wpc * 32 * EX_U * h->elem
-                                     : (size_t)2 * (2 * (EX_U * h->elem / 16) + 1) * EX_NT * 16;
+                                     : (size_t)2 * ((var ? 3 : 2) * (EX_U * h->elem / 16) + 1) * EX_NT * 16;
         if (smem > budget) {
             h->err = "exact solver: an x line of more than 25600 fp64 unknowns does not fit shared memory";
             return WAVE2D_ERR_UNSUPPORTED;
         }
         P.ex_smem = (int)smem;
-        P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double>)
-                                         : reinterpret_cast<const void*>(&wave2d_exact_x<float>);
+        if (var)
+            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, true>)
+                                             : reinterpret_cast<const void*>(&wave2d_exact_x<float, true>);
+        else
+            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, false>)
+                                             : reinterpret_cast<const void*>(&wave2d_exact_x<float, false>);
         const int passes = (P.nlines + EX_NW / wpc - 1) / (EX_NW / wpc);
         P.grid = std::max(1, std::min(passes, 4 * h->num_sms));
     } else {
-        const size_t col = (size_t)units * (EX_U + 1) * h->elem;   // one column of the strip
+        const size_t col = (size_t)units * (EX_U + 1) * h->elem * (var ? 2 : 1);   // one column of the strip (+ its a_p)
         int sc = 16;
         while (sc > 1 && sc * col > budget) sc /= 2;
         if (sc * col > budget) {
@@ -473,8 +484,12 @@ int plan_exact(wave2d_t* h, int d)
         P.ex_sc = sc;
         P.ex_nseg = nseg;
         P.ex_smem = (int)(sc * col);
-        P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double>)
-                                         : reinterpret_cast<const void*>(&wave2d_exact_y<float>);
+        if (var)
+            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, true>)
+                                             : reinterpret_cast<const void*>(&wave2d_exact_y<float, true>);
+        else
+            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, false>)
+                                             : reinterpret_cast<const void*>(&wave2d_exact_y<float, false>);
         const int strips = (P.nlines + sc - 1) / sc;
         P.grid = std::max(1, std::min(strips, 4 * h->num_sms));
     }
@@ -525,7 +540,11 @@ int plan_dir(wave2d_t* h, int d)
     P.halo = H;
     const int nbk = (H + U - 1) / U;
     const bool fits = nbk <= std::min(NBK_MAX, V.nw) && pconv <= KMAX;
-    if (h->opt_solver == WAVE2D_SOLVER_EXACT || (h->opt_solver == WAVE2D_SOLVER_AUTO && !fits)) {
+    if (h->have_cs && h->opt_solver == WAVE2D_SOLVER_STREAM) {
+        h->err = "variable speed: the streamed kernels assume Toeplitz systems (use solver AUTO or EXACT)";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    if (h->have_cs || h->opt_solver == WAVE2D_SOLVER_EXACT || (h->opt_solver == WAVE2D_SOLVER_AUTO && !fits)) {
         P.solver = WAVE2D_SOLVER_EXACT;
         return plan_exact(h, d);
     }
@@ -577,7 +596,11 @@ int plan_line(wave2d_t* h)
         h->err = "solver LINE: more than 256 unknowns per line";
         return WAVE2D_ERR_UNSUPPORTED;
     }
-    if (!fits || (h->opt_solver != WAVE2D_SOLVER_AUTO && h->opt_solver != WAVE2D_SOLVER_LINE)) return WAVE2D_OK;
+    if (h->have_cs && h->opt_solver == WAVE2D_SOLVER_LINE) {
+        h->err = "variable speed: the small-grid kernel assumes Toeplitz systems (use solver AUTO or EXACT)";
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    if (!fits || h->have_cs || (h->opt_solver != WAVE2D_SOLVER_AUTO && h->opt_solver != WAVE2D_SOLVER_LINE)) return WAVE2D_OK;
     const int U = nmax <= 32 * 4 ? 4 : 8;
     h->line_unit = U;
     if (h->dtype == WAVE2D_F64) h->line_fn = U == 4 ? line_kernel<double, 4>() : line_kernel<double, 8>();
@@ -774,9 +797,12 @@ int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own
     double* cpv = h->d_piv;
     double* ivv = h->d_piv + std::max(h->n1, h->n2);
     int* conv = reinterpret_cast<int*>(h->d_piv + 2 * (size_t)std::max(h->n1, h->n2));
-    wave2d_exact_pivots<<<1, 256, 0, stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv, conv);
+    if (!h->have_cs)   // (with a variable speed every line computes its own pivots inside the solver)
+        wave2d_exact_pivots<<<1, 256, 0, stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv, conv);
     ExactArgs a;
     a.conv = conv;
+    a.cs = h->d_cs;
+    a.gamma = h->gamma;
     a.fs = field_set(h);
     a.table = h->d_table; a.period = h->table_period; a.d_k = dk; a.n_off = n_off;
     a.n = P.n; a.nlines = P.nlines; a.pitch = h->pitch; a.cpv = cpv; a.ivv = ivv;
@@ -794,7 +820,10 @@ int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own
     return WAVE2D_OK;
 }
 
-int kernels_per_sweep(const wave2d_t* h, int d) { return h->plan[d].solver == WAVE2D_SOLVER_STREAM ? 1 : 2; }
+int kernels_per_sweep(const wave2d_t* h, int d)
+{
+    return h->plan[d].solver == WAVE2D_SOLVER_STREAM || h->have_cs ? 1 : 2;   // exact: pivots + solver
+}
 
 // A chunk of the step loop (A7): `steps` time steps = sweeps n_off = 0 .. 2 steps - 1 relative to the device step
 // counter, then wave2d_end_chunk, which counts them and re-zeroes the counters they used.  The same sequence is
@@ -803,8 +832,8 @@ int launch_chunk(wave2d_t* h, cudaStream_t stream, int steps)
 {
     int st = WAVE2D_OK;
     for (int s = 0; s < steps && st == WAVE2D_OK; ++s) {
-        st = launch_half_step(h, stream, 2 * s, s > 0 && kernels_per_sweep(h, 1) == 1);
-        if (st == WAVE2D_OK) st = launch_half_step(h, stream, 2 * s + 1, kernels_per_sweep(h, 0) == 1);
+        st = launch_half_step(h, stream, 2 * s, s > 0 && h->plan[1].solver == WAVE2D_SOLVER_STREAM);
+        if (st == WAVE2D_OK) st = launch_half_step(h, stream, 2 * s + 1, h->plan[0].solver == WAVE2D_SOLVER_STREAM);
     }
     if (st) return st;
     wave2d_end_chunk<<<1, 2 * SLOTS, 0, stream>>>(h->d_k, steps, h->d_tickets);
@@ -979,6 +1008,7 @@ void wave2d_destroy(wave2d_t* h)
     for (int b = 0; b < 4; ++b) cudaFree(h->buf[b]);
     cudaFree(h->src_dev[0]);
     cudaFree(h->src_dev[1]);
+    cudaFree(h->d_cs);
     cudaFree(h->d_table);
     cudaFree(h->d_k);
     cudaFree(h->d_piv);
@@ -1010,6 +1040,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "kappa")) h->kappa = value;
     else if (!strcmp(name, "scheme")) {
         if ((iv != 0 && iv != 1) || h->have_initial) return WAVE2D_ERR_ARG;
+        if (iv == 1 && h->have_cs) return WAVE2D_ERR_UNSUPPORTED;   // variable speed: split scheme only
         if (iv == 1 && !h->buf[3]) {
             const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
             int st = dev_alloc(h, &h->buf[3], fbytes);
@@ -1094,6 +1125,37 @@ int wave2d_set_speed(wave2d_t* h, const double* c_half, int count)
         if (!(c_half[n] > 0.0)) return WAVE2D_ERR_ARG;   // PAPER.md:31, "positive speed function"
     for (int n = 0; n <= 2 * h->M; ++n) h->c_half[n] = count == 1 ? c_half[0] : c_half[n];
     invalidate_plan(h);
+    return WAVE2D_OK;
+}
+
+int wave2d_set_speed_field(wave2d_t* h, const void* cs, long ld)
+{
+    if (!h) return WAVE2D_ERR_ARG;
+    if (h->ran) return WAVE2D_ERR_STATE;
+    if (cs && (ld < h->n1 || h->scheme == 1)) return h->scheme == 1 ? WAVE2D_ERR_UNSUPPORTED : WAVE2D_ERR_ARG;
+    invalidate_plan(h);
+    h->have_cs = false;
+    if (!cs) return WAVE2D_OK;
+    const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
+    if (!h->d_cs) {
+        int st = dev_alloc(h, &h->d_cs, fbytes);
+        if (st) return st;
+    }
+    W2D_CUDA(h, cudaMemsetAsync(h->d_cs, 0, fbytes, h->stream));
+    int st = copy_in(h, h->d_cs, cs, ld);
+    if (st) return st;
+    // every value must be positive: checked on a host copy
+    const size_t e = h->elem, n1 = h->n1, n2 = h->n2;
+    std::vector<unsigned char> host(n1 * n2 * e);
+    W2D_CUDA(h, cudaMemcpy2DAsync(host.data(), n1 * e, h->d_cs, (size_t)h->pitch * e, n1 * e, n2, cudaMemcpyDeviceToHost,
+                                  h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    for (size_t i = 0; i < n1 * n2; ++i) {
+        const double v = h->dtype == WAVE2D_F64 ? reinterpret_cast<const double*>(host.data())[i]
+                                                : (double)reinterpret_cast<const float*>(host.data())[i];
+        if (!(v > 0.0)) return WAVE2D_ERR_ARG;
+    }
+    h->have_cs = true;
     return WAVE2D_OK;
 }
 
@@ -1310,7 +1372,7 @@ int wave2d_profile_sweeps(wave2d_t* h, int steps, double* ms_x, double* ms_y)
         st = launch_half_step(h, h->stream, 0, false);
         if (st) return st;
         W2D_CUDA(h, cudaEventRecord(ev[3 * s + 1], h->stream));
-        st = launch_half_step(h, h->stream, 1, kernels_per_sweep(h, 0) == 1);
+        st = launch_half_step(h, h->stream, 1, h->plan[0].solver == WAVE2D_SOLVER_STREAM);
         if (st) return st;
         W2D_CUDA(h, cudaEventRecord(ev[3 * s + 2], h->stream));
         wave2d_end_chunk<<<1, 2 * SLOTS, 0, h->stream>>>(h->d_k, 1, h->d_tickets);

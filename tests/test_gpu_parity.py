@@ -812,3 +812,111 @@ def test_exact_solver_full_grid_tau_16h():
     assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
     assert info["strip_y"] == 4                           # 4 columns x 4095 rows x (9/8) x 8 B = 147 KB on chip
     assert relerr(u, r) <= 1e-10
+
+
+# ---- variable speed c(t) cs(x,y): per-line pivots by a scan of linear-fractional maps -------------
+def _speed_field(rng, shape, lo=0.4, hi=2.2):
+    """Smooth + rough positive field: a few random Fourier modes plus point noise."""
+    n2, n1 = shape
+    y = np.linspace(0, 1, n2)[:, None]
+    x = np.linspace(0, 1, n1)[None, :]
+    f = 1.0 + 0.4 * np.sin(2 * np.pi * x * rng.integers(1, 4)) * np.cos(np.pi * y * rng.integers(1, 4)) + 0.3 * x - 0.2 * y
+    f = f + 0.15 * rng.uniform(-1, 1, shape)
+    return np.clip(f, lo, hi)
+
+
+def gpu_var(w, cs, **opts):
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+    try:
+        for k, v in opts.items():
+            h.set_option(k, v)
+        npdt = np.float64 if w.dtype == "f64" else np.float32
+        h.set_speed(w.c_half)
+        h.set_speed_field(cs.astype(npdt))
+        if w.s is not None:
+            h.set_source(w.s.astype(npdt), w.g_half)
+        h.set_initial(w.phi.astype(npdt), None if w.psi is None else w.psi.astype(npdt))
+        h.run(w.M)
+        u = h.get()
+        info = {k: h.info(k) for k in ("solver_x", "solver_y", "launches", "strip_y")}
+    finally:
+        h.close()
+    return u, info
+
+
+@pytest.mark.parametrize("N1,N2", [(2, 2), (3, 9), (9, 3), (17, 16), (33, 34), (130, 66), (257, 40), (40, 257), (300, 260),
+                                   (1030, 270), (270, 1030), (4096, 24), (24, 4096), (2050, 2050)])
+@pytest.mark.parametrize("ratio", [0.9, 3.0, 16.0])
+def test_variable_speed_matches_oracle(N1, N2, ratio):
+    """Random positive speed field, time-varying c(t), source, psi != 0; tau = 0.9 h, 3 h and 16 h (the pivot scan is exact
+    for any tau).  Element by element against the oracle's variable-speed mode; fp64 and fp32."""
+    M = 5 if max(N1, N2) < 2000 else 3
+    rng = np.random.default_rng(N1 * 13 + N2 + int(ratio))
+    tau = ratio / max(N1, N2)
+    shape = (N2 - 1, N1 - 1)
+    phi, psi, s = (rng.uniform(-1, 1, shape) for _ in range(3))
+    c = rng.uniform(0.7, 1.3, 2 * M + 1)
+    g = rng.uniform(-1, 1, 2 * M)
+    cs = _speed_field(rng, shape)
+    alpha = 0.5 * ratio ** 2 * 1.3 * 2.2 * (max(N1, N2) / min(N1, N2)) ** 0       # along the long direction
+    for dtype, tol in (("f64", 1e-10), ("f32", max(1e-4, 12 * (1.0 + 2.0 * alpha) * 6e-8 * 4))):
+        w = W.Workload("var", N1, N2, 1.0, tau, M, dtype, phi, psi, c, s=s, g_half=g)
+        npdt = np.float64 if dtype == "f64" else np.float32
+        cast = lambda a: a.astype(npdt).astype(np.float64)
+        r = oracle.solve(N1, N2, 1.0, tau, M, cast(phi), cast(psi), c_half=c, s=cast(s), g_half=g, cs=cast(cs))
+        u, info = gpu_var(w, cs)
+        assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
+        assert info["launches"] == 2 * M + 2      # one kernel per sweep; two chunks (2 + 1 or 4 + 1 steps)
+        assert relerr(u, r) <= tol, (dtype, relerr(u, r))
+
+
+def test_variable_speed_constant_field_and_state_machine():
+    w = W.cfg2(N=300, M=12)
+    ones = np.full(w.phi.shape, 1.25)
+    u, _ = gpu_var(w, ones)
+    w2 = W.cfg2(N=300, M=12)
+    w2.c_half = 1.25 * w.c_half
+    v, info = gpu(w2, solver=B.SOLVER_EXACT)
+    assert relerr(u, v) <= 1e-12                       # cs == const is the Toeplitz problem with c scaled
+    h = B.Wave2D(32, 32, 1.0, 0.01, 4)
+    try:
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_speed_field(np.zeros((31, 31)))      # must be positive (PAPER.md:31)
+        assert e.value.status == -1
+        h.set_speed_field(np.ones((31, 31)))
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_option("scheme", 1)                  # split scheme only
+        assert e.value.status == -5
+        h.set_option("solver", B.SOLVER_STREAM)
+        h.set_initial(np.ones((31, 31)))
+        with pytest.raises(B.Wave2DError) as e:
+            h.run(1)                                   # the streamed kernels assume Toeplitz systems
+        assert e.value.status == -5
+        h.set_speed_field(None)                        # back to c = c(t)
+        h.run(1)
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_speed_field(np.ones((31, 31)))       # not after the first run
+        assert e.value.status == -2
+    finally:
+        h.close()
+    big = B.Wave2D(4200, 16, 1.0, 0.01, 2)
+    try:
+        big.set_speed_field(np.ones((15, 4199)))
+        big.set_initial(np.ones((15, 4199)))
+        with pytest.raises(B.Wave2DError) as e:
+            big.run(1)                                 # lines of more than 4096 unknowns: not yet
+        assert e.value.status == -5
+    finally:
+        big.close()
+
+
+def test_variable_speed_full_grid_4095():
+    M = 4
+    w = W.cfg3(N=4096, M=M)
+    w.phi = W.cfg2(N=4096, M=1).phi
+    w.g_half = W.ricker(W.half_times(w.tau, 2 * M) + 0.058)
+    cs = _speed_field(np.random.default_rng(5), w.phi.shape)
+    r = oracle.solve(w.N1, w.N2, w.l, w.tau, M, w.phi, None, c_half=w.c_half, s=w.s, g_half=w.g_half, cs=cs)
+    u, info = gpu_var(w, cs)
+    assert info["strip_y"] == 2                          # r and a_p of 2 columns x 4095 rows on chip
+    assert relerr(u, r) <= 1e-10
