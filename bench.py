@@ -57,6 +57,10 @@ def parse_args():
     ap.add_argument("--speed-field", action="store_true",
                     help="off-config (SURVEY.md 8f NEXT-4): c(t) cs(x,y) with a smooth seeded positive field cs; the "
                          "variable-coefficient solvers run, 4 field passes per sweep")
+    ap.add_argument("--solver", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="off-default: wave2d_set_option('solver'): 0 auto, 1 exact whole-line, 2 streamed, 3 small-grid cluster")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="off-default: any wave2d_set_option tuning option (repeatable), e.g. --opt tail_min=2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps per end-to-end iteration (default: --steps)")
@@ -322,6 +326,11 @@ def run_ours(args):
     h.set_stream(stream)
     if sch:
         h.set_option("scheme", sch)      # factorised (2.8): set_initial stands at level 1, every run step is a solve
+    if args.solver:
+        h.set_option("solver", args.solver)
+    for kv in args.opt:
+        name, _, val = kv.partition("=")
+        h.set_option(name, float(val))
     h.set_speed(w.c_half)
     if args.speed_field:
         yy = np.linspace(0.0, 1.0, w.n2)[:, None]

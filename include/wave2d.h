@@ -60,7 +60,7 @@ enum {
 enum {
     WAVE2D_SOLVER_AUTO = 0,     /* LINE on small grids; else streamed kernels where the decay bound
                                  * rho^H <= tol allows, else EXACT                                        */
-    WAVE2D_SOLVER_EXACT = 1,    /* untruncated two-pass elimination through HBM (any tau/h)              */
+    WAVE2D_SOLVER_EXACT = 1,    /* whole lines on chip, nothing truncated (any tau/h; lines up to 16384 unknowns) */
     WAVE2D_SOLVER_STREAM = 2,   /* force the streamed kernels; ERR_UNSUPPORTED if the bound fails        */
     WAVE2D_SOLVER_LINE = 3      /* small grids (at most 256 unknowns per line in both directions): the whole step
                                  * loop in one launch of one thread-block cluster, every line solved whole and

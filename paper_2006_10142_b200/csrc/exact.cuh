@@ -1,15 +1,21 @@
 // exact.cuh -- the untruncated line solvers (solver EXACT): any tau / h, any line length up to 16384 unknowns.
 //
 // The north_star's solver sketch -- a line "staged whole in shared memory ... solved by cyclic reduction (or PCR
-// for the last levels) with warp shuffles" (CRM_forward, cr_div, CRM_backward) -- with the two
+// for the last levels) with warp shuffles" (CRM_forward, cr_div, CRM_backward) -- with the
 // changes the scalar coefficients allow:
 //   * register blocking: a thread owns U = 8 consecutive points and eliminates them serially (the first log2 U
 //     reduction levels happen in registers, no strided shared-memory access, no bank conflicts);
-//   * the remaining levels are a scan: with the LU pivots cp_p, inv_p of the half-step's Toeplitz matrix both sweeps
-//     are first-order linear recurrences, so the carries between units follow from the inclusive scan of the pairs
-//     (A, L) -> (A A', L + A L') -- five shuffle rounds inside a warp, one more scan over the warp aggregates of the
-//     line in shared memory.  That is the log2(n+1) - 1 levels of P:124-128 with 2 CTA barriers per sweep direction.
-// Nothing is truncated, so the result is the LU solution to rounding for every tau / h.
+//   * the remaining levels are a scan: both elimination sweeps are first-order linear recurrences, so the carries
+//     between units follow from the inclusive scan of the pairs (A, L) -> (A A', L + A L') -- five shuffle rounds inside
+//     a warp, one more scan over the warp aggregates of the line in shared memory.  That is the log2(n+1) - 1 levels
+//     of P:124-128 with 2 barriers (of the line's warps) per sweep direction;
+//   * Toeplitz systems (c = c(t)) run the recurrences with the STATIONARY factors everywhere (cp = rho,
+//     inv = 1 / (beta - ap rho): the exact LU of the matrix whose first diagonal entry is beta - ap rho instead of beta),
+//     on the line padded to whole warps, and repair both ends afterwards: the difference to the true solution solves
+//     the homogeneous recurrence, so it is  A rho^(p+1) + B rho^(n-p)  with two scalars per line that follow from the
+//     first value and the value at index n of the stationary solution (see boundary_scalars).  No pivot arrays, no
+//     per-point coefficients, the scan carries values only; exact to rounding for every tau / h.
+//   * a variable speed c(t) cs(x,y) (VAR) keeps per-point pivots: a scan of linear-fractional maps (group_pivots).
 //
 // x half-step (lines = grid rows): a group of warps owns a row; a thread's points are 16-byte vectors of the row
 //   (coalesced, straight into registers).  Lines longer than one pass of the CTA (n > 4096) are walked in segments:
@@ -28,55 +34,9 @@ namespace w2d {
 constexpr int EX_U = 8;          // points per thread
 constexpr int EX_NT = 512;       // threads per CTA
 constexpr int EX_NW = EX_NT / 32;
-
-// cpv[p], ivv[p], p < n: the LU pivots of tridiag(-ap, beta, -ap).  The first KMAX come from the host table; if the
-// recurrence has not reached its fixed point (rho, 1 / (beta - ap rho)) by then, one thread continues it until it has
-// (to 1e-15 relative), and the rest is filled in parallel.  conv[0] = first index from which every pivot is the fixed
-// point to 2e-15: units beyond it take the stationary fast path of the solvers.
-__global__ void wave2d_exact_pivots(const double* table, int period, const int* d_k, int n_off, int n, double* cpv,
-                                    double* ivv, int* conv)
-{
-    __shared__ int s_conv, s_head;
-    const int nh = n_off + 2 * (*d_k);
-    const double* row = table + static_cast<size_t>(period ? nh % period : nh) * ROW_DOUBLES;
-    const double ap = row[ROW_AP], beta = row[ROW_BETA], rho = row[ROW_RHO], inv = row[ROW_INV];
-    const int head = n < KMAX ? n : KMAX;
-    if (threadIdx.x == 0) s_head = 0;
-    __syncthreads();
-    for (int p = threadIdx.x; p < head; p += blockDim.x) {
-        const double c = row[ROW_CP + p], v = row[ROW_INVP + p];
-        cpv[p] = c;
-        ivv[p] = v;
-        if (!(fabs(c - rho) <= 2e-15 * rho && fabs(v - inv) <= 2e-15 * inv)) atomicMax(&s_head, p + 1);
-    }
-    __syncthreads();
-    if (n <= KMAX || s_head < KMAX) {           // stationary inside the table: the rest is the fixed point
-        for (int p = KMAX + threadIdx.x; p < n; p += blockDim.x) {
-            cpv[p] = rho;
-            ivv[p] = inv;
-        }
-        if (threadIdx.x == 0) conv[0] = s_head;
-        return;
-    }
-    if (threadIdx.x == 0) {
-        double cp = cpv[KMAX - 1];
-        int p = KMAX;
-        for (; p < n; ++p) {
-            const double iv = 1.0 / (beta - ap * cp);
-            cp = ap * iv;
-            cpv[p] = cp;
-            ivv[p] = iv;
-            if (fabs(cp - rho) <= 1e-15 * rho && fabs(iv - inv) <= 1e-15 * inv) { ++p; break; }
-        }
-        s_conv = p;
-        conv[0] = p;
-    }
-    __syncthreads();
-    for (int p = s_conv + threadIdx.x; p < n; p += blockDim.x) {
-        cpv[p] = rho;
-        ivv[p] = inv;
-    }
-}
+// y strips: elements between the columns of a strip -- a unit of U rows is U + 1 apart (a warp reading one row offset of 32
+// consecutive units touches 32 distinct banks), made odd so that the columns of a row do not share a bank either
+__host__ __device__ constexpr int ex_cpitch(int units) { return (units * (EX_U + 1)) | 1; }
 
 // Stationary scalars of a half-step (units whose pivots are all the fixed point): rho^(e+1), A = rho^U and its powers.
 template <typename T, int U>
@@ -96,64 +56,109 @@ struct Stat {
         double A = pw[U - 1];
 #pragma unroll
         for (int d = 0; d < 6; ++d, A *= A) Ap[d] = static_cast<T>(A);
-        Alane = static_cast<T>(pow(static_cast<double>(pw[U - 1]), static_cast<double>(lane)));
-        Arev = static_cast<T>(pow(static_cast<double>(pw[U - 1]), static_cast<double>(31 - lane)));
+        double al = 1.0, ar = 1.0, Ad = pw[U - 1];    // A^lane, A^(31 - lane) by binary powering
+#pragma unroll
+        for (int d = 0; d < 5; ++d, Ad *= Ad) {
+            if ((lane >> d) & 1) al *= Ad;
+            if (((31 - lane) >> d) & 1) ar *= Ad;
+        }
+        Alane = static_cast<T>(al);
+        Arev = static_cast<T>(ar);
     }
 };
+
+// The two ends of a Toeplitz line.  x'' = the stationary recurrences run over the padded line (x''_{npad} = 0).  The true
+// solution x (x_{-1} = x_n = 0, true first pivot) differs from it by a solution of the homogeneous recurrence,
+//      x_p = x''_p - A rho^(p+1) - B rho^(n-p),       0 <= p < n,
+// and the first and last equation of the line give, with eps = rho^(n+1),
+//      A + B eps = rho x''_0 ,     A eps + B = x''_n        (x''_n := 0 if the padded line ends at n).
+template <typename T>
+struct Ends {
+    double lnr, rho, eps, den;     // ln rho, rho, rho^(n+1), 1 / (1 - eps^2)
+    __device__ __forceinline__ void init(double rho_d, double ln_rho, int n)
+    {
+        rho = rho_d;
+        lnr = ln_rho;
+        eps = exp((n + 1) * lnr);
+        den = 1.0 / (1.0 - eps * eps);
+    }
+    __device__ __forceinline__ T power(int k) const   // rho^k, 0 where it is below every rounding unit that matters
+    {
+        const double x = k * lnr;
+        return x < -96.0 ? T(0) : static_cast<T>(exp(x));
+    }
+    __device__ __forceinline__ void scalars(T x0, T xn, T& A, T& B) const
+    {
+        const double a = (rho * static_cast<double>(x0) - eps * static_cast<double>(xn)) * den;
+        const double b = (static_cast<double>(xn) - eps * rho * static_cast<double>(x0)) * den;
+        A = static_cast<T>(a);
+        B = static_cast<T>(b);
+    }
+};
+// x[e] -= A rho^(p0+e+1) + B rho^(n-p0-e) for the points of a unit that lie on the line (m = n - p0 of them, if fewer
+// than U); PA = rho^(p0+1), PB = rho^(m-U+1) (Ends::power; unused in the unit that holds the end of the line, which
+// reads rho^(m-e) from the table spw[k] = rho^(k+1) in shared memory).  Points beyond the line are set to 0.
+template <typename T, int U>
+__device__ __forceinline__ void repair_unit(T (&x)[U], const Stat<T, U>& S, T A, T B, T PA, T PB, int m, const T* spw)
+{
+    const T a = A * PA;
+    if (m >= U) {
+        const T b = B * PB;
+        if (a == T(0) && b == T(0)) return;
+#pragma unroll
+        for (int e = 0; e < U; ++e) {
+            const T fa = e == 0 ? T(1) : S.pw[e - 1], fb = e == U - 1 ? T(1) : S.pw[U - 2 - e];
+            x[e] -= fmaT(a, fa, b * fb);
+        }
+    } else {
+#pragma unroll
+        for (int e = 0; e < U; ++e) {
+            const T fa = e == 0 ? T(1) : S.pw[e - 1];
+            x[e] = e < m ? x[e] - fmaT(a, fa, B * spw[m - e - 1]) : T(0);
+        }
+    }
+}
+
+// The warps of one line synchronise among themselves only (hardware barriers 1..8: wpc >= 2 means at most 8 groups),
+// so the lines a CTA works on at the same time do not wait for one another.
+__device__ __forceinline__ void group_sync(int group, int wpc)
+{
+    if (wpc > 1) named_bar_sync(1 + group, 32 * wpc);
+    else __syncwarp();
+}
 
 // ---- block-wide solve of one line segment ------------------------------------------------------------------
 // A "group" is wpc consecutive warps of the CTA; thread (gw, lane) of the group owns unit gw * 32 + lane of the segment.
 // sA, sL (forward) and sB, sH (backward) are the group's slices [wpc] of the CTA's aggregate arrays.  Every thread of
-// the CTA must call these (they contain one CTA barrier each).
+// a group must call these (they contain one barrier of the group each).
 
+// General coefficients (variable speed): cp[], iv[] are this unit's pivots.
 // y[] holds r on entry and the true y on exit.  cin: y just before the segment.  Returns y at the end of the segment.
-// FAST (warp-uniform): all 32 units of this warp are whole and stationary -- cp = rho, inv constant, A = rho^U, so the
-// scan needs no products and half the shuffles; cp[] / iv[] are not read.
-template <typename T, int U, bool FAST>
-__device__ __forceinline__ T group_forward_impl(T (&y)[U], const T (&cp)[U], const T (&iv)[U], const Stat<T, U>& S,
-                                                T cin, int wpc, int gw, int lane, T* sA, T* sL)
+template <typename T, int U>
+__device__ __forceinline__ T group_forward(T (&y)[U], const T (&cp)[U], const T (&iv)[U], T cin, int wpc, int gw, int lane,
+                                           T* sA, T* sL, int group)
 {
     constexpr unsigned FULL = 0xffffffffu;
-    T a, v;
-    if constexpr (FAST) {
-        T f = y[0] * S.inv;
-        y[0] = f;
+    T a = T(1), v = T(0);
 #pragma unroll
-        for (int e = 1; e < U; ++e) {
-            f = fmaT(S.rho, f, y[e] * S.inv);
-            y[e] = f;
-        }
-        v = f;
+    for (int e = 0; e < U; ++e) {
+        v = fmaT(cp[e], v, y[e] * iv[e]);
+        y[e] = v;
+        a *= cp[e];
+    }
 #pragma unroll
-        for (int d = 0; d < 5; ++d) {
-            const T v2 = __shfl_up_sync(FULL, v, 1 << d);
-            if (lane >= (1 << d)) v = fmaT(S.Ap[d], v2, v);
-        }
-        a = S.Ap[5];                                   // (lane 31's prefix product: the whole warp)
-    } else {
-        T A = T(1), f = T(0);
-#pragma unroll
-        for (int e = 0; e < U; ++e) {
-            f = fmaT(cp[e], f, y[e] * iv[e]);
-            y[e] = f;
-            A *= cp[e];
-        }
-        a = A;
-        v = f;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const T a2 = __shfl_up_sync(FULL, a, d), v2 = __shfl_up_sync(FULL, v, d);
-            if (lane >= d) {
-                v = fmaT(a, v2, v);
-                a *= a2;
-            }
+    for (int d = 1; d < 32; d <<= 1) {
+        const T a2 = __shfl_up_sync(FULL, a, d), v2 = __shfl_up_sync(FULL, v, d);
+        if (lane >= d) {
+            v = fmaT(a, v2, v);
+            a *= a2;
         }
     }
     if (lane == 31) {
         sA[gw] = a;
         sL[gw] = v;
     }
-    named_bar_sync(1, EX_NT);   // (fast and general warps arrive from different copies of this code)
+    group_sync(group, wpc);
     T ga = lane < wpc ? sA[lane] : T(1), gv = lane < wpc ? sL[lane] : T(0);
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -167,63 +172,42 @@ __device__ __forceinline__ T group_forward_impl(T (&y)[U], const T (&cp)[U], con
     T cw = fmaT(__shfl_sync(FULL, ga, gp), cin, __shfl_sync(FULL, gv, gp));   // y entering this warp
     if (gw == 0) cw = cin;
     const T cout = fmaT(__shfl_sync(FULL, ga, wpc - 1), cin, __shfl_sync(FULL, gv, wpc - 1));
-    const T pv = __shfl_up_sync(FULL, v, 1);
-    if constexpr (FAST) {
-        const T c = lane == 0 ? cw : fmaT(S.Alane, cw, pv);   // y at the end of the previous unit
+    const T pv = __shfl_up_sync(FULL, v, 1), pa = __shfl_up_sync(FULL, a, 1);
+    T c = lane == 0 ? cw : fmaT(pa, cw, pv);
 #pragma unroll
-        for (int e = 0; e < U; ++e) y[e] = fmaT(S.pw[e], c, y[e]);
-    } else {
-        const T pa = __shfl_up_sync(FULL, a, 1);
-        T c = lane == 0 ? cw : fmaT(pa, cw, pv);
-#pragma unroll
-        for (int e = 0; e < U; ++e) {
-            c *= cp[e];
-            y[e] += c;
-        }
+    for (int e = 0; e < U; ++e) {
+        c *= cp[e];
+        y[e] += c;
     }
     return cout;
 }
 
 // y[] holds the true y on entry and x on exit.  xin: x just after the segment.  Returns x at the start of the segment.
-template <typename T, int U, bool FAST>
-__device__ __forceinline__ T group_backward_impl(T (&y)[U], const T (&cp)[U], const Stat<T, U>& S, T xin, int wpc,
-                                                 int gw, int lane, T* sB, T* sH)
+template <typename T, int U>
+__device__ __forceinline__ T group_backward(T (&y)[U], const T (&cp)[U], T xin, int wpc, int gw, int lane, T* sB, T* sH,
+                                            int group)
 {
     constexpr unsigned FULL = 0xffffffffu;
-    T a, v;
-    if constexpr (FAST) {
+    T a = cp[U - 1];
 #pragma unroll
-        for (int e = U - 2; e >= 0; --e) y[e] = fmaT(S.rho, y[e + 1], y[e]);
-        v = y[0];
+    for (int e = U - 2; e >= 0; --e) {
+        y[e] = fmaT(cp[e], y[e + 1], y[e]);
+        a *= cp[e];
+    }
+    T v = y[0];
 #pragma unroll
-        for (int d = 0; d < 5; ++d) {
-            const T v2 = __shfl_down_sync(FULL, v, 1 << d);
-            if (lane + (1 << d) < 32) v = fmaT(S.Ap[d], v2, v);
-        }
-        a = S.Ap[5];
-    } else {
-        T A = cp[U - 1];
-#pragma unroll
-        for (int e = U - 2; e >= 0; --e) {
-            y[e] = fmaT(cp[e], y[e + 1], y[e]);
-            A *= cp[e];
-        }
-        a = A;
-        v = y[0];
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const T a2 = __shfl_down_sync(FULL, a, d), v2 = __shfl_down_sync(FULL, v, d);
-            if (lane + d < 32) {
-                v = fmaT(a, v2, v);
-                a *= a2;
-            }
+    for (int d = 1; d < 32; d <<= 1) {
+        const T a2 = __shfl_down_sync(FULL, a, d), v2 = __shfl_down_sync(FULL, v, d);
+        if (lane + d < 32) {
+            v = fmaT(a, v2, v);
+            a *= a2;
         }
     }
     if (lane == 0) {
         sB[gw] = a;
         sH[gw] = v;
     }
-    named_bar_sync(1, EX_NT);
+    group_sync(group, wpc);
     T ga = lane < wpc ? sB[lane] : T(1), gv = lane < wpc ? sH[lane] : T(0);
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -237,37 +221,89 @@ __device__ __forceinline__ T group_backward_impl(T (&y)[U], const T (&cp)[U], co
     T xw = fmaT(__shfl_sync(FULL, ga, gn), xin, __shfl_sync(FULL, gv, gn));   // x entering this warp from the right
     if (gw + 1 >= wpc) xw = xin;
     const T cout = fmaT(__shfl_sync(FULL, ga, 0), xin, __shfl_sync(FULL, gv, 0));
-    const T nv = __shfl_down_sync(FULL, v, 1);
-    if constexpr (FAST) {
-        const T c = lane == 31 ? xw : fmaT(S.Arev, xw, nv);   // x at the start of the next unit
+    const T nv = __shfl_down_sync(FULL, v, 1), na = __shfl_down_sync(FULL, a, 1);
+    T c = lane == 31 ? xw : fmaT(na, xw, nv);
 #pragma unroll
-        for (int e = 0; e < U; ++e) y[e] = fmaT(S.pw[U - 1 - e], c, y[e]);
-    } else {
-        const T na = __shfl_down_sync(FULL, a, 1);
-        T c = lane == 31 ? xw : fmaT(na, xw, nv);
-#pragma unroll
-        for (int e = U - 1; e >= 0; --e) {
-            c *= cp[e];
-            y[e] += c;
-        }
+    for (int e = U - 1; e >= 0; --e) {
+        c *= cp[e];
+        y[e] += c;
     }
     return cout;
 }
 
-// fast: warp-uniform (see above).  Both variants hold exactly one CTA barrier, so warps of one CTA may differ.
+// ---- the stationary recurrences (Toeplitz lines) --------------------------------------------------------------
+// Every unit has cp = rho, inv constant, A = rho^U: the scans carry values only.  Inside a warp five shuffle rounds with the
+// constant factors A^(2^d); across the warps of the line a Horner loop over the warp aggregates in shared memory
+// (W = A^32 per warp).  y[] holds r on entry and the true y on exit; cin: y just before the segment; returns y at the end of
+// the segment (only if `chain`: a further segment follows).
 template <typename T, int U>
-__device__ __forceinline__ T group_forward(bool fast, T (&y)[U], const T (&cp)[U], const T (&iv)[U], const Stat<T, U>& S,
-                                           T cin, int wpc, int gw, int lane, T* sA, T* sL)
+__device__ __forceinline__ T stat_forward(T (&y)[U], const Stat<T, U>& S, T cin, int wpc, int gw, int lane, T* sL, int group,
+                                          bool chain)
 {
-    return fast ? group_forward_impl<T, U, true>(y, cp, iv, S, cin, wpc, gw, lane, sA, sL)
-                : group_forward_impl<T, U, false>(y, cp, iv, S, cin, wpc, gw, lane, sA, sL);
+    constexpr unsigned FULL = 0xffffffffu;
+    T f = y[0] * S.inv;
+    y[0] = f;
+#pragma unroll
+    for (int e = 1; e < U; ++e) {
+        f = fmaT(S.rho, f, y[e] * S.inv);
+        y[e] = f;
+    }
+    T v = f;
+#pragma unroll
+    for (int d = 0; d < 5; ++d) {
+        const T v2 = __shfl_up_sync(FULL, v, 1 << d);
+        if (lane >= (1 << d)) v = fmaT(S.Ap[d], v2, v);
+    }
+    T cw = cin, cout = T(0);
+    if (wpc > 1) {
+        if (lane == 31) sL[gw] = v;
+        group_sync(group, wpc);
+        for (int j = 0; j < gw; ++j) cw = fmaT(S.Ap[5], cw, sL[j]);      // y entering this warp
+        if (chain) {
+            cout = cw;
+            for (int j = gw; j < wpc; ++j) cout = fmaT(S.Ap[5], cout, sL[j]);
+        }
+    } else if (chain) {
+        cout = fmaT(S.Ap[5], cin, __shfl_sync(FULL, v, 31));
+    }
+    const T pv = __shfl_up_sync(FULL, v, 1);
+    const T c = lane == 0 ? cw : fmaT(S.Alane, cw, pv);   // y at the end of the previous unit
+#pragma unroll
+    for (int e = 0; e < U; ++e) y[e] = fmaT(S.pw[e], c, y[e]);
+    return cout;
 }
+
+// y[] holds the true y on entry and x on exit.  xin: x just after the segment.  Returns x at the start of the segment.
 template <typename T, int U>
-__device__ __forceinline__ T group_backward(bool fast, T (&y)[U], const T (&cp)[U], const Stat<T, U>& S, T xin, int wpc,
-                                            int gw, int lane, T* sB, T* sH)
+__device__ __forceinline__ T stat_backward(T (&y)[U], const Stat<T, U>& S, T xin, int wpc, int gw, int lane, T* sH, int group,
+                                           bool chain)
 {
-    return fast ? group_backward_impl<T, U, true>(y, cp, S, xin, wpc, gw, lane, sB, sH)
-                : group_backward_impl<T, U, false>(y, cp, S, xin, wpc, gw, lane, sB, sH);
+    constexpr unsigned FULL = 0xffffffffu;
+#pragma unroll
+    for (int e = U - 2; e >= 0; --e) y[e] = fmaT(S.rho, y[e + 1], y[e]);
+    T v = y[0];
+#pragma unroll
+    for (int d = 0; d < 5; ++d) {
+        const T v2 = __shfl_down_sync(FULL, v, 1 << d);
+        if (lane + (1 << d) < 32) v = fmaT(S.Ap[d], v2, v);
+    }
+    T xw = xin, cout = T(0);
+    if (wpc > 1) {
+        if (lane == 0) sH[gw] = v;
+        group_sync(group, wpc);
+        for (int j = wpc - 1; j > gw; --j) xw = fmaT(S.Ap[5], xw, sH[j]);   // x entering this warp from the right
+        if (chain) {
+            cout = xw;
+            for (int j = gw; j >= 0; --j) cout = fmaT(S.Ap[5], cout, sH[j]);
+        }
+    } else if (chain) {
+        cout = fmaT(S.Ap[5], xin, __shfl_sync(FULL, v, 0));
+    }
+    const T nv = __shfl_down_sync(FULL, v, 1);
+    const T c = lane == 31 ? xw : fmaT(S.Arev, xw, nv);   // x at the start of the next unit
+#pragma unroll
+    for (int e = 0; e < U; ++e) y[e] = fmaT(S.pw[U - 1 - e], c, y[e]);
+    return cout;
 }
 
 // ---- variable speed: the pivots of a non-Toeplitz line -------------------------------------------
@@ -303,7 +339,7 @@ __device__ __forceinline__ T mob_apply(const Mob<T>& m, T c) { return fmaT(m.A, 
 // of the segment.  sM: the group's slice [3][wpc] of a CTA array (one CTA barrier inside; every thread must call).
 template <typename T, int U>
 __device__ __forceinline__ T group_pivots(const T (&a)[U], T gamma, T (&cp)[U], T (&iv)[U], T cin, int wpc, int gw,
-                                          int lane, T* sMA, T* sMB, T* sMC)
+                                          int lane, T* sMA, T* sMB, T* sMC, int group)
 {
     constexpr unsigned FULL = 0xffffffffu;
     // the unit's map: rows (n0, n1), (d0, d1) of N and D as linear forms of the (N, D) entering the unit
@@ -336,7 +372,7 @@ __device__ __forceinline__ T group_pivots(const T (&a)[U], T gamma, T (&cp)[U], 
         sMB[gw] = m.B;
         sMC[gw] = m.C;
     }
-    named_bar_sync(1, EX_NT);
+    group_sync(group, wpc);
     Mob<T> g;
     g.A = lane < wpc ? sMA[lane] : T(1);
     g.B = lane < wpc ? sMB[lane] : T(0);
@@ -384,9 +420,6 @@ struct ExactArgs {
     int n_off;
     int n, nlines;
     long long pitch;
-    const double* cpv;     // pivots of this half-step (wave2d_exact_pivots)
-    const double* ivv;
-    const int* conv;       // first index from which the pivots are the fixed point
     const void* src;       // compact source window [p - sp0][line - sl0], or NULL
     int sl0, snl, sp0, snp;
     double g2;
@@ -410,47 +443,52 @@ __device__ __forceinline__ void ld16(const T* p, T* v)
     }
 }
 template <typename T>
+__device__ __forceinline__ T ld1(const T* p)
+{
+    return *p;
+}
+template <typename T>
 __device__ __forceinline__ void st16g(T* p, const T* v)
 {
     if constexpr (sizeof(T) == 8) *reinterpret_cast<double2*>(p) = make_double2(v[0], v[1]);
     else *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
 }
 
-// per-thread asynchronous copies global -> shared (LDGSTS): a thread prefetches its own points of the next row
+// per-thread asynchronous copies global -> shared (LDGSTS, through L2 only): a thread prefetches its own points of
+// the next row
 __device__ __forceinline__ void cp_async16(void* dst, const void* src)
 {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-template <int BYTES>
-__device__ __forceinline__ void cp_async_small(void* dst, const void* src)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(dst)), "l"(src), "n"(BYTES) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// Scratch of the block-wide scans, double-buffered: consecutive forward (or backward) calls of a group alternate, so a
+// warp that runs ahead into the next call never overwrites what a slower warp still reads (one barrier per call).
+template <typename T>
+struct ExactScratch {
+    T agg[2][4][EX_NW];
+    T mob[2][3][EX_NW];   // aggregates of the pivot scan (VAR), double-buffered likewise
+    T ends[EX_NW][2];     // per group: x''_0 and x''_n of its line (Toeplitz lines, see Ends)
+    T pw[EX_NW][EX_U];    // per group: rho^(k+1)
+};
+
 // ---- x half-step: (A1 + A2) exact ------------------------------------------------------------------------------
-// grid: CTAs loop over passes of EX_NW / wpc rows.  Dynamic shared memory:
+// The CTAs loop over passes of EX_NW / wpc rows.  Dynamic shared memory:
 //   nseg == 1: two prefetch slots of EX_NT * (2 NV + 1) 16-byte cells -- while a pass is solved, every thread's own
 //              points of the next pass's row (and the two neighbour values of a warp) are already on their way;
 //   nseg  > 1: the parked line, nseg * wpc * 32 * U values (no prefetch: the line itself fills shared memory).
-// VAR: variable speed -- one more field (cs) per row, the pivots come from group_pivots, no stationary fast path.
+// VAR: variable speed -- one more field (cs) per row, the pivots come from group_pivots, no stationary path.
 template <typename T, bool VAR>
-__global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ ExactArgs a)
+__device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, unsigned char* ex_smem, ExactScratch<T>& sc_)
 {
     constexpr int U = EX_U, V = 16 / (int)sizeof(T), NV = U / V;
     constexpr unsigned FULL = 0xffffffffu;
-    extern __shared__ __align__(16) unsigned char ex_smem[];
     T* const s_line = reinterpret_cast<T*>(ex_smem);
-    // aggregates of the block-wide scans, double-buffered: consecutive forward (or backward) calls alternate, so a warp
-    // that runs ahead into the next call never overwrites what a slower warp still reads (one barrier per call)
-    __shared__ T s_agg[2][4][EX_NW];
-    __shared__ T s_mob[VAR ? 2 : 1][3][EX_NW];   // aggregates of the pivot scan (VAR), double-buffered likewise
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wpc = a.wpc, group = warp / wpc, gw = warp % wpc, ngroups = EX_NW / wpc;
-    const int nh = a.n_off + 2 * (*a.d_k);
     const Roles R = roles_of(nh, a.fs.ring);
     const T* const prev = static_cast<const T*>(a.fs.b[R.prev]);
     const T* const cur = static_cast<const T*>(a.fs.b[R.cur]);
@@ -461,25 +499,32 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
     [[maybe_unused]] const T ap = static_cast<T>(row[ROW_AP]), gam = static_cast<T>(a.gamma);
     const T g2 = static_cast<T>(a.g2);
     const bool one = a.one != 0;
-    const int n = a.n, seg_pts = wpc * 32 * U;
+    const int n = a.n, seg_pts = wpc * 32 * U, npad = a.nseg * seg_pts;
     const T* const src = static_cast<const T*>(a.src);
     int pf = 0, pb = 0;   // buffer parity of the next forward / backward call
     [[maybe_unused]] int pp = 0;
 
-    auto pivots = [&](int p0, T (&cp)[U], T (&iv)[U]) {
-#pragma unroll
-        for (int e = 0; e < U; ++e) {            // beyond the line: cp = inv = 0 decouples the padding (x = 0 there)
-            const bool in = p0 + e < n;
-            cp[e] = in ? static_cast<T>(a.cpv[p0 + e]) : T(0);
-            iv[e] = in ? static_cast<T>(a.ivv[p0 + e]) : T(0);
-        }
-    };
     Stat<T, U> S;
     S.init(row[ROW_RHO], row[ROW_INV], lane);
-    const int pc = VAR ? 0x7fffffff : *a.conv;    // pivots are the fixed point from here on (never, with a variable speed)
+    [[maybe_unused]] Ends<T> E;
+    [[maybe_unused]] T PA = T(0), PB = T(0);      // nseg == 1: this thread's rho^(p0+1), rho^(n-p0-U+1)
+    [[maybe_unused]] T* const s_ends = sc_.ends[group];
+    [[maybe_unused]] const T* const s_pw = sc_.pw[group];
+    if constexpr (!VAR) {
+        E.init(row[ROW_RHO], row[ROW_LNR], n);
+        if (gw == 0 && lane == 0) {
+#pragma unroll
+            for (int e = 0; e < U; ++e) sc_.pw[group][e] = S.pw[e];
+        }
+        const int p0 = (gw * 32 + lane) * U;
+        if (a.nseg == 1 && p0 < n) {
+            PA = E.power(p0 + 1);
+            if (n - p0 >= U) PB = E.power(n - p0 - U + 1);
+        }
+    }
 
     // prefetch (nseg == 1): cell c of slot s of this thread; cells [0, NV): prev, [NV, 2 NV): cur, (VAR: [2 NV, 3 NV): cs,)
-    // last: neighbour of the warp
+    // last: the 16 bytes of prev next to the warp (lane 0: before its first point, lane 31: after its last)
     constexpr int CELLS = (VAR ? 3 : 2) * NV + 1;
     const bool pre = a.nseg == 1;
     auto cell = [&](int slot, int c) -> unsigned char* {
@@ -496,8 +541,8 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
                 cp_async16(cell(slot, NV + c), cur + rn + c * V);
                 if constexpr (VAR) cp_async16(cell(slot, 2 * NV + c), csf + rn + c * V);
             }
-            if (!one && lane == 0 && q0 > 0) cp_async_small<sizeof(T)>(cell(slot, CELLS - 1), prev + rn - 1);
-            if (!one && lane == 31 && q0 + U < a.pitch) cp_async_small<sizeof(T)>(cell(slot, CELLS - 1), prev + rn + U);
+            if (!one && lane == 0 && q0 > 0) cp_async16(cell(slot, CELLS - 1), prev + rn - V);
+            if (!one && lane == 31 && q0 + U < a.pitch) cp_async16(cell(slot, CELLS - 1), prev + rn + U);
         }
         cp_async_commit();
     };
@@ -506,16 +551,14 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
 
     for (int base = blockIdx.x * ngroups; base < a.nlines; base += gridDim.x * ngroups, ++it) {
         const int j = base + group;
-        const bool live = j < a.nlines;           // (a dead group still walks through the barriers)
+        const bool live = j < a.nlines;           // (a dead group still walks through its barriers)
         const long long ro = static_cast<long long>(live ? j : 0) * a.pitch;
         const bool src_row = src != nullptr && live && j >= a.sl0 && j < a.sl0 + a.snl;
         T carry = T(0);
-        T y[U], cp[U], iv[U];
+        T y[U];
+        [[maybe_unused]] T cp[VAR ? U : 1], iv[VAR ? U : 1];
         for (int s = 0; s < a.nseg; ++s) {
             const int p0 = s * seg_pts + (gw * 32 + lane) * U;
-            const int w0 = s * seg_pts + gw * 32 * U;                  // first point of this warp
-            const bool fast = live && w0 >= pc && w0 + 32 * U <= n;     // 32 whole stationary units (warp-uniform)
-            if (!VAR && !fast) pivots(p0, cp, iv);
             T wp[U], wc[U];
             [[maybe_unused]] T wa[U];                   // VAR: cs, then a_p = ap cs_p
 #pragma unroll
@@ -532,8 +575,8 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
                         ld16(reinterpret_cast<const T*>(cell(it & 1, NV + c)), wc + c * V);
                         if constexpr (VAR) ld16(reinterpret_cast<const T*>(cell(it & 1, 2 * NV + c)), wa + c * V);
                     }
-                    if (!one && ((lane == 0 && p0 > 0) || (lane == 31 && p0 + U < a.pitch)))
-                        edge = *reinterpret_cast<const T*>(cell(it & 1, CELLS - 1));
+                    if (!one && lane == 0 && p0 > 0) edge = reinterpret_cast<const T*>(cell(it & 1, CELLS - 1))[V - 1];
+                    if (!one && lane == 31 && p0 + U < a.pitch) edge = reinterpret_cast<const T*>(cell(it & 1, CELLS - 1))[0];
                 }
             } else if (inrow) {
 #pragma unroll
@@ -542,8 +585,8 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
                     ld16(cur + ro + p0 + c * V, wc + c * V);
                     if constexpr (VAR) ld16(csf + ro + p0 + c * V, wa + c * V);
                 }
-                if (!one && lane == 0 && p0 > 0) edge = prev[ro + p0 - 1];
-                if (!one && lane == 31 && p0 + U < a.pitch) edge = prev[ro + p0 + U];
+                if (!one && lane == 0 && p0 > 0) edge = ld1(prev + ro + p0 - 1);
+                if (!one && lane == 31 && p0 + U < a.pitch) edge = ld1(prev + ro + p0 + U);
             }
             if (one) {
 #pragma unroll
@@ -573,12 +616,14 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
             if constexpr (VAR) {                   // this line's own pivots (host: nseg == 1 with a variable speed)
 #pragma unroll
                 for (int e = 0; e < U; ++e) wa[e] = p0 + e < n ? ap * wa[e] : T(0);
-                group_pivots<T, U>(wa, gam, cp, iv, T(0), wpc, gw, lane, &s_mob[pp][0][group * wpc],
-                                   &s_mob[pp][1][group * wpc], &s_mob[pp][2][group * wpc]);
+                group_pivots<T, U>(wa, gam, cp, iv, T(0), wpc, gw, lane, &sc_.mob[pp][0][group * wpc],
+                                   &sc_.mob[pp][1][group * wpc], &sc_.mob[pp][2][group * wpc], group);
                 pp ^= 1;
+                carry = group_forward<T, U>(y, cp, iv, carry, wpc, gw, lane, &sc_.agg[pf][0][group * wpc],
+                                                        &sc_.agg[pf][1][group * wpc], group);
+            } else {                               // Toeplitz: stationary factors on the padded line (see Ends)
+                carry = stat_forward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pf][1][group * wpc], group, a.nseg > 1);
             }
-            carry = group_forward<T, U>(fast, y, cp, iv, S, carry, wpc, gw, lane, &s_agg[pf][0][group * wpc],
-                                        &s_agg[pf][1][group * wpc]);
             pf ^= 1;
             if (a.nseg > 1) {
 #pragma unroll
@@ -588,22 +633,69 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
         carry = T(0);
         for (int s = a.nseg - 1; s >= 0; --s) {
             const int p0 = s * seg_pts + (gw * 32 + lane) * U;
-            const int w0 = s * seg_pts + gw * 32 * U;
-            const bool fast = live && w0 >= pc && w0 + 32 * U <= n;
             if (a.nseg > 1) {
-                if (!fast) pivots(p0, cp, iv);
 #pragma unroll
                 for (int e = 0; e < U; ++e) y[e] = s_line[static_cast<size_t>(p0 + e)];
             }
-            carry = group_backward<T, U>(fast, y, cp, S, carry, wpc, gw, lane, &s_agg[pb][2][group * wpc],
-                                         &s_agg[pb][3][group * wpc]);
-            pb ^= 1;
-            if (live && p0 < a.pitch) {
+            if constexpr (VAR) {
+                carry = group_backward<T, U>(y, cp, carry, wpc, gw, lane, &sc_.agg[pb][2][group * wpc],
+                                                         &sc_.agg[pb][3][group * wpc], group);
+                pb ^= 1;
+                if (live && p0 < a.pitch) {
 #pragma unroll
-                for (int c = 0; c < NV; ++c) st16g(out + ro + p0 + c * V, y + c * V);
+                    for (int c = 0; c < NV; ++c) st16g(out + ro + p0 + c * V, y + c * V);
+                }
+            } else {
+                carry = stat_backward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pb][3][group * wpc], group, a.nseg > 1);
+                pb ^= 1;
+                if (p0 == 0) s_ends[0] = y[0];                 // x''_0
+                if (p0 <= n && n < p0 + U) {                   // x''_n (nobody holds it if the padded line ends at n)
+                    T xn = y[0];
+#pragma unroll
+                    for (int e = 1; e < U; ++e) xn = n - p0 == e ? y[e] : xn;
+                    s_ends[1] = xn;
+                }
+                if (a.nseg > 1) {
+#pragma unroll
+                    for (int e = 0; e < U; ++e) s_line[static_cast<size_t>(p0 + e)] = y[e];   // x'' until both ends are known
+                }
             }
         }
+        if constexpr (!VAR) {                      // repair both ends (see Ends), then store
+            group_sync(group, wpc);
+            T A, B;
+            E.scalars(s_ends[0], n < npad ? s_ends[1] : T(0), A, B);
+            if (a.nseg == 1) {
+                const int p0 = (gw * 32 + lane) * U;
+                repair_unit<T, U>(y, S, A, B, PA, PB, n - p0, s_pw);
+                if (live && p0 < a.pitch) {
+#pragma unroll
+                    for (int c = 0; c < NV; ++c) st16g(out + ro + p0 + c * V, y + c * V);
+                }
+            } else {
+                for (int s = 0; s < a.nseg; ++s) {
+                    const int p0 = s * seg_pts + (gw * 32 + lane) * U, m = n - p0;
+#pragma unroll
+                    for (int e = 0; e < U; ++e) y[e] = s_line[static_cast<size_t>(p0 + e)];
+                    repair_unit<T, U>(y, S, A, B, m > 0 ? E.power(p0 + 1) : T(0), m >= U ? E.power(m - U + 1) : T(0), m, s_pw);
+                    if (live && p0 < a.pitch) {
+#pragma unroll
+                        for (int c = 0; c < NV; ++c) st16g(out + ro + p0 + c * V, y + c * V);
+                    }
+                }
+            }
+            if (a.nseg > 1) group_sync(group, wpc);   // the parked line is rewritten by the next pass
+        }
     }
+    cp_async_wait<0>();
+}
+
+template <typename T, bool VAR>
+__global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ ExactArgs a)
+{
+    extern __shared__ __align__(16) unsigned char ex_smem[];
+    __shared__ ExactScratch<T> scratch;
+    exact_x_half_step<T, VAR>(a, a.n_off + 2 * (*a.d_k), ex_smem, scratch);
 }
 
 // ---- y half-step: (A3 + A4) exact ------------------------------------------------------------------------------
@@ -611,17 +703,13 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ 
 // apart: a warp reading one row offset of 32 consecutive units touches 32 distinct bank pairs).
 // VAR: a second strip holds a_p = ap cs_p (the solve needs it along the column), so strips are half as wide.
 template <typename T, bool VAR>
-__global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ ExactArgs a)
+__device__ __forceinline__ void exact_y_half_step(const ExactArgs& a, int nh, unsigned char* ex_smem, ExactScratch<T>& sc_)
 {
     constexpr int U = EX_U, V = 16 / (int)sizeof(T);
-    extern __shared__ __align__(16) unsigned char ex_smem[];
     T* const strip = reinterpret_cast<T*>(ex_smem);
-    __shared__ T s_agg[2][4][EX_NW];   // double-buffered like in wave2d_exact_x
-    __shared__ T s_mob[VAR ? 2 : 1][3][EX_NW];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wpc = a.wpc, group = warp / wpc, gw = warp % wpc, ngroups = EX_NW / wpc;
-    const int nh = a.n_off + 2 * (*a.d_k);
     const Roles R = roles_of(nh, a.fs.ring);
     const T* const prev = static_cast<const T*>(a.fs.b[R.prev]);
     const T* const cur = static_cast<const T*>(a.fs.b[R.cur]);
@@ -631,67 +719,94 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
     const T g2 = static_cast<T>(a.g2);
     const bool one = a.one != 0;
     const int n = a.n, sc = a.sc;
-    const int units = (n + U - 1) / U, cpitch = units * (U + 1);   // strip pitch per column
+    static_assert(U == 8, "strip addressing uses r + (r >> 3)");
+    const int units = (n + U - 1) / U, cpitch = ex_cpitch(units);   // strip pitch per column
     const int seg_units = wpc * 32, nseg = (units + seg_units - 1) / seg_units;
     const T* const src = static_cast<const T*>(a.src);
     int pf = 0, pb = 0;
     [[maybe_unused]] int pp = 0;
     Stat<T, U> S;
     S.init(row[ROW_RHO], row[ROW_INV], lane);
-    const int pc = VAR ? 0x7fffffff : *a.conv;
+    const int npad = nseg * seg_units * U;
+    [[maybe_unused]] Ends<T> E;
+    [[maybe_unused]] T PA = T(0), PB = T(0);      // nseg == 1: this thread's rho^(p0+1), rho^(n-p0-U+1)
+    [[maybe_unused]] T* const s_ends = sc_.ends[group];
+    [[maybe_unused]] const T* const s_pw = sc_.pw[group];
+    if constexpr (!VAR) {
+        E.init(row[ROW_RHO], row[ROW_LNR], n);
+        if (gw == 0 && lane == 0) {
+#pragma unroll
+            for (int e = 0; e < U; ++e) sc_.pw[group][e] = S.pw[e];
+        }
+        const int p0 = (gw * 32 + lane) * U;
+        if (nseg == 1 && p0 < n) {
+            PA = E.power(p0 + 1);
+            if (n - p0 >= U) PB = E.power(n - p0 - U + 1);
+        }
+    }
     [[maybe_unused]] const T* const csf = static_cast<const T*>(a.cs);
     [[maybe_unused]] const T ap = static_cast<T>(row[ROW_AP]), gam = static_cast<T>(a.gamma);
     [[maybe_unused]] T* const strip_a = strip + static_cast<size_t>(sc) * cpitch;   // VAR: a_p, same layout
     const int ve = sc < V ? sc : V;                  // elements a loader thread moves per access
-    const int kcn = sc / ve;                         // accesses per strip row
+    const int kcn = sc / ve;                         // accesses per strip row (a power of two, at most 8)
+    const int lk = 31 - __clz(kcn);
 
     for (int c0 = blockIdx.x * sc; c0 < a.nlines; c0 += gridDim.x * sc) {
-        // ---- A3: right-hand side of (2.12), assembled by coalesced loads into the strip
-        // (batches of UN accesses per thread, all loads of a batch issued before the first use: the fill runs at the
-        // memory system's rate, not at one round trip per row)
-        constexpr int UN = 4;
-        const int total = n * kcn;
-        for (int i0 = threadIdx.x; i0 < total; i0 += EX_NT * UN) {
-            T vc[UN][V], vm[UN][V], vu[UN][V], vd[UN][V];
-            [[maybe_unused]] T vs[UN][V];
+        // ---- A3: right-hand side of (2.12), assembled by coalesced loads into the strip.  A thread takes RB = 4
+        // consecutive rows of one 16-byte column chunk: the stencil neighbours of w_{n-1} inside the block are its own
+        // registers (6 loads of w_{n-1} for 4 rows), and all loads of a block are issued before the first use.
+        // Consecutive lanes take the chunks of a row block, then the next row block.
+        constexpr int RB = 4;
+        const int items = ((n + RB - 1) / RB) << lk;
+        for (int i = threadIdx.x; i < items; i += EX_NT) {
+            const int r0 = (i >> lk) * RB, kc = i & (kcn - 1);
+            T vc[RB][V], vm[RB + 2][V];
+            [[maybe_unused]] T vs[RB][V];
 #pragma unroll
-            for (int k = 0; k < UN; ++k) {
+            for (int k = 0; k < RB + 2; ++k) {
 #pragma unroll
-                for (int e = 0; e < V; ++e) vc[k][e] = vm[k][e] = vu[k][e] = vd[k][e] = vs[k][e] = T(0);
-                const int idx = i0 + k * EX_NT;
-                if (idx < total) {
-                    const int r = idx / kcn, kc = idx % kcn;
-                    const long long o = static_cast<long long>(r) * a.pitch + c0 + kc * ve;   // inside the pitch (pad columns are zero)
-                    if constexpr (VAR) {
-                        if (ve == V) ld16(csf + o, vs[k]);
-                        else
-                            for (int e = 0; e < ve; ++e) vs[k][e] = csf[o + e];
+                for (int e = 0; e < V; ++e) {
+                    vm[k][e] = T(0);
+                    if (k < RB) vc[k][e] = vs[k][e] = T(0);
+                }
+            }
+            const T* const pc_ = cur + static_cast<long long>(r0) * a.pitch + c0 + kc * ve;   // inside the pitch (pad columns are zero)
+            const T* const pm_ = prev + static_cast<long long>(r0 - 1) * a.pitch + c0 + kc * ve;
+            if (ve == V) {
+#pragma unroll
+                for (int k = 0; k < RB; ++k) {
+                    if (r0 + k < n) {
+                        ld16(pc_ + k * a.pitch, vc[k]);
+                        if constexpr (VAR) ld16(csf + (pc_ - cur) + k * a.pitch, vs[k]);
                     }
-                    if (ve == V) {
-                        ld16(cur + o, vc[k]);
-                        if (!one) {
-                            ld16(prev + o, vm[k]);
-                            if (r > 0) ld16(prev + o - a.pitch, vu[k]);
-                            if (r + 1 < n) ld16(prev + o + a.pitch, vd[k]);
+                }
+                if (!one) {
+#pragma unroll
+                    for (int k = 0; k < RB + 2; ++k)
+                        if (r0 + k - 1 >= 0 && r0 + k - 1 < n) ld16(pm_ + k * a.pitch, vm[k]);
+                }
+            } else {
+                for (int e = 0; e < ve; ++e) {
+#pragma unroll
+                    for (int k = 0; k < RB; ++k) {
+                        if (r0 + k < n) {
+                            vc[k][e] = ld1(pc_ + k * a.pitch + e);
+                            if constexpr (VAR) vs[k][e] = ld1(csf + (pc_ - cur) + k * a.pitch + e);
                         }
-                    } else {
-                        for (int e = 0; e < ve; ++e) {
-                            vc[k][e] = cur[o + e];
-                            if (!one) {
-                                vm[k][e] = prev[o + e];
-                                if (r > 0) vu[k][e] = prev[o + e - a.pitch];
-                                if (r + 1 < n) vd[k][e] = prev[o + e + a.pitch];
-                            }
-                        }
+                    }
+                    if (!one) {
+#pragma unroll
+                        for (int k = 0; k < RB + 2; ++k)
+                            if (r0 + k - 1 >= 0 && r0 + k - 1 < n) vm[k][e] = ld1(pm_ + k * a.pitch + e);
                     }
                 }
             }
 #pragma unroll
-            for (int k = 0; k < UN; ++k) {
-                const int idx = i0 + k * EX_NT;
-                if (idx < total) {
-                    const int r = idx / kcn, kc = idx % kcn;
+            for (int k = 0; k < RB; ++k) {
+                const int r = r0 + k;
+                if (r < n) {
                     const bool src_r = src != nullptr && !one && r >= a.sp0 && r < a.sp0 + a.snp;
+                    const int so = r + (r >> 3);
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         if (e < ve) {
@@ -699,14 +814,14 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
                             T rv;
                             if constexpr (VAR) {   // am_p = am cs_p at the point of the equation
                                 const T amp = am * vs[k][e];
-                                rv = fmaT(g2, vc[k][e], fmaT(amp, vu[k][e] + vd[k][e], -fmaT(T(2), amp, gam) * vm[k][e]));
-                                strip_a[(kc * ve + e) * cpitch + r + r / U] = ap * vs[k][e];
+                                rv = fmaT(g2, vc[k][e], fmaT(amp, vm[k][e] + vm[k + 2][e], -fmaT(T(2), amp, gam) * vm[k + 1][e]));
+                                strip_a[(kc * ve + e) * cpitch + so] = ap * vs[k][e];
                             } else {
-                                rv = one ? vc[k][e] : fmaT(g2, vc[k][e], fmaT(am, vu[k][e] + vd[k][e], c1 * vm[k][e]));
+                                rv = one ? vc[k][e] : fmaT(g2, vc[k][e], fmaT(am, vm[k][e] + vm[k + 2][e], c1 * vm[k + 1][e]));
                             }
                             if (src_r && col >= a.sl0 && col < a.sl0 + a.snl)
                                 rv = fmaT(q, src[static_cast<size_t>(r - a.sp0) * a.snl + (col - a.sl0)], rv);
-                            strip[(kc * ve + e) * cpitch + r + r / U] = rv;
+                            strip[(kc * ve + e) * cpitch + so] = rv;
                         }
                     }
                 }
@@ -719,31 +834,25 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
             const bool live = col < sc;
             T* const line = strip + static_cast<size_t>(live ? col : 0) * cpitch;
             T carry = T(0);
-            T y[U], cp[U], iv[U];
+            T y[U];
+            [[maybe_unused]] T cp[VAR ? U : 1], iv[VAR ? U : 1];
             for (int s = 0; s < nseg; ++s) {
                 const int u = s * seg_units + gw * 32 + lane, p0 = u * U;
-                const int w0 = (s * seg_units + gw * 32) * U;
-                const bool fast = live && w0 >= pc && w0 + 32 * U <= n;
 #pragma unroll
-                for (int e = 0; e < U; ++e) {
-                    const bool in = live && p0 + e < n;
-                    if (!VAR && !fast) {
-                        cp[e] = p0 + e < n ? static_cast<T>(a.cpv[p0 + e]) : T(0);
-                        iv[e] = p0 + e < n ? static_cast<T>(a.ivv[p0 + e]) : T(0);
-                    }
-                    y[e] = in ? line[u * (U + 1) + e] : T(0);
-                }
+                for (int e = 0; e < U; ++e) y[e] = live && p0 + e < n ? line[u * (U + 1) + e] : T(0);
                 if constexpr (VAR) {               // this column's own pivots (host: nseg == 1 with a variable speed)
                     T wa[U];
 #pragma unroll
                     for (int e = 0; e < U; ++e)
                         wa[e] = live && p0 + e < n ? strip_a[static_cast<size_t>(col) * cpitch + u * (U + 1) + e] : T(0);
-                    group_pivots<T, U>(wa, gam, cp, iv, T(0), wpc, gw, lane, &s_mob[pp][0][group * wpc],
-                                       &s_mob[pp][1][group * wpc], &s_mob[pp][2][group * wpc]);
+                    group_pivots<T, U>(wa, gam, cp, iv, T(0), wpc, gw, lane, &sc_.mob[pp][0][group * wpc],
+                                       &sc_.mob[pp][1][group * wpc], &sc_.mob[pp][2][group * wpc], group);
                     pp ^= 1;
+                    carry = group_forward<T, U>(y, cp, iv, carry, wpc, gw, lane, &sc_.agg[pf][0][group * wpc],
+                                                            &sc_.agg[pf][1][group * wpc], group);
+                } else {                           // Toeplitz: stationary factors on the padded line (see Ends)
+                    carry = stat_forward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pf][1][group * wpc], group, nseg > 1);
                 }
-                carry = group_forward<T, U>(fast, y, cp, iv, S, carry, wpc, gw, lane, &s_agg[pf][0][group * wpc],
-                                            &s_agg[pf][1][group * wpc]);
                 pf ^= 1;
                 if (nseg > 1 && live) {
 #pragma unroll
@@ -754,39 +863,80 @@ __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ 
             carry = T(0);
             for (int s = nseg - 1; s >= 0; --s) {
                 const int u = s * seg_units + gw * 32 + lane, p0 = u * U;
-                const int w0 = (s * seg_units + gw * 32) * U;
-                const bool fast = live && w0 >= pc && w0 + 32 * U <= n;
                 if (nseg > 1) {
 #pragma unroll
-                    for (int e = 0; e < U; ++e) {
-                        if (!fast) cp[e] = p0 + e < n ? static_cast<T>(a.cpv[p0 + e]) : T(0);
-                        y[e] = live && p0 + e < n ? line[u * (U + 1) + e] : T(0);
+                    for (int e = 0; e < U; ++e) y[e] = live && p0 + e < n ? line[u * (U + 1) + e] : T(0);
+                }
+                if constexpr (VAR) {
+                    carry = group_backward<T, U>(y, cp, carry, wpc, gw, lane, &sc_.agg[pb][2][group * wpc],
+                                                             &sc_.agg[pb][3][group * wpc], group);
+                } else {
+                    carry = stat_backward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pb][3][group * wpc], group, nseg > 1);
+                    if (p0 == 0) s_ends[0] = y[0];             // x''_0
+                    if (p0 <= n && n < p0 + U) {               // x''_n (nobody holds it if the padded line ends at n)
+                        T xn = y[0];
+#pragma unroll
+                        for (int e = 1; e < U; ++e) xn = n - p0 == e ? y[e] : xn;
+                        s_ends[1] = xn;
                     }
                 }
-                carry = group_backward<T, U>(fast, y, cp, S, carry, wpc, gw, lane, &s_agg[pb][2][group * wpc],
-                                             &s_agg[pb][3][group * wpc]);
                 pb ^= 1;
-                if (live) {
+                if (live && (VAR || nseg > 1)) {   // (Toeplitz, one segment: repaired in registers below)
 #pragma unroll
                     for (int e = 0; e < U; ++e)
                         if (p0 + e < n) line[u * (U + 1) + e] = y[e];
                 }
             }
+            if constexpr (!VAR) {                  // repair both ends (see Ends)
+                group_sync(group, wpc);
+                T A, B;
+                E.scalars(s_ends[0], n < npad ? s_ends[1] : T(0), A, B);
+                for (int s = 0; s < nseg; ++s) {
+                    const int u = s * seg_units + gw * 32 + lane, p0 = u * U, m = n - p0;
+                    if (nseg > 1) {
+#pragma unroll
+                        for (int e = 0; e < U; ++e) y[e] = live && p0 + e < n ? line[u * (U + 1) + e] : T(0);
+                        repair_unit<T, U>(y, S, A, B, m > 0 ? E.power(p0 + 1) : T(0), m >= U ? E.power(m - U + 1) : T(0), m, s_pw);
+                    } else {
+                        repair_unit<T, U>(y, S, A, B, PA, PB, m, s_pw);
+                    }
+                    if (live) {
+#pragma unroll
+                        for (int e = 0; e < U; ++e)
+                            if (p0 + e < n) line[u * (U + 1) + e] = y[e];
+                    }
+                }
+            }
         }
         __syncthreads();
-        // ---- coalesced stores of the strip
-        for (int idx = threadIdx.x; idx < n * kcn; idx += EX_NT) {
-            const int r = idx / kcn, kc = idx % kcn;
-            T* const o = out + static_cast<long long>(r) * a.pitch + c0 + kc * ve;
-            T vo[V];
+        // ---- coalesced stores of the strip (same mapping as the fill)
+        for (int i = threadIdx.x; i < items; i += EX_NT) {
+            const int r0 = (i >> lk) * RB, kc = i & (kcn - 1);
+            T* const o = out + static_cast<long long>(r0) * a.pitch + c0 + kc * ve;
 #pragma unroll
-            for (int e = 0; e < V; ++e) vo[e] = e < ve ? strip[(kc * ve + e) * cpitch + r + r / U] : T(0);
-            if (ve == V) st16g(o, vo);
-            else
-                for (int e = 0; e < ve; ++e) o[e] = vo[e];
+            for (int k = 0; k < RB; ++k) {
+                const int r = r0 + k;
+                if (r < n) {
+                    const int so = r + (r >> 3);
+                    T vo[V];
+#pragma unroll
+                    for (int e = 0; e < V; ++e) vo[e] = e < ve ? strip[(kc * ve + e) * cpitch + so] : T(0);
+                    if (ve == V) st16g(o + k * a.pitch, vo);
+                    else
+                        for (int e = 0; e < ve; ++e) o[k * a.pitch + e] = vo[e];
+                }
+            }
         }
         __syncthreads();   // the strip is refilled by the next pass
     }
+}
+
+template <typename T, bool VAR>
+__global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ ExactArgs a)
+{
+    extern __shared__ __align__(16) unsigned char ex_smem[];
+    __shared__ ExactScratch<T> scratch;
+    exact_y_half_step<T, VAR>(a, a.n_off + 2 * (*a.d_k), ex_smem, scratch);
 }
 
 }  // namespace w2d

@@ -54,7 +54,7 @@ __device__ __forceinline__ float fmaT(float a, float b, float c) { return ::fmaf
 // ---- per-half-step scalar table (fp64, built on the host; row n serves half-step n -> n+1) ------
 constexpr int KMAX = 256;    // boundary rows with their own (cp_p, inv_p); >= the longest line of the small-grid kernel
 constexpr int NBK_MAX = 8;   // longest carry series (units)
-constexpr int ROW_AM = 0, ROW_Q = 1, ROW_RHO = 2, ROW_INV = 3, ROW_C1 = 4, ROW_AP = 5, ROW_BETA = 6;
+constexpr int ROW_AM = 0, ROW_Q = 1, ROW_RHO = 2, ROW_INV = 3, ROW_C1 = 4, ROW_AP = 5, ROW_BETA = 6, ROW_LNR = 7;
 constexpr int ROW_CP = 8, ROW_INVP = 8 + KMAX, ROW_DOUBLES = 8 + 2 * KMAX;
 
 // A piece of work: output units [ua, ub) of the 32 lines of panel `panel`; nst stages of NW units are

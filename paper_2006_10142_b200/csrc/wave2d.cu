@@ -156,7 +156,6 @@ struct wave2d_s {
     double* d_table = nullptr;
     size_t table_bytes = 0, pieces_bytes[2] = {0, 0}, cta_off_bytes[2] = {0, 0}, trace_bytes[2] = {0, 0};
     int* d_k = nullptr;
-    double* d_piv = nullptr;             // exact path: cp[nmax], inv[nmax]
     bool plan_ok = false;
     DirPlan plan[2];
     bool line_mode = false;              // small grid: the step loop runs in wave2d_line_steps (line.cuh)
@@ -241,6 +240,7 @@ void fill_row(double* row, double gamma, double ap, double am, double qv)
     row[ROW_C1] = -(gamma + 2.0 * am);
     row[ROW_AP] = ap;
     row[ROW_BETA] = beta;
+    row[ROW_LNR] = std::log(rho);
     double cp = 0.0;
     for (int p = 0; p < KMAX; ++p) {   // LU pivots of tridiag(-ap, beta, -ap): inv_p = 1/u_pp, cp_p = ap/u_pp
         const double iv = 1.0 / (beta - ap * cp);
@@ -471,9 +471,9 @@ int plan_exact(wave2d_t* h, int d)
             P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, false>)
                                              : reinterpret_cast<const void*>(&wave2d_exact_x<float, false>);
         const int passes = (P.nlines + EX_NW / wpc - 1) / (EX_NW / wpc);
-        P.grid = std::max(1, std::min(passes, 4 * h->num_sms));
+        P.grid = passes;
     } else {
-        const size_t col = (size_t)units * (EX_U + 1) * h->elem * (var ? 2 : 1);   // one column of the strip (+ its a_p)
+        const size_t col = (size_t)ex_cpitch(units) * h->elem * (var ? 2 : 1);   // one column of the strip (+ its a_p)
         int sc = 16;
         while (sc > 1 && sc * col > budget) sc /= 2;
         if (sc * col > budget) {
@@ -491,9 +491,13 @@ int plan_exact(wave2d_t* h, int d)
             P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, false>)
                                              : reinterpret_cast<const void*>(&wave2d_exact_y<float, false>);
         const int strips = (P.nlines + sc - 1) / sc;
-        P.grid = std::max(1, std::min(strips, 4 * h->num_sms));
+        P.grid = strips;
     }
     W2D_CUDA(h, cudaFuncSetAttribute(P.ex_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget));
+    // persistent CTAs, one wave: a CTA's start-up (scalars, first loads) is paid once per SM slot, not once per few lines
+    int per_sm = 0;
+    W2D_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, P.ex_fn, EX_NT, (size_t)P.ex_smem));
+    P.grid = std::max(1, std::min(P.grid, std::max(1, per_sm) * h->num_sms));
     return WAVE2D_OK;
 }
 
@@ -725,10 +729,6 @@ int ensure_plan(wave2d_t* h)
             W2D_CUDA(h, cudaMemset(h->d_trace[d], 0, tb));
         }
     }
-    if ((h->plan[0].solver == WAVE2D_SOLVER_EXACT || h->plan[1].solver == WAVE2D_SOLVER_EXACT) && !h->d_piv) {
-        st = dev_alloc(h, reinterpret_cast<void**>(&h->d_piv), sizeof(double) * (2 * (size_t)std::max(h->n1, h->n2) + 1));
-        if (st) return st;
-    }
     h->plan_ok = true;
     // The step loop's graphs are part of the plan: captured, instantiated and uploaded here, never inside a run call
     // that may be timed (wave2d_run(h, 0) forces the plan).
@@ -748,6 +748,25 @@ FieldSet field_set(const wave2d_t* h)
     for (int b = 0; b < 4; ++b) fs.b[b] = h->buf[b];
     fs.ring = h->scheme == 1 ? 4 : 3;
     return fs;
+}
+
+// Arguments of a whole-line half-step (exact.cuh) of direction d that do not depend on the time level.
+ExactArgs exact_args(const wave2d_t* h, int d)
+{
+    const DirPlan& P = h->plan[d];
+    ExactArgs a = {};
+    a.fs = field_set(h);
+    a.table = h->d_table; a.period = h->table_period;
+    a.n = P.n; a.nlines = P.nlines; a.pitch = h->pitch;
+    a.src = h->have_src && !(h->scheme == 1 && d == 1) ? h->src_dev[d] : nullptr;   // scheme 1: f enters in x only
+    a.sl0 = d == 0 ? h->win_j0 : h->win_i0; a.snl = d == 0 ? h->win_h : h->win_w;
+    a.sp0 = d == 0 ? h->win_i0 : h->win_j0; a.snp = d == 0 ? h->win_w : h->win_h;
+    a.g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
+    a.one = h->scheme == 1 && d == 1;
+    a.wpc = P.ex_wpc; a.nseg = P.ex_nseg; a.sc = P.ex_sc;
+    a.cs = h->d_cs;
+    a.gamma = h->gamma;
+    return a;
 }
 
 // One half-step: sweep n_off of the current chunk (the kernels add twice the device step counter; the direction is
@@ -793,23 +812,9 @@ int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own
         W2D_CUDA(h, cudaLaunchKernelExC(&cfg, P.var->fn, args));
         return WAVE2D_OK;
     }
-    // exact path: pivots of this half-step, then the whole-line solver of the direction (exact.cuh)
-    double* cpv = h->d_piv;
-    double* ivv = h->d_piv + std::max(h->n1, h->n2);
-    int* conv = reinterpret_cast<int*>(h->d_piv + 2 * (size_t)std::max(h->n1, h->n2));
-    if (!h->have_cs)   // (with a variable speed every line computes its own pivots inside the solver)
-        wave2d_exact_pivots<<<1, 256, 0, stream>>>(h->d_table, h->table_period, dk, n_off, P.n, cpv, ivv, conv);
-    ExactArgs a;
-    a.conv = conv;
-    a.cs = h->d_cs;
-    a.gamma = h->gamma;
-    a.fs = field_set(h);
-    a.table = h->d_table; a.period = h->table_period; a.d_k = dk; a.n_off = n_off;
-    a.n = P.n; a.nlines = P.nlines; a.pitch = h->pitch; a.cpv = cpv; a.ivv = ivv;
-    a.src = src; a.sl0 = sl0; a.snl = snl; a.sp0 = sp0; a.snp = snp;
-    a.g2 = h->scheme == 1 ? 2.0 : 2.0 * h->gamma;
-    a.one = h->scheme == 1 && d == 1;
-    a.wpc = P.ex_wpc; a.nseg = P.ex_nseg; a.sc = P.ex_sc;
+    // exact path: the whole-line solver of the direction (exact.cuh)
+    ExactArgs a = exact_args(h, d);
+    a.d_k = dk; a.n_off = n_off;
     void* args[1] = {&a};
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(P.grid);
@@ -822,7 +827,8 @@ int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own
 
 int kernels_per_sweep(const wave2d_t* h, int d)
 {
-    return h->plan[d].solver == WAVE2D_SOLVER_STREAM || h->have_cs ? 1 : 2;   // exact: pivots + solver
+    (void)h; (void)d;
+    return 1;
 }
 
 // A chunk of the step loop (A7): `steps` time steps = sweeps n_off = 0 .. 2 steps - 1 relative to the device step
@@ -1011,7 +1017,6 @@ void wave2d_destroy(wave2d_t* h)
     cudaFree(h->d_cs);
     cudaFree(h->d_table);
     cudaFree(h->d_k);
-    cudaFree(h->d_piv);
     for (int d = 0; d < 2; ++d) {
         cudaFree(h->d_pieces[d]);
         cudaFree(h->d_cta_off[d]);

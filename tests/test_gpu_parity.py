@@ -793,11 +793,32 @@ def test_exact_solver_long_lines_any_tau(N1, N2, alpha):
         r = oracle.solve(N1, N2, 1.0, tau, M, cast(phi), cast(psi), c_half=c, s=cast(s), g_half=g)
         u, info = gpu(w, solver=B.SOLVER_EXACT)
         assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
-        assert info["launches"] == 4 * M + 2             # per sweep: pivots + solver; M = 3 steps = chunks of 2 + 1
+        assert info["launches"] == 2 * M + 2             # one kernel per sweep; M = 3 steps = chunks of 2 + 1
         assert relerr(u, r) <= tol, (dtype, relerr(u, r))
         r1 = oracle.solve(N1, N2, 1.0, tau, M, cast(phi), cast(psi), c_half=c, s=cast(s), g_half=g, scheme=1)
         u1, _ = gpu1(w, solver=B.SOLVER_EXACT)
         assert relerr(u1, r1) <= tol, (dtype, "scheme 1", relerr(u1, r1))
+
+
+@pytest.mark.parametrize("N1,N2", [(2, 2), (3, 9), (9, 8), (33, 18), (257, 40), (40, 257), (513, 24), (300, 1025),
+                                   (4097, 12), (12, 4098)])
+@pytest.mark.parametrize("alpha", [1e-6, 0.5, 5000.0])
+def test_exact_solver_both_ends_repaired_at_extreme_alpha(N1, N2, alpha):
+    """The Toeplitz lines of solver EXACT run the stationary recurrences on the padded line and repair both ends with
+    A rho^(p+1) + B rho^(n-p) (exact.cuh, Ends).  rho = 5e-7 (alpha = 1e-6: the repair vanishes after one point) up to
+    rho = 0.986 (alpha = 5000, tau = 100 h: both modes span the whole line, and rho^(n+1) couples the two ends on the
+    short lines); lines that end exactly on the padded length (n = 256, 512, 4096: no x''_n) and one point beyond it."""
+    M = 3
+    rng = np.random.default_rng(N1 * 11 + N2)
+    tau = np.sqrt(2.0 * alpha) / max(N1, N2)
+    shape = (N2 - 1, N1 - 1)
+    phi, psi, s = (rng.uniform(-1, 1, shape) for _ in range(3))
+    c = rng.uniform(0.8, 1.2, 2 * M + 1)
+    g = rng.uniform(-1, 1, 2 * M)
+    w = W.Workload("rand", N1, N2, 1.0, tau, M, "f64", phi, psi, c, s=s, g_half=g)
+    u, info = gpu(w, solver=B.SOLVER_EXACT)
+    assert info["solver_x"] == B.SOLVER_EXACT and info["solver_y"] == B.SOLVER_EXACT
+    assert relerr(u, ref(w)) <= 1e-11
 
 
 def test_exact_solver_full_grid_tau_16h():
