@@ -208,7 +208,7 @@ class Wave2DOracle:
 
 
 def solve(N1, N2, l, tau, M, phi, psi=None, c_half=None, s=None, g_half=None, steps=None,
-          gamma=None, kappa=None, scheme=0, cs=None) -> np.ndarray:
+          gamma=None, kappa=None, scheme=0, cs=None, sigma=None, start=None) -> np.ndarray:
     """Convenience: advance to time level `steps` (default M) and return u^steps.
     scheme 1 (factorised (2.8)): set_initial already stands at level 1, so steps - 1 solves are run."""
     o = Wave2DOracle(N1, N2, l, tau, M)
@@ -219,6 +219,10 @@ def solve(N1, N2, l, tau, M, phi, psi=None, c_half=None, s=None, g_half=None, st
             o.set_option("gamma", gamma)
         if kappa is not None:
             o.set_option("kappa", kappa)
+        if sigma is not None:
+            o.set_option("sigma", sigma)
+        if start is not None:
+            o.set_option("start", start)
         if c_half is not None:
             o.set_speed(c_half)
         if cs is not None:

@@ -39,6 +39,14 @@
  * A variable speed c(t) cs(x,y) (oracle_half_step_var) has its pins in
  * tests/test_oracle_varspeed.py.
  *
+ * Two more options of SURVEY.md 8f NEXT-4 (pins in tests/test_oracle_variants.py):
+ *   "sigma"  weight of the implicit operator in the split scheme: ap = sigma tau^2 c_{n+1} / h_d^2,
+ *            am = (1 - sigma) tau^2 c_{n-1} / h_d^2.  sigma = 1/2 is (2.11)-(2.12); sigma = 1 (with gamma = 1, c = 1) is
+ *            the system Listing 1 prints: a = c = tau^2, b = 2 tau^2 + h^2, f = h^2 u^{k-1} - 2 h^2 u^k.
+ *   "start"  2: second-order start of the three-level scheme (2.8) (scheme 1) for psi != 0 or f != 0:
+ *            u^1 = phi + tau psi + (tau^2 / 2) (c^0 Lap_h phi + f^0), the Taylor value with u_tt from (2.1);
+ *            1 (default): (2.9) as printed, u^1 = phi + tau psi.
+ *
  * Parity pins (tests/test_oracle_*.py): dense LU of the Kronecker system on tiny grids, the exact
  * discrete modal recurrence, the PDE standing wave (observed order 1), forced response, tridiagonal
  * residuals, linearity / reflection invariants.  Nothing here is "parity unpinned".
@@ -245,6 +253,9 @@ typedef struct oracle_wave2d_s {
     int have_initial; /* set_initial called                                        */
     int n_done;       /* half-steps taken so far (scheme 1: 2 x the time level k)  */
     int scheme;       /* 0: split scheme (2.11)-(2.12); 1: factorised (2.8)        */
+    double sigma;     /* weight of the implicit operator in the split scheme (1/2)   */
+    int start;        /* scheme 1: 1 = (2.9) as printed, 2 = second-order start      */
+    int start_done;   /* the second-order term has been added (at the first run)     */
 } oracle_wave2d_t;
 
 int oracle_wave2d_create(oracle_wave2d_t **out, int N1, int N2, double l, double tau, int M)
@@ -256,6 +267,8 @@ int oracle_wave2d_create(oracle_wave2d_t **out, int N1, int N2, double l, double
     h->l = l; h->tau = tau;
     h->gamma = 2.0;   /* DESIGN.md reading A2: consistent LOD form */
     h->kappa = 0.5;
+    h->sigma = 0.5;
+    h->start = 1;
     size_t npts = (size_t)h->n1 * (size_t)h->n2;
     h->c_half = (double *)malloc(sizeof(double) * (size_t)(2 * M + 1));
     for (int k = 0; k < 3; ++k) h->w[k] = (double *)calloc(npts, sizeof(double));
@@ -280,6 +293,8 @@ int oracle_wave2d_set_option(oracle_wave2d_t *h, const char *name, double value)
     if (h->n_done > 0) return ORACLE_ERR_STATE;
     if (!strcmp(name, "gamma")) { if (!(value > 0.0)) return ORACLE_ERR_ARG; h->gamma = value; return ORACLE_OK; }
     if (!strcmp(name, "kappa")) { h->kappa = value; return ORACLE_OK; }
+    if (!strcmp(name, "sigma")) { if (!(value > 0.0 && value <= 1.0)) return ORACLE_ERR_ARG; h->sigma = value; return ORACLE_OK; }
+    if (!strcmp(name, "start")) { if (value != 1.0 && value != 2.0) return ORACLE_ERR_ARG; h->start = (int)value; return ORACLE_OK; }
     if (!strcmp(name, "scheme")) {   /* before set_initial */
         if ((value != 0.0 && value != 1.0) || h->have_initial) return ORACLE_ERR_ARG;
         h->scheme = (int)value;
@@ -307,8 +322,26 @@ int oracle_wave2d_set_initial(oracle_wave2d_t *h, const double *phi, const doubl
             }
         }
     h->have_initial = 1;
+    h->start_done = 0;
     h->n_done = h->scheme == 1 ? 2 : 0;
     return ORACLE_OK;
+}
+
+/* Second-order start of (2.8): u^1 += (tau^2 / 2) (c^0 Lap_h phi + g^0 s), with u^0 = phi in w[0], u^1 in w[1] and
+ * Lap_h the five-point Laplacian with zero Dirichlet ghosts (2.10).  Applied at the first run: the speed and source
+ * samples may be set after the initial data. */
+static void oracle_second_order_start(oracle_wave2d_t *h)
+{
+    const double h1 = h->l / h->N1, h2 = h->l / h->N2, c0 = h->c_half[0], g0 = h->g_half ? h->g_half[0] : 1.0;
+    const double *phi = h->w[0];
+    for (int j = 0; j < h->n2; ++j)
+        for (int i = 0; i < h->n1; ++i) {
+            const size_t o = (size_t)j * h->n1 + i;
+            const double we = i > 0 ? phi[o - 1] : 0.0, ea = i < h->n1 - 1 ? phi[o + 1] : 0.0;
+            const double so = j > 0 ? phi[o - h->n1] : 0.0, no = j < h->n2 - 1 ? phi[o + h->n1] : 0.0;
+            const double lap = (we - 2.0 * phi[o] + ea) / (h1 * h1) + (so - 2.0 * phi[o] + no) / (h2 * h2);
+            h->w[1][o] += 0.5 * h->tau * h->tau * (c0 * lap + (h->s ? g0 * h->s[o] : 0.0));
+        }
 }
 
 /* c_half[n] = c(n tau/2), n = 0..2M  (count == 2M+1), or one constant (count == 1). */
@@ -365,7 +398,13 @@ int oracle_wave2d_run(oracle_wave2d_t *h, int steps)
     if (!h || steps < 0) return ORACLE_ERR_ARG;
     if (!h->have_initial) return ORACLE_ERR_STATE;
     if (h->n_done / 2 + steps > h->M) return ORACLE_ERR_RANGE;
-    if (h->scheme == 1 && h->cs) return ORACLE_ERR_ARG;
+    if (h->scheme == 1 && (h->cs || h->sigma != 0.5)) return ORACLE_ERR_ARG;
+    if (h->scheme == 0 && h->start != 1) return ORACLE_ERR_ARG;   /* (2.9) belongs to the three-level scheme (2.8) */
+    if (h->scheme == 1 && h->start == 2 && !h->start_done && steps > 0) {
+        if (h->n_done != 2) return ORACLE_ERR_STATE;
+        oracle_second_order_start(h);
+        h->start_done = 1;
+    }
     if (h->scheme == 1) {   /* (2.8) factorised: level k -> k+1 needs c^{k-1}, c^{k+1}, g^k (integer levels) */
         for (int it = 0; it < steps; ++it) {
             const int k = h->n_done / 2;
@@ -386,8 +425,8 @@ int oracle_wave2d_run(oracle_wave2d_t *h, int steps)
         const int dir = n & 1;                                   /* x if n even, y if n odd */
         const double hd = h->l / (dir == 0 ? h->N1 : h->N2);     /* reading A3: h1 in x, h2 in y */
         const double t2 = h->tau * h->tau;
-        const double ap = t2 * h->c_half[n + 1] / (2.0 * hd * hd);
-        const double am = t2 * h->c_half[n > 0 ? n - 1 : 0] / (2.0 * hd * hd);   /* reading A5 */
+        const double ap = h->sigma * t2 * h->c_half[n + 1] / (hd * hd);                       /* sigma = 1/2: (2.11)-(2.12) */
+        const double am = (1.0 - h->sigma) * t2 * h->c_half[n > 0 ? n - 1 : 0] / (hd * hd);   /* reading A5 */
         const double g = h->g_half ? h->g_half[n] : 1.0;                        /* reading A8 */
         const double q = h->kappa * t2 * g;
         if (h->cs) oracle_half_step_var(h->n1, h->n2, dir, ap, am, h->gamma, q, h->cs, h->w[0], h->w[1], h->s, h->w[2]);
