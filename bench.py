@@ -57,6 +57,9 @@ def parse_args():
     ap.add_argument("--speed-field", action="store_true",
                     help="off-config (SURVEY.md 8f NEXT-4): c(t) cs(x,y) with a smooth seeded positive field cs; the "
                          "variable-coefficient solvers run, 4 field passes per sweep")
+    ap.add_argument("--dense-source", action="store_true",
+                    help="off-config: replace the workload's source shape by one that is non-zero on the whole grid "
+                         "(wave2d_set_source with a full grid: + 1 field read per sweep)")
     ap.add_argument("--solver", type=int, default=0, choices=[0, 1, 2, 3],
                     help="off-default: wave2d_set_option('solver'): 0 auto, 1 exact whole-line, 2 streamed, 3 small-grid cluster")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
@@ -338,6 +341,13 @@ def run_ours(args):
         cs = 1.0 + 0.4 * np.sin(2 * np.pi * xx) * np.cos(np.pi * yy) + 0.3 * xx - 0.2 * yy
         h.set_speed_field(cs.astype(npdt))
         w.name += " with speed field cs(x,y) (off-config)"
+    if args.dense_source:
+        yy = np.linspace(0.0, 1.0, w.n2)[:, None]
+        xx = np.linspace(0.0, 1.0, w.n1)[None, :]
+        w.s = 1.0 + 0.5 * np.sin(3 * np.pi * xx) * np.cos(2 * np.pi * yy)      # non-zero everywhere
+        if w.g_half is None:
+            w.g_half = np.cos(np.arange(2 * w.M) * 0.01)
+        w.name += " with a dense source s(x,y) (off-config)"
     if w.s is not None:
         h.set_source(w.s.astype(npdt, copy=False), w.g_half)
     h.set_initial(phi_pin)
@@ -394,8 +404,11 @@ def run_ours(args):
     bytes_x, bytes_y = 3 * fbytes, (2 if sch else 3) * fbytes
     if args.speed_field:                      # + the speed field in every sweep
         bytes_x, bytes_y = 4 * fbytes, 4 * fbytes
+    if args.dense_source:                     # + the source shape in every sweep that adds f (scheme 1: the x sweep only)
+        bytes_x += fbytes
+        bytes_y += 0 if sch else fbytes
     sweep_bytes = bytes_x if dom == "x" else bytes_y
-    passes = 8 if args.speed_field else 5 if sch else 6
+    passes = (8 if args.speed_field else 5 if sch else 6) + (0 if not args.dense_source else 1 if sch else 2)
     step_s = ms * 1e-3 / K
     # The timed region is K steps = K launches of each sweep kernel back to back (graph replay), timed by the two
     # events above.  The dominant kernel's average launch duration in that region is its share of the step (from

@@ -90,6 +90,16 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "kappa"  source weight.              Default 0.5.   | locally-one-dimensional form of (2.11)-(2.12);
  *                                                       | gamma = kappa = 1 is the scheme as printed
  *                                                       |, which solves u_tt = 2c Lap u + 4f.
+ *   "sigma"  weight of the implicit operator in the split scheme, in (0, 1].  Default 0.5 = (2.11)-(2.12):
+ *            alpha+ = sigma tau^2 c_{n+1} / h_d^2 on w_{n+1}, alpha- = (1 - sigma) tau^2 c_{n-1} / h_d^2 on w_{n-1}.
+ *            sigma = 1 with gamma = 1 and c = 1 is the tridiagonal system Listing 1 prints (PAPER.md:157-162:
+ *            a = c = tau^2, b = 2 tau^2 + h^2, f = h^2 u^{k-1} - 2 h^2 u^k), the fully implicit three-level step.
+ *            Scheme 0 only (ERR_UNSUPPORTED with scheme 1, whose weight is 1/2 by definition).
+ *   "start"  scheme 1 only.  1 (default): (2.9) as printed, u^1 = phi + tau psi (first order).
+ *            2: u^1 = phi + tau psi + (tau^2 / 2) (c^0 Lap_h phi + g^0 s), the Taylor value with u_tt from (2.1): the
+ *            three-level scheme (2.8) is then second order in tau also for psi != 0 or f != 0.  The extra term needs
+ *            the final speed and source samples, so it is added at the first wave2d_run (wave2d_get before that
+ *            returns phi + tau psi).  With scheme 0, wave2d_run returns ERR_UNSUPPORTED.
  *   "scheme" 0 (default): the split scheme (2.11)-(2.12) driven by Algorithm 1.
  *            1: the factorised form of the unsplit three-level scheme (2.8),
  *                 (I - ax+ Dx)(I - ay+ Dy) u^{k+1} = 2 u^k - (I - ax- Dx)(I - ay- Dy) u^{k-1} + tau^2 f^k,

@@ -213,10 +213,15 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
 //           warps whose look-ahead heads are all in this stage finish and store their unit now, the last
 //           few keep it one more stage ("deferred").
 // ---------------------------------------------------------------------------------------------------
-template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB, bool ONE = false>
+// SRCM: how the source term q s enters.  1 (every shape): a compact window (config 3's 155^2 points) -- the few units it
+// covers load their values where they use them.  2: a source on much of the grid -- every unit requests its values
+// before it waits for the stage and calls the next stage's into L2.  0: compiled without a source (none is set; ONE
+// never adds one).  The host picks the kernel per launch.
+template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB, bool ONE = false, int SRCM = 1>
 __global__ void __launch_bounds__(32 * NW, MINB)
 wave2d_sweep_panel(const __grid_constant__ SweepMaps maps, const __grid_constant__ SweepArgs a)
 {
+    constexpr bool SRC = SRCM != 0 && !ONE, DENSE = SRCM == 2 && !ONE;
     using K = PanelCfg<T, DIR, UT, NW, NSTAGE, ONE>;
     constexpr int U = UT, TL = K::TL, V = K::V, SUB = K::SUB, NT = K::NT, RING = 2 * NW;
 
@@ -493,9 +498,9 @@ wave2d_sweep_panel(const __grid_constant__ SweepMaps maps, const __grid_constant
             const Piece pc = a.pieces[pid];
             const int line0 = pc.panel * TL, line = line0 + lane;
             const int gbase = max(pc.ua - nbk, 0) & ~(SUB - 1);
-            const bool src_tile = a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
-            const bool src_line = line >= a.sl0 && line < a.sl0 + a.snl;
-            const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
+            [[maybe_unused]] const bool src_tile = SRC && a.src != nullptr && line0 < a.sl0 + a.snl && line0 + TL > a.sl0;
+            [[maybe_unused]] const bool src_line = SRC && line >= a.sl0 && line < a.sl0 + a.snl;
+            [[maybe_unused]] const T* srcp = reinterpret_cast<const T*>(a.src) + (line - a.sl0);
 
             if (!signaled && ord > own_count) {   // static share and one drawn piece done: its stores have landed
                 publish_static_done();
@@ -512,123 +517,160 @@ wave2d_sweep_panel(const __grid_constant__ SweepMaps maps, const __grid_constant
             s_L[(NW + warp) * TL + lane] = T(0);   // "stage -1": zero carries
             if (lane == 0) s_A[NW + warp] = T(0);
 
-            for (int s = 0; s < pc.nst; ++s) {
-                const int ring = (s & 1) * NW + warp;
-                const int g = gbase + s * NW + warp, p0 = g * U;
-                T xl[U];
-                // ---- shared memory -> registers
-                mbar_wait(bar32 + 8 * slot, phase);
-                draw_ahead();   // (thread 0) the ticket's round trip overlaps this stage's first half
-                const unsigned char* st = sm + slot * K::STAGE_BYTES;
-                if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
-                [[maybe_unused]] T wp[U], wl, wr;
-                T wc[U];
-                if constexpr (DIR == 0) {
-                    const unsigned char* tp = st + tix * 4096;
-                    load_unit_x<T, U>(tp, lane, sub, wp);
-                    load_unit_x<T, U>(tp + K::FIELD_BYTES, lane, sub, wc);
-                    if (sub > 0) wl = tile_elem_x<T>(tp, lane, sub * U - 1);
-                    else if (tix > 0) wl = tile_elem_x<T>(tp - 4096, lane, K::TU - 1);
-                    else wl = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES)[lane * V + V - 1];
-                    if (sub < SUB - 1) wr = tile_elem_x<T>(tp, lane, (sub + 1) * U);
-                    else if (tix < NT - 1) wr = tile_elem_x<T>(tp + 4096, lane, 0);
-                    else wr = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V];
-                } else if constexpr (ONE) {
-                    const T* ccv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
-#pragma unroll
-                    for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
-                } else {
-                    const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
-                    const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
-                    wl = cpv[0];
-#pragma unroll
-                    for (int e = 0; e < U; ++e) wp[e] = cpv[(e + 1) * TL];
-                    wr = cpv[(U + 1) * TL];
-#pragma unroll
-                    for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
-                }
-                // ---- RHS + local forward elimination
-                const bool fast = g >= kb && p0 + U <= n;   // stationary pivots, whole unit inside the line
-                T Aval;
-                if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
-#pragma unroll
-                    for (int e = 0; e < U; ++e) {
-                        if constexpr (ONE) {
-                            xl[e] = inv * wc[e];
-                        } else {
-                            const T left = e == 0 ? wl : wp[e - 1];
-                            const T right = e == U - 1 ? wr : wp[e + 1];
-                            xl[e] = fmaT(g2i, wc[e], fmaT(ami, left + right, c1i * wp[e]));
+            // The stages of the piece.  (Two copies, with and without the source term, chosen per piece by whether its lines
+            // meet a compact window, were measured: 140.5 instead of 130.3 us per step at config 3 -- the instruction
+            // cache pays more than the leaner loop saves.)
+            auto stages = [&](auto src_c) {
+                constexpr bool PSRC = decltype(src_c)::value, PDENSE = PSRC && DENSE;
+                for (int s = 0; s < pc.nst; ++s) {
+                    const int ring = (s & 1) * NW + warp;
+                    const int g = gbase + s * NW + warp, p0 = g * U;
+                    T xl[U];
+                    // ---- source values of this unit (a source window that covers it: rare with a compact window, every unit
+                    // with a dense s): requested before the stage's data is awaited, used at the end of the right-hand side
+                    [[maybe_unused]] bool src_unit = false;
+                    [[maybe_unused]] T sv[PDENSE ? U : 1];
+                    if constexpr (PSRC) src_unit = src_tile && src_line && p0 < a.sp0 + a.snp && p0 + U > a.sp0;
+                    if constexpr (PDENSE) {
+                        if (src_unit) {
+    #pragma unroll
+                            for (int e = 0; e < U; ++e) {
+                                const int ps = p0 + e - a.sp0;
+                                sv[e] = ps >= 0 && ps < a.snp && p0 + e < n ? srcp[static_cast<size_t>(ps) * a.snl] : T(0);
+                            }
+                        }
+                        if (src_tile && src_line && (lane & 15) == 0) {   // and the next stage's lines of s are called into L2
+                            const int ps0 = p0 + NW * U - a.sp0;
+    #pragma unroll
+                            for (int e = 0; e < U; ++e)
+                                if (ps0 + e >= 0 && ps0 + e < a.snp) prefetch_l2(srcp + static_cast<size_t>(ps0 + e) * a.snl);
                         }
                     }
-                    if (src_tile && src_line && p0 < a.sp0 + a.snp && p0 + U > a.sp0) {
-#pragma unroll
+                    // ---- shared memory -> registers
+                    mbar_wait(bar32 + 8 * slot, phase);
+                    draw_ahead();   // (thread 0) the ticket's round trip overlaps this stage's first half
+                    const unsigned char* st = sm + slot * K::STAGE_BYTES;
+                    if (++slot == NSTAGE) { slot = 0; phase ^= 1; }
+                    [[maybe_unused]] T wp[U], wl, wr;
+                    T wc[U];
+                    if constexpr (DIR == 0) {
+                        const unsigned char* tp = st + tix * 4096;
+                        load_unit_x<T, U>(tp, lane, sub, wp);
+                        load_unit_x<T, U>(tp + K::FIELD_BYTES, lane, sub, wc);
+                        if (sub > 0) wl = tile_elem_x<T>(tp, lane, sub * U - 1);
+                        else if (tix > 0) wl = tile_elem_x<T>(tp - 4096, lane, K::TU - 1);
+                        else wl = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES)[lane * V + V - 1];
+                        if (sub < SUB - 1) wr = tile_elem_x<T>(tp, lane, (sub + 1) * U);
+                        else if (tix < NT - 1) wr = tile_elem_x<T>(tp + 4096, lane, 0);
+                        else wr = reinterpret_cast<const T*>(st + 2 * K::FIELD_BYTES + K::EDGE_BYTES)[lane * V];
+                    } else if constexpr (ONE) {
+                        const T* ccv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
+    #pragma unroll
+                        for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
+                    } else {
+                        const T* cpv = reinterpret_cast<const T*>(st) + (warp * U) * TL + lane;
+                        const T* ccv = reinterpret_cast<const T*>(st + K::FIELD_BYTES) + (warp * U + 1) * TL + lane;
+                        wl = cpv[0];
+    #pragma unroll
+                        for (int e = 0; e < U; ++e) wp[e] = cpv[(e + 1) * TL];
+                        wr = cpv[(U + 1) * TL];
+    #pragma unroll
+                        for (int e = 0; e < U; ++e) wc[e] = ccv[e * TL];
+                    }
+                    // ---- RHS + local forward elimination
+                    const bool fast = g >= kb && p0 + U <= n;   // stationary pivots, whole unit inside the line
+                    T Aval;
+                    if (fast) {   // y_e = rho y_{e-1} + inv r_e from y_{-1} = 0
+    #pragma unroll
                         for (int e = 0; e < U; ++e) {
-                            const int ps = p0 + e - a.sp0;
-                            if (ps >= 0 && ps < a.snp) xl[e] = fmaT(qi, srcp[static_cast<size_t>(ps) * a.snl], xl[e]);
+                            if constexpr (ONE) {
+                                xl[e] = inv * wc[e];
+                            } else {
+                                const T left = e == 0 ? wl : wp[e - 1];
+                                const T right = e == U - 1 ? wr : wp[e + 1];
+                                xl[e] = fmaT(g2i, wc[e], fmaT(ami, left + right, c1i * wp[e]));
+                            }
                         }
-                    }
-#pragma unroll
-                    for (int e = 1; e < U; ++e) xl[e] = fmaT(rho, xl[e - 1], xl[e]);
-                    Aval = pw_at(U - 1);
-                } else {
-                    const bool src_unit = src_tile && src_line;
-                    T fy = T(0), prod = T(1);
-#pragma unroll
-                    for (int e = 0; e < U; ++e) {
-                        const int p = p0 + e;
-                        T r;
-                        if constexpr (ONE) {
-                            r = wc[e];
-                        } else {
-                            const T left = e == 0 ? wl : wp[e - 1];
-                            const T right = e == U - 1 ? wr : wp[e + 1];
-                            r = fmaT(g2, wc[e], fmaT(am, left + right, c1 * wp[e]));
+                        if constexpr (PDENSE) {
+                            if (src_unit) {
+    #pragma unroll
+                                for (int e = 0; e < U; ++e) xl[e] = fmaT(qi, sv[e], xl[e]);
+                            }
+                        } else if constexpr (PSRC) {
+                            if (src_unit) {
+    #pragma unroll
+                                for (int e = 0; e < U; ++e) {
+                                    const int ps = p0 + e - a.sp0;
+                                    if (ps >= 0 && ps < a.snp) xl[e] = fmaT(qi, srcp[static_cast<size_t>(ps) * a.snl], xl[e]);
+                                }
+                            }
                         }
-                        if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
-                            r = fmaT(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
-                        const T cpe = cp_at(p);
-                        fy = fmaT(cpe, fy, r * inv_at(p));
-                        if (p >= n) fy = T(0);
-                        prod *= cpe;
-                        xl[e] = fy;
+    #pragma unroll
+                        for (int e = 1; e < U; ++e) xl[e] = fmaT(rho, xl[e - 1], xl[e]);
+                        Aval = pw_at(U - 1);
+                    } else {
+                        T fy = T(0), prod = T(1);
+    #pragma unroll
+                        for (int e = 0; e < U; ++e) {
+                            const int p = p0 + e;
+                            T r;
+                            if constexpr (ONE) {
+                                r = wc[e];
+                            } else {
+                                const T left = e == 0 ? wl : wp[e - 1];
+                                const T right = e == U - 1 ? wr : wp[e + 1];
+                                r = fmaT(g2, wc[e], fmaT(am, left + right, c1 * wp[e]));
+                            }
+                            if constexpr (PDENSE) {
+                                if (src_unit) r = fmaT(q, sv[e], r);
+                            } else if constexpr (PSRC) {
+                                if (src_unit && p >= a.sp0 && p < a.sp0 + a.snp)
+                                    r = fmaT(q, srcp[static_cast<size_t>(p - a.sp0) * a.snl], r);
+                            }
+                            const T cpe = cp_at(p);
+                            fy = fmaT(cpe, fy, r * inv_at(p));
+                            if (p >= n) fy = T(0);
+                            prod *= cpe;
+                            xl[e] = fy;
+                        }
+                        Aval = prod;
                     }
-                    Aval = prod;
-                }
-                s_L[ring * TL + lane] = xl[U - 1];
-                if (lane == 0) s_A[ring] = Aval;
-                named_bar_sync(1, NW * 32);
-                produce();   // every warp holds its stage data in registers: refill the slot
+                    s_L[ring * TL + lane] = xl[U - 1];
+                    if (lane == 0) s_A[ring] = Aval;
+                    named_bar_sync(1, NW * 32);
+                    produce();   // every warp holds its stage data in registers: refill the slot
 
-                // ---- carry from the left, local back substitution
-                const T Yin = carry(sL_lane, s_A, ring, -1, g - nbk >= kb && p0 <= n);   // y at the end of unit g-1
-                if (fast) {
-                    xl[U - 1] = fmaT(pw_at(U - 1), Yin, xl[U - 1]);
-#pragma unroll
-                    for (int e = U - 2; e >= 0; --e) xl[e] = fmaT(rho, xl[e + 1], fmaT(pw_at(e), Yin, xl[e]));
-                } else {
-                    T c = Yin;
-#pragma unroll
-                    for (int e = 0; e < U; ++e) {
-                        c *= cp_at(p0 + e);
-                        xl[e] = p0 + e < n ? xl[e] + c : T(0);
+                    // ---- carry from the left, local back substitution
+                    const T Yin = carry(sL_lane, s_A, ring, -1, g - nbk >= kb && p0 <= n);   // y at the end of unit g-1
+                    if (fast) {
+                        xl[U - 1] = fmaT(pw_at(U - 1), Yin, xl[U - 1]);
+    #pragma unroll
+                        for (int e = U - 2; e >= 0; --e) xl[e] = fmaT(rho, xl[e + 1], fmaT(pw_at(e), Yin, xl[e]));
+                    } else {
+                        T c = Yin;
+    #pragma unroll
+                        for (int e = 0; e < U; ++e) {
+                            c *= cp_at(p0 + e);
+                            xl[e] = p0 + e < n ? xl[e] + c : T(0);
+                        }
+    #pragma unroll
+                        for (int e = U - 2; e >= 0; --e) xl[e] = fmaT(cp_at(p0 + e), xl[e + 1], xl[e]);
                     }
-#pragma unroll
-                    for (int e = U - 2; e >= 0; --e) xl[e] = fmaT(cp_at(p0 + e), xl[e + 1], xl[e]);
-                }
-                s_H[ring * TL + lane] = xl[0];
-                if (lane == 0) s_AH[ring] = Aval;
-                named_bar_sync(1, NW * 32);
+                    s_H[ring * TL + lane] = xl[0];
+                    if (lane == 0) s_AH[ring] = Aval;
+                    named_bar_sync(1, NW * 32);
 
-                // ---- carry from the right, store
-                if constexpr (DEF) {
-                    if (s > 0) finish(pend, g - NW, ring ^ NW, pc);
-#pragma unroll
-                    for (int e = 0; e < U; ++e) pend[e] = xl[e];
-                } else {
-                    finish(xl, g, ring, pc);
+                    // ---- carry from the right, store
+                    if constexpr (DEF) {
+                        if (s > 0) finish(pend, g - NW, ring ^ NW, pc);
+    #pragma unroll
+                        for (int e = 0; e < U; ++e) pend[e] = xl[e];
+                    } else {
+                        finish(xl, g, ring, pc);
+                    }
                 }
-            }
+            };
+            stages(std::integral_constant<bool, SRC>{});
             // ---- flush: the deferred units of the last stage see zero heads beyond it
             const int ringf = (pc.nst & 1) * NW + warp;
             named_bar_sync(1, NW * 32);   // the deferred warps have read the heads of stage nst-2 (same half of the ring)
@@ -696,6 +738,25 @@ __global__ void wave2d_apply_y(T* __restrict__ out, const T* __restrict__ in, in
     const long long o = j * pitch + i;
     const T up = j > 0 ? in[o - pitch] : T(0), dn = j < n2 - 1 ? in[o + pitch] : T(0), c0 = in[o];
     out[o] = c0 - static_cast<T>(ay) * (up - T(2) * c0 + dn);
+}
+
+// Second-order start of the three-level scheme (2.8) (option "start" = 2, scheme 1; one-time):
+// u1 += ax (phi[i-1] - 2 phi + phi[i+1]) + ay (phi[j-1] - 2 phi + phi[j+1]) + qs s,  ax = tau^2 c^0 / (2 h1^2), ay likewise,
+// qs = tau^2 g^0 / 2, zero ghosts (2.10); s: compact source window [j - j0][i - i0] or NULL.
+template <typename T>
+__global__ void wave2d_start2(T* __restrict__ u1, const T* __restrict__ phi, int n1, int n2, long long pitch, double ax,
+                              double ay, double qs, const T* __restrict__ s, int i0, int j0, int sw, int sh)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= n1 || j >= n2) return;
+    const long long o = j * pitch + i;
+    const T c0 = phi[o];
+    const T we = i > 0 ? phi[o - 1] : T(0), ea = i < n1 - 1 ? phi[o + 1] : T(0);
+    const T so = j > 0 ? phi[o - pitch] : T(0), no = j < n2 - 1 ? phi[o + pitch] : T(0);
+    T v = static_cast<T>(ax) * (we - T(2) * c0 + ea) + static_cast<T>(ay) * (so - T(2) * c0 + no);
+    if (s != nullptr && i >= i0 && i < i0 + sw && j >= j0 && j < j0 + sh)
+        v += static_cast<T>(qs) * s[static_cast<size_t>(j - j0) * sw + (i - i0)];
+    u1[o] += v;
 }
 
 // dst[p][l] = src[l][p] for a small window (compact source, transposed copy for the x sweep)

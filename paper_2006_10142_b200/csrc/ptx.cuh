@@ -83,6 +83,9 @@ __device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wai
 // make generic-proxy writes to shared memory visible to the async proxy (before a TMA store)
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// bring the cache line of p into L2 (no register, no wait)
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // ---- programmatic dependent launch ------------------------------------------------------------------
 // launch_dependents: the next kernel in the stream may start launching (its CTAs take SMs as ours exit);
 // wait: block until the previous kernel in the stream has completed and its writes are visible.

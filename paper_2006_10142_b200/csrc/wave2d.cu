@@ -30,25 +30,33 @@ struct Variant {
     int vec;                                               // grid lines per lane (2: fp32 y sweep on vec2f)
     int one;                                               // 1: single-input y sweep of scheme 1
     const void* fn;
+    const void* fn_nosrc;                                  // the same shape compiled without the source term, or NULL
+    const void* fn_dense;                                  // ... for a source on much of the grid, or NULL
 };
 
-template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB = 1, bool ONE = false>
+// NOSRC: also instantiate the shape without the source term and for a dense source (the default shapes)
+template <typename T, int DIR, int UT, int NW, int NSTAGE, int MINB = 1, bool ONE = false, bool NOSRC = false>
 Variant make_variant()
 {
     using K = PanelCfg<T, DIR, UT, NW, NSTAGE, ONE>;
     constexpr int VEC = std::is_same<T, vec2f>::value ? 2 : 1;
+    const void *nosrc = nullptr, *dense = nullptr;
+    if constexpr (NOSRC) {
+        nosrc = reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB, ONE, 0>);
+        dense = reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB, ONE, 2>);
+    }
     return Variant{DIR, NW, NSTAGE, UT, K::SUB, K::SMEM_BYTES, K::THREADS, (int)sizeof(T) / VEC, VEC, ONE ? 1 : 0,
-                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB, ONE>)};
+                   reinterpret_cast<const void*>(&wave2d_sweep_panel<T, DIR, UT, NW, NSTAGE, MINB, ONE, 1>), nosrc, dense};
 }
 
 constexpr int NVAR = 4;   // shape variants per (dtype, dir); index 0 is the default
 void add_shapes_f64(std::vector<Variant>& v)
 {
-    v.push_back(make_variant<double, 0, 8, 16, 2>());
+    v.push_back(make_variant<double, 0, 8, 16, 2, 1, false, true>());
     v.push_back(make_variant<double, 0, 8, 8, 2, 2>());
     v.push_back(make_variant<double, 0, 16, 8, 2>());
     v.push_back(make_variant<double, 0, 4, 16, 2>());
-    v.push_back(make_variant<double, 1, 8, 16, 2>());
+    v.push_back(make_variant<double, 1, 8, 16, 2, 1, false, true>());
     v.push_back(make_variant<double, 1, 8, 8, 3, 2>());
     v.push_back(make_variant<double, 1, 16, 8, 3>());
     v.push_back(make_variant<double, 1, 8, 16, 3>());
@@ -62,12 +70,12 @@ void add_shapes_one(std::vector<Variant>& v)   // scheme 1 y sweep; shape index 
 }
 void add_shapes_f32(std::vector<Variant>& v)
 {
-    v.push_back(make_variant<float, 0, 16, 16, 2>());
+    v.push_back(make_variant<float, 0, 16, 16, 2, 1, false, true>());
     v.push_back(make_variant<float, 0, 16, 8, 2, 2>());
     v.push_back(make_variant<float, 0, 32, 8, 2>());
     v.push_back(make_variant<float, 0, 8, 16, 2>());
-    v.push_back(make_variant<vec2f, 1, 8, 16, 2>());    // two columns per lane; not with a source (falls to shape 1)
-    v.push_back(make_variant<float, 1, 8, 8, 3, 2>());
+    v.push_back(make_variant<vec2f, 1, 8, 16, 2, 1, false, true>());    // two columns per lane; not with a source (falls to shape 1)
+    v.push_back(make_variant<float, 1, 8, 8, 3, 2, false, true>());   // (the fp32 y sweep of a run with a source)
     v.push_back(make_variant<float, 1, 16, 8, 3>());
     v.push_back(make_variant<float, 1, 8, 16, 4>());
 }
@@ -134,7 +142,8 @@ struct DirPlan {
 
 struct wave2d_s {
     int N1, N2, n1, n2, M, dtype, elem;
-    double l, tau, gamma = 2.0, kappa = 0.5;
+    double l, tau, gamma = 2.0, kappa = 0.5, sigma = 0.5;
+    int opt_start = 1;                   // scheme 1: 1 = (2.9) as printed, 2 = second-order start
     int opt_solver = WAVE2D_SOLVER_AUTO, opt_graph = 1, opt_graph_steps = MAX_CHUNK, opt_shape[2] = {0, 0};
     int opt_quota[2] = {0, 0};
     cudaStream_t own_stream = nullptr, stream = nullptr;
@@ -279,8 +288,9 @@ void build_table(wave2d_t* h)
     }
     for (int n = 0; n < nhalf; ++n) {
         const double hd = h->l / ((n & 1) == 0 ? h->N1 : h->N2);                  // reading R3
-        const double ap = t2 * h->c_half[n + 1] / (2.0 * hd * hd);
-        const double am = t2 * h->c_half[n > 0 ? n - 1 : 0] / (2.0 * hd * hd);      // reading R5: c_{-1} := c_0
+        // sigma = 1/2: (2.11)-(2.12); sigma = 1: the fully implicit weights of Listing 1
+        const double ap = h->sigma * t2 * h->c_half[n + 1] / (hd * hd);
+        const double am = (1.0 - h->sigma) * t2 * h->c_half[n > 0 ? n - 1 : 0] / (hd * hd);   // reading R5: c_{-1} := c_0
         const double g = h->g_half.empty() ? 1.0 : h->g_half[n];                   // reading R8
         fill_row(&h->table[static_cast<size_t>(n) * ROW_DOUBLES], h->gamma, ap, am, h->have_src ? h->kappa * t2 * g : 0.0);
     }
@@ -561,6 +571,8 @@ int plan_dir(wave2d_t* h, int d)
     P.halo = nbk * U;
     P.kb = (pconv + U - 1) / U;
     W2D_CUDA(h, cudaFuncSetAttribute(V.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, V.smem));
+    if (V.fn_nosrc) W2D_CUDA(h, cudaFuncSetAttribute(V.fn_nosrc, cudaFuncAttributeMaxDynamicSharedMemorySize, V.smem));
+    if (V.fn_dense) W2D_CUDA(h, cudaFuncSetAttribute(V.fn_dense, cudaFuncAttributeMaxDynamicSharedMemorySize, V.smem));
     int per_sm = 0;
     W2D_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, V.fn, V.threads, V.smem));
     if (per_sm < 1) {
@@ -809,7 +821,10 @@ int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own
         // Only behind a sweep of the same chunk: the first sweep of a chunk follows wave2d_end_chunk (or a copy) and
         // reads the step counter before griddepcontrol.wait, so it must see it final.
         cfg.numAttrs = h->opt_pdl && after_own ? 1 : 0;
-        W2D_CUDA(h, cudaLaunchKernelExC(&cfg, P.var->fn, args));
+        // a window that covers more than 1/8 of the grid counts as dense (kernels.cuh, SRCM)
+        const bool dense = src != nullptr && 8.0 * h->win_w * h->win_h > (double)h->n1 * h->n2;
+        const void* fn = src == nullptr && P.var->fn_nosrc ? P.var->fn_nosrc : dense && P.var->fn_dense ? P.var->fn_dense : P.var->fn;
+        W2D_CUDA(h, cudaLaunchKernelExC(&cfg, fn, args));
         return WAVE2D_OK;
     }
     // exact path: the whole-line solver of the direction (exact.cuh)
@@ -936,6 +951,21 @@ int set_initial_factored(wave2d_t* h, const void* phi, const void* psi, long ld)
 // Scheme 1: V^0 = (I - ay(c^0) Dy) U^0 -> buf[1], V^1 = (I - ay(c^1) Dy) U^1 -> buf[2]   (roles of solve t = 0)
 int init_factored_v(wave2d_t* h)
 {
+    if (h->opt_start == 2) {   // U^1 += tau^2 / 2 (c^0 Lap_h phi + g^0 s): U^0 = phi in buf[3], U^1 in buf[0]
+        const double h1 = h->l / h->N1, hy = h->l / h->N2, ht2 = 0.5 * h->tau * h->tau;
+        const double g0 = h->have_src ? (h->g_half.empty() ? 1.0 : h->g_half[0]) : 0.0;
+        const dim3 blk(128), grd((h->n1 + 127) / 128, h->n2);
+        if (h->dtype == WAVE2D_F64)
+            wave2d_start2<double><<<grd, blk, 0, h->stream>>>((double*)h->buf[0], (const double*)h->buf[3], h->n1, h->n2, h->pitch,
+                                                              ht2 * h->c_half[0] / (h1 * h1), ht2 * h->c_half[0] / (hy * hy), ht2 * g0,
+                                                              (const double*)h->src_dev[1], h->win_i0, h->win_j0, h->win_w, h->win_h);
+        else
+            wave2d_start2<float><<<grd, blk, 0, h->stream>>>((float*)h->buf[0], (const float*)h->buf[3], h->n1, h->n2, h->pitch,
+                                                             ht2 * h->c_half[0] / (h1 * h1), ht2 * h->c_half[0] / (hy * hy), ht2 * g0,
+                                                             (const float*)h->src_dev[1], h->win_i0, h->win_j0, h->win_w, h->win_h);
+        W2D_CUDA(h, cudaGetLastError());
+        h->launches += 1;
+    }
     const double h2 = h->l / h->N2, t2 = h->tau * h->tau;
     const double ay0 = t2 * h->c_half[0] / (2.0 * h2 * h2), ay1 = t2 * h->c_half[2] / (2.0 * h2 * h2);
     const dim3 blk(128), grd((h->n1 + 127) / 128, h->n2);
@@ -1043,9 +1073,18 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     const int iv = (int)value;
     if (!strcmp(name, "gamma")) { if (!(value > 0.0)) return WAVE2D_ERR_ARG; h->gamma = value; }
     else if (!strcmp(name, "kappa")) h->kappa = value;
+    else if (!strcmp(name, "sigma")) {
+        if (!(value > 0.0 && value <= 1.0)) return WAVE2D_ERR_ARG;
+        if (h->scheme == 1 && value != 0.5) return WAVE2D_ERR_UNSUPPORTED;   // (2.8) has the weight 1/2 by definition
+        h->sigma = value;
+    }
+    else if (!strcmp(name, "start")) {
+        if (iv != 1 && iv != 2) return WAVE2D_ERR_ARG;
+        h->opt_start = iv;
+    }
     else if (!strcmp(name, "scheme")) {
         if ((iv != 0 && iv != 1) || h->have_initial) return WAVE2D_ERR_ARG;
-        if (iv == 1 && h->have_cs) return WAVE2D_ERR_UNSUPPORTED;   // variable speed: split scheme only
+        if (iv == 1 && (h->have_cs || h->sigma != 0.5)) return WAVE2D_ERR_UNSUPPORTED;   // variable speed, sigma: split scheme only
         if (iv == 1 && !h->buf[3]) {
             const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
             int st = dev_alloc(h, &h->buf[3], fbytes);
@@ -1218,6 +1257,7 @@ int wave2d_run(wave2d_t* h, int steps)
     if (!h || steps < 0) return WAVE2D_ERR_ARG;
     if (!h->have_initial) return WAVE2D_ERR_STATE;
     if ((long long)h->k + steps > h->M) return WAVE2D_ERR_RANGE;
+    if (h->scheme == 0 && h->opt_start != 1) return WAVE2D_ERR_UNSUPPORTED;   // (2.9) belongs to the three-level scheme (2.8)
     int st = ensure_plan(h);   // also builds the graphs: wave2d_run(h, 0) prepares everything
     if (st) return st;
     if (steps > 0) h->ran = true;

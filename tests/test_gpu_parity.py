@@ -941,3 +941,96 @@ def test_variable_speed_full_grid_4095():
     u, info = gpu_var(w, cs)
     assert info["strip_y"] == 2                          # r and a_p of 2 columns x 4095 rows on chip
     assert relerr(u, r) <= 1e-10
+
+
+# ---- SURVEY.md 8f NEXT-4, the rest: the weight sigma (Listing 1: sigma = 1) and the second-order start of (2.8) ----------
+@pytest.mark.parametrize("sigma,gamma", [(1.0, 1.0), (1.0, 2.0), (0.75, 2.0)])
+@pytest.mark.parametrize("name,w", [("cfg1", W.cfg1()), ("cfg2_N700", W.cfg2(N=700, M=30)),
+                                    ("cfg3_N1000", W.cfg3(N=1000, M=250)), ("cfg4_1030x270", W.cfg4(N1=1030, N2=270, M=24))],
+                         ids=["cfg1", "cfg2_N700", "cfg3_N1000", "cfg4_1030x270"])
+def test_sigma_weight_matches_oracle_on_every_solver_path(name, w, sigma, gamma):
+    """Option "sigma": sigma = 1, gamma = 1 is the system Listing 1 prints.  The weights enter through
+    the per-half-step scalars only, so every kernel family must agree with the oracle's sigma mode."""
+    r = oracle.solve(w.N1, w.N2, w.l, w.tau, w.M, w.phi, w.psi, c_half=w.c_half, s=w.s, g_half=w.g_half, gamma=gamma,
+                     sigma=sigma)
+    for opts in ({}, {"solver": B.SOLVER_STREAM}, {"solver": B.SOLVER_EXACT}):
+        u, info = gpu(w, gamma=gamma, sigma=sigma, **opts)
+        assert relerr(u, r) <= 1e-10, (opts, relerr(u, r))
+    assert relerr(r, ref(w)) > 1e-4      # and sigma changes the answer
+
+
+def test_sigma_with_variable_speed_and_fp32():
+    w = W.cfg4(N1=300, N2=200, M=20, dtype="f32")
+    rng = np.random.default_rng(5)
+    cs = rng.uniform(0.5, 1.5, (w.n2, w.n1)).astype(np.float32)
+    r = oracle.solve(w.N1, w.N2, w.l, w.tau, w.M, w.phi, w.psi, c_half=w.c_half, cs=cs.astype(np.float64), sigma=1.0)
+    h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, "f32")
+    try:
+        h.set_option("sigma", 1.0)
+        h.set_speed(w.c_half)
+        h.set_speed_field(cs)
+        h.set_initial(w.phi.astype(np.float32))
+        h.run(w.M)
+        u = h.get()
+    finally:
+        h.close()
+    assert relerr(u, r) <= 1e-4
+
+
+@pytest.mark.parametrize("N1,N2", [(96, 80), (700, 300), (1500, 1200)])
+def test_second_order_start_of_the_factored_scheme(N1, N2):
+    """Option "start" = 2 (scheme 1): u^1 = phi + tau psi + tau^2/2 (c^0 Lap_h phi + g^0 s); small-grid kernel, streamed
+    kernels and exact solvers; the term is added at the first run."""
+    M = 12
+    rng = np.random.default_rng(N1 + N2)
+    w = W.cfg2(N=N1, M=M)
+    shape = (N2 - 1, N1 - 1)
+    yy, xx = np.meshgrid(np.arange(1, N2) / N2, np.arange(1, N1) / N1, indexing="ij")
+    phi = np.exp(-((xx - 0.4) ** 2 + (yy - 0.55) ** 2) / 0.02)
+    psi = np.sin(3 * np.pi * xx) * np.sin(2 * np.pi * yy)
+    s = np.zeros(shape)
+    s[N2 // 3:N2 // 3 + 20, N1 // 4:N1 // 4 + 30] = rng.uniform(-1, 1, (20, 30))
+    g = np.cos(np.arange(2 * M) * 0.2) + 0.5
+    tau = 1.0 / max(N1, N2)
+    c = w.c_half
+    r = oracle.solve(N1, N2, 1.0, tau, M, phi, psi, c_half=c, s=s, g_half=g, scheme=1, start=2)
+    r1 = oracle.solve(N1, N2, 1.0, tau, M, phi, psi, c_half=c, s=s, g_half=g, scheme=1)
+    assert relerr(r1, r) > 1e-6
+    for opts in ({}, {"solver": B.SOLVER_EXACT}):
+        h = B.Wave2D(N1, N2, 1.0, tau, M, "f64")
+        try:
+            h.set_option("scheme", 1)
+            h.set_option("start", 2)
+            for k, v in opts.items():
+                h.set_option(k, v)
+            h.set_initial(phi, psi)                      # before the speed and the source: the term waits for the run
+            h.set_speed(c)
+            h.set_source(s, g)
+            np.testing.assert_allclose(h.get(), phi + tau * psi, rtol=0, atol=1e-15)
+            h.run(M - 1)
+            u = h.get()
+        finally:
+            h.close()
+        assert relerr(u, r) <= 1e-10, (opts, relerr(u, r))
+
+
+def test_sigma_and_start_are_refused_where_they_do_not_apply():
+    h = B.Wave2D(64, 64, 1.0, 0.01, 4, "f64")
+    try:
+        h.set_option("start", 2)
+        h.set_initial(np.ones((63, 63)))
+        with pytest.raises(B.Wave2DError) as e:
+            h.run(1)
+        assert e.value.status == -5
+    finally:
+        h.close()
+    h = B.Wave2D(64, 64, 1.0, 0.01, 4, "f64")
+    try:
+        h.set_option("scheme", 1)
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_option("sigma", 1.0)
+        assert e.value.status == -5
+        with pytest.raises(B.Wave2DError):
+            h.set_option("sigma", 0.0)
+    finally:
+        h.close()
