@@ -168,6 +168,8 @@ struct wave2d_s {
     bool plan_ok = false;
     DirPlan plan[2];
     bool line_mode = false;              // small grid: the step loop runs in wave2d_line_steps (line.cuh)
+    bool line_resident = false;          // ... in wave2d_line_resident: the fields stay in the cluster's shared memory
+    int opt_resident = 1;
     const void* line_fn = nullptr;
     int line_unit = 0, line_ctas = 0, line_smem = 0;
     SweepMaps maps[2];                   // per direction: TMA descriptors of every ring buffer
@@ -602,6 +604,8 @@ constexpr int LINE_WARPS = 16;   // warps per CTA of the small-grid kernel
 
 template <typename T, int U>
 const void* line_kernel() { return reinterpret_cast<const void*>(&wave2d_line_steps<T, U, LINE_WARPS>); }
+template <typename T, int U>
+const void* resident_kernel() { return reinterpret_cast<const void*>(&wave2d_line_resident<T, U, LINE_WARPS>); }
 
 int plan_line(wave2d_t* h)
 {
@@ -622,10 +626,22 @@ int plan_line(wave2d_t* h)
     if (h->dtype == WAVE2D_F64) h->line_fn = U == 4 ? line_kernel<double, 4>() : line_kernel<double, 8>();
     else h->line_fn = U == 4 ? line_kernel<float, 4>() : line_kernel<float, 8>();
     h->line_smem = 2 * 16 * (32 * U + 1) * h->elem;
-    W2D_CUDA(h, cudaFuncSetAttribute(h->line_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->line_smem));
     // one CTA per 16 rows of the x half-step / per 16-column strip of the y half-step, at most one portable cluster
     const int want = std::max((h->n2 + LINE_WARPS - 1) / LINE_WARPS, (h->n1 + 15) / 16);
     h->line_ctas = std::max(1, std::min(8, want));
+    // Split scheme, six line buffers per CTA within shared memory: the fields stay on chip for the whole launch
+    h->line_resident = false;
+    if (h->scheme == 0 && h->opt_resident) {
+        const int lb = std::max((h->n2 + h->line_ctas - 1) / h->line_ctas, (h->n1 + h->line_ctas - 1) / h->line_ctas);
+        const size_t need = (size_t)6 * lb * (32 * U + 1) * h->elem;
+        if (need <= 200 * 1024) {
+            h->line_resident = true;
+            h->line_smem = (int)need;
+            if (h->dtype == WAVE2D_F64) h->line_fn = U == 4 ? resident_kernel<double, 4>() : resident_kernel<double, 8>();
+            else h->line_fn = U == 4 ? resident_kernel<float, 4>() : resident_kernel<float, 8>();
+        }
+    }
+    W2D_CUDA(h, cudaFuncSetAttribute(h->line_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, h->line_smem));
     for (int d = 0; d < 2; ++d) {
         DirPlan& P = h->plan[d];
         P = DirPlan();
@@ -1101,6 +1117,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     }
     else if (!strcmp(name, "shape_x")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[0] = iv; }
     else if (!strcmp(name, "shape_y")) { if (iv < 0 || iv >= NVAR) return WAVE2D_ERR_ARG; h->opt_shape[1] = iv; }
+    else if (!strcmp(name, "resident")) h->opt_resident = iv != 0;
     else if (!strcmp(name, "trace")) h->opt_trace = iv != 0;
     else if (!strcmp(name, "pdl")) h->opt_pdl = iv != 0;
     else if (!strcmp(name, "early")) h->opt_early = iv != 0;
@@ -1350,6 +1367,7 @@ int wave2d_get_info(wave2d_t* h, const char* name, double* value)
         else if (key == "threads") *value = 32 * LINE_WARPS;
         else if (key == "smem") *value = h->line_smem;
         else if (key == "unit") *value = h->line_unit;
+        else if (key == "resident") *value = h->line_resident ? 1 : 0;
         else if (key == "ctas_per_sm") *value = 1;
         else if (key == "chunks") *value = 1;
         else if (key == "halo" || key == "nbk" || key == "kb" || key == "upc" || key == "quota" || key == "static" ||
