@@ -60,6 +60,10 @@ def parse_args():
     ap.add_argument("--dense-source", action="store_true",
                     help="off-config: replace the workload's source shape by one that is non-zero on the whole grid "
                          "(wave2d_set_source with a full grid: + 1 field read per sweep)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="off-default (SURVEY.md 8f NEXT-3): ONE simulation over the N ranks -- every rank owns a row block "
+                         "with halo rows refreshed from its neighbours after every step (paper_2006_10142_b200/sharded.py); "
+                         "strong scaling.  The default for N > 1 stays N independent replicas (north_star: no sharding)")
     ap.add_argument("--solver", type=int, default=0, choices=[0, 1, 2, 3],
                     help="off-default: wave2d_set_option('solver'): 0 auto, 1 exact whole-line, 2 streamed, 3 small-grid cluster")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
@@ -478,10 +482,72 @@ def run_ours(args):
     ranks.close()
 
 
+def run_sharded(args):
+    """One simulation sharded by grid rows over the ranks; a step = run(1) on every block + the halo refresh."""
+    import torch
+    from paper_2006_10142_b200.replicas import Ranks
+    from paper_2006_10142_b200 import build as _build, sharded as S
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the hot path is CUDA only, there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if local == 0:
+        _build.build()
+    else:
+        for _ in range(600):
+            if not _build.needs_build():
+                break
+            time.sleep(0.5)
+    dev = torch.device("cuda", local)
+    ranks = Ranks("nccl", dev)
+    K, Wm = args.steps, args.warmup
+    w = load_workload(args.workload, Wm + K + 2)
+    shards, G = S.make_shards(w.N1, w.N2, w.l, w.tau, w.M, w.dtype, world, w.phi, w.psi, w.c_half, w.s, w.g_half,
+                              ranks=[rank])
+    sh = shards[0]
+    ex = S.DistExchange(sh, rank, world, dev) if world > 1 else None
+
+    def steps(n):
+        for _ in range(n):
+            sh.step(1)
+            if ex is not None:
+                ex.refresh()
+
+    sh.engine.run(0)
+    steps(Wm)
+    sh.engine.sync()
+    ranks.barrier(); torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    steps(K)
+    sh.engine.sync()
+    ranks.barrier(); torch.cuda.synchronize()
+    sec = ranks.max_over_ranks(time.perf_counter() - t0)   # (run(1) + get/set_rows synchronise the stream every step)
+    peak, peak_src = measured_peaks()
+    esz = 8 if w.dtype == "f64" else 4
+    line = {"metric": METRIC, "value": w.points * K / sec / 1e9, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": sec / K * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": w.dtype, "data": "synthetic",
+            "config": {"workload": w.name + " sharded by grid rows (off-default, SURVEY.md 8f NEXT-3)", "N1": w.N1, "N2": w.N2,
+                       "parallelism": f"{world} row blocks, {G} halo rows refreshed per step and cut (NCCL point-to-point)",
+                       "rows_owned": sh.block.b - sh.block.a, "rows_local": sh.block.rows},
+            "gpu_launches": int(sh.engine.info("launches")),
+            "roofline": {"bound": "hbm", "achieved": 6 * w.points * esz * K / sec / 1e9, "peak": peak * world, "unit": "GB/s",
+                         "frac": 6 * w.points * esz * K / sec / 1e9 / (peak * world), "traffic": None, "peak_source": peak_src,
+                         "how": "6 field passes of the whole grid / wall time of K steps incl. the halo exchange, against "
+                                "N x the measured single-GPU peak"},
+            "e2e": None}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    sh.engine.close()
+    ranks.close()
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.sharded:
+        run_sharded(args)
     else:
         run_ours(args)
 

@@ -90,6 +90,7 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "kappa"  source weight.              Default 0.5.   | locally-one-dimensional form of (2.11)-(2.12);
  *                                                       | gamma = kappa = 1 is the scheme as printed
  *                                                       |, which solves u_tt = 2c Lap u + 4f.
+ *   "ly"     extent in y of this grid (h2 = ly / N2); default 0 = l.  For row blocks of a larger domain (wave2d_get_rows).
  *   "sigma"  weight of the implicit operator in the split scheme, in (0, 1].  Default 0.5 = (2.11)-(2.12):
  *            alpha+ = sigma tau^2 c_{n+1} / h_d^2 on w_{n+1}, alpha- = (1 - sigma) tau^2 c_{n-1} / h_d^2 on w_{n-1}.
  *            sigma = 1 with gamma = 1 and c = 1 is the tridiagonal system Listing 1 prints (PAPER.md:157-162:
@@ -184,6 +185,17 @@ int wave2d_run(wave2d_t *h, int steps);
 /* Copy u^k (k = steps done so far) / u^{k-1/2} to u_out (host or device).  Synchronises the stream. */
 int wave2d_get(wave2d_t *h, void *u_out, long ld);
 int wave2d_get_prev(wave2d_t *h, void *u_out, long ld);
+
+/*
+ * Row blocks of a time level (split scheme only; ERR_UNSUPPORTED with scheme 1): rows [j0, j0 + count) of level 0 = u^k or
+ * level 1 = u^{k-1/2}, `count` rows of n1 values, row stride ld >= n1, host or device pointer.  wave2d_get_rows copies
+ * them out, wave2d_set_rows overwrites them (both synchronise the handle's stream).  With option "ly" (the extent in y of
+ * THIS grid, h2 = ly / N2, default l) a handle can hold a row block of a larger domain plus halo rows: the step of the
+ * block is exact up to rho^G in its interior when G halo rows per side are refreshed from the neighbouring blocks after
+ * every step (paper_2006_10142_b200/sharded.py).  Errors: ERR_ARG, ERR_STATE (no initial data).
+ */
+int wave2d_get_rows(wave2d_t *h, int level, int j0, int count, void *out, long ld);
+int wave2d_set_rows(wave2d_t *h, int level, int j0, int count, const void *in, long ld);
 
 /* Number of completed time steps k. */
 int wave2d_steps_done(const wave2d_t *h, int *k);

@@ -21,7 +21,7 @@ EXPORTS = [
     "wave2d_create", "wave2d_destroy", "wave2d_set_stream", "wave2d_set_option", "wave2d_set_initial",
     "wave2d_set_state",
     "wave2d_set_speed", "wave2d_set_speed_field", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
-    "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
+    "wave2d_get_rows", "wave2d_set_rows", "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
     "wave2d_host_scalars", "wave2d_host_plan", "wave2d_strerror", "wave2d_last_error",
 ]
 
@@ -60,6 +60,8 @@ def load_library() -> C.CDLL:
     L.wave2d_run.argtypes = [vp, C.c_int]
     L.wave2d_get.argtypes = [vp, vp, C.c_long]
     L.wave2d_get_prev.argtypes = [vp, vp, C.c_long]
+    L.wave2d_get_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, C.c_long]
+    L.wave2d_set_rows.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp, C.c_long]
     L.wave2d_steps_done.argtypes = [vp, ip]
     L.wave2d_sync.argtypes = [vp]
     L.wave2d_get_info.argtypes = [vp, C.c_char_p, dp]
@@ -204,6 +206,30 @@ class Wave2D:
 
     def get_prev(self, out=None):
         return self._out(self._L.wave2d_get_prev, "wave2d_get_prev", out)
+
+    def _rows(self, a, count: int):
+        """-> (pointer, ld, array) for a host/device array of `count` rows of n1 values."""
+        if _is_torch(a):
+            if a.dim() != 2 or tuple(a.shape) != (count, self.n1) or a.stride(1) != 1:
+                raise ValueError(f"expected a torch tensor of shape {(count, self.n1)} with unit inner stride")
+            return C.c_void_p(a.data_ptr()), int(a.stride(0)) if count > 1 else self.n1, a
+        if a.shape != (count, self.n1) or a.dtype != self._np or a.strides[1] != a.itemsize:
+            raise ValueError(f"expected a {self._np.__name__} array of shape {(count, self.n1)} with unit inner stride")
+        return C.c_void_p(a.ctypes.data), int(a.strides[0] // a.itemsize) if count > 1 else self.n1, a
+
+    def get_rows(self, level: int, j0: int, count: int, out=None):
+        if out is None:
+            out = np.empty((count, self.n1), dtype=self._np)
+        p, ld, _ = self._rows(out, count)
+        self._check(self._L.wave2d_get_rows(self._h, int(level), int(j0), int(count), p, ld), "wave2d_get_rows")
+        return out
+
+    def set_rows(self, level: int, j0: int, rows):
+        if not _is_torch(rows):
+            rows = np.ascontiguousarray(rows, dtype=self._np)
+        count = int(rows.shape[0])
+        p, ld, keep = self._rows(rows, count)
+        self._check(self._L.wave2d_set_rows(self._h, int(level), int(j0), count, p, ld), "wave2d_set_rows")
 
     def steps_done(self) -> int:
         k = C.c_int()

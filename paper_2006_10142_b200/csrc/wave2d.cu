@@ -143,6 +143,7 @@ struct DirPlan {
 struct wave2d_s {
     int N1, N2, n1, n2, M, dtype, elem;
     double l, tau, gamma = 2.0, kappa = 0.5, sigma = 0.5;
+    double ly = 0.0;                     // > 0: extent in y of THIS grid (h2 = ly / N2): a row block of a larger domain
     int opt_start = 1;                   // scheme 1: 1 = (2.9) as printed, 2 = second-order start
     int opt_solver = WAVE2D_SOLVER_AUTO, opt_graph = 1, opt_graph_steps = MAX_CHUNK, opt_shape[2] = {0, 0};
     int opt_quota[2] = {0, 0};
@@ -193,6 +194,8 @@ struct wave2d_s {
 };
 
 namespace {
+
+double step_y(const wave2d_t* h) { return (h->ly > 0.0 ? h->ly : h->l) / h->N2; }
 
 #define W2D_CUDA(h, call)                                                                      \
     do {                                                                                       \
@@ -279,7 +282,7 @@ void build_table(wave2d_t* h)
         // (V^j = (I - ay(c^j) Dy) U^j is carried); a_d^+- = tau^2 c^{k+-1} / (2 h_d^2).
         for (int t = 0; t + 2 <= (constant ? 2 : h->M); ++t) {
             const int k = t + 1;
-            const double h1 = h->l / h->N1, h2 = h->l / h->N2;
+            const double h1 = h->l / h->N1, h2 = step_y(h);
             const double cp1 = h->c_half[2 * (k + 1)], cm1 = h->c_half[2 * (k - 1)];
             const double g = h->g_half.empty() ? 1.0 : h->g_half[2 * k];
             fill_row(&h->table[static_cast<size_t>(2 * t) * ROW_DOUBLES], 1.0, t2 * cp1 / (2.0 * h1 * h1),
@@ -289,7 +292,7 @@ void build_table(wave2d_t* h)
         return;
     }
     for (int n = 0; n < nhalf; ++n) {
-        const double hd = h->l / ((n & 1) == 0 ? h->N1 : h->N2);                  // reading R3
+        const double hd = (n & 1) == 0 ? h->l / h->N1 : step_y(h);                    // reading R3
         // sigma = 1/2: (2.11)-(2.12); sigma = 1: the fully implicit weights of Listing 1
         const double ap = h->sigma * t2 * h->c_half[n + 1] / (hd * hd);
         const double am = (1.0 - h->sigma) * t2 * h->c_half[n > 0 ? n - 1 : 0] / (hd * hd);   // reading R5: c_{-1} := c_0
@@ -968,7 +971,7 @@ int set_initial_factored(wave2d_t* h, const void* phi, const void* psi, long ld)
 int init_factored_v(wave2d_t* h)
 {
     if (h->opt_start == 2) {   // U^1 += tau^2 / 2 (c^0 Lap_h phi + g^0 s): U^0 = phi in buf[3], U^1 in buf[0]
-        const double h1 = h->l / h->N1, hy = h->l / h->N2, ht2 = 0.5 * h->tau * h->tau;
+        const double h1 = h->l / h->N1, hy = step_y(h), ht2 = 0.5 * h->tau * h->tau;
         const double g0 = h->have_src ? (h->g_half.empty() ? 1.0 : h->g_half[0]) : 0.0;
         const dim3 blk(128), grd((h->n1 + 127) / 128, h->n2);
         if (h->dtype == WAVE2D_F64)
@@ -982,7 +985,7 @@ int init_factored_v(wave2d_t* h)
         W2D_CUDA(h, cudaGetLastError());
         h->launches += 1;
     }
-    const double h2 = h->l / h->N2, t2 = h->tau * h->tau;
+    const double h2 = step_y(h), t2 = h->tau * h->tau;
     const double ay0 = t2 * h->c_half[0] / (2.0 * h2 * h2), ay1 = t2 * h->c_half[2] / (2.0 * h2 * h2);
     const dim3 blk(128), grd((h->n1 + 127) / 128, h->n2);
     if (h->dtype == WAVE2D_F64) {
@@ -1089,6 +1092,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     const int iv = (int)value;
     if (!strcmp(name, "gamma")) { if (!(value > 0.0)) return WAVE2D_ERR_ARG; h->gamma = value; }
     else if (!strcmp(name, "kappa")) h->kappa = value;
+    else if (!strcmp(name, "ly")) { if (!(value >= 0.0)) return WAVE2D_ERR_ARG; h->ly = value; }
     else if (!strcmp(name, "sigma")) {
         if (!(value > 0.0 && value <= 1.0)) return WAVE2D_ERR_ARG;
         if (h->scheme == 1 && value != 0.5) return WAVE2D_ERR_UNSUPPORTED;   // (2.8) has the weight 1/2 by definition
@@ -1327,6 +1331,41 @@ int wave2d_get_prev(wave2d_t* h, void* u_out, long ld)
         return WAVE2D_ERR_UNSUPPORTED;
     }
     return copy_out(h, u_out, ld, h->buf[(2 * h->k) % 3]);
+}
+
+// Rows [j0, j0 + count) of a time level: 0 = u^k, 1 = u^{k-1/2} (split scheme only).
+static int rows_of_level(wave2d_t* h, int level, int j0, int count, void** base)
+{
+    if (!h || level < 0 || level > 1 || j0 < 0 || count < 1 || j0 + count > h->n2) return WAVE2D_ERR_ARG;
+    if (h->scheme != 0) return WAVE2D_ERR_UNSUPPORTED;
+    if (!h->have_initial) return WAVE2D_ERR_STATE;
+    const int b = level == 0 ? (2 * h->k + 1) % 3 : (2 * h->k) % 3;
+    *base = static_cast<unsigned char*>(h->buf[b]) + (size_t)j0 * h->pitch * h->elem;
+    return WAVE2D_OK;
+}
+
+int wave2d_get_rows(wave2d_t* h, int level, int j0, int count, void* out, long ld)
+{
+    void* src = nullptr;
+    int st = rows_of_level(h, level, j0, count, &src);
+    if (st) return st;
+    if (!out || ld < h->n1) return WAVE2D_ERR_ARG;
+    W2D_CUDA(h, cudaMemcpy2DAsync(out, (size_t)ld * h->elem, src, (size_t)h->pitch * h->elem, (size_t)h->n1 * h->elem, count,
+                                  cudaMemcpyDefault, h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    return WAVE2D_OK;
+}
+
+int wave2d_set_rows(wave2d_t* h, int level, int j0, int count, const void* in, long ld)
+{
+    void* dst = nullptr;
+    int st = rows_of_level(h, level, j0, count, &dst);
+    if (st) return st;
+    if (!in || ld < h->n1) return WAVE2D_ERR_ARG;
+    W2D_CUDA(h, cudaMemcpy2DAsync(dst, (size_t)h->pitch * h->elem, in, (size_t)ld * h->elem, (size_t)h->n1 * h->elem, count,
+                                  cudaMemcpyDefault, h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));   // the caller may reuse `in`
+    return WAVE2D_OK;
 }
 
 int wave2d_steps_done(const wave2d_t* h, int* k)
