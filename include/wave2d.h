@@ -126,7 +126,7 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *            last drawn pieces begins with a piece of its share that touches only grid lines that sweep completed in
  *            its static part; needs "pdl".  0: every CTA waits for the whole previous sweep.
  *   "trace"  1: sweep kernels record per-CTA timing (see wave2d_get_trace).  Default 0.
- *   "static_frac"          tuning: share of a sweep's work dealt out statically (0..1, default 0.75); the rest is
+ *   "static_frac"          tuning: share of a sweep's work dealt out statically (0..1; default 0.70 in fp64, 0.75 in fp32); the rest is
  *                          drawn from the ticket counter in short pieces.
  *   "tail_min", "tail_max", "tail_div"   tuning of the drawn pieces: shortest / longest length in stages (tail_min 0 =
  *                          planned from the stage size; tail_max default 6) and the divisor d of the guided length

@@ -480,7 +480,8 @@ struct ExactScratch {
 //              points of the next pass's row (and the two neighbour values of a warp) are already on their way;
 //   nseg  > 1: the parked line, nseg * wpc * 32 * U values (no prefetch: the line itself fills shared memory).
 // VAR: variable speed -- one more field (cs) per row, the pivots come from group_pivots, no stationary path.
-template <typename T, bool VAR>
+// SEG1: compiled for lines of one segment (n <= 4096: the segment loops, the parked line and their tests fold away).
+template <typename T, bool VAR, bool SEG1>
 __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, unsigned char* ex_smem, ExactScratch<T>& sc_)
 {
     constexpr int U = EX_U, V = 16 / (int)sizeof(T), NV = U / V;
@@ -499,7 +500,8 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
     [[maybe_unused]] const T ap = static_cast<T>(row[ROW_AP]), gam = static_cast<T>(a.gamma);
     const T g2 = static_cast<T>(a.g2);
     const bool one = a.one != 0;
-    const int n = a.n, seg_pts = wpc * 32 * U, npad = a.nseg * seg_pts;
+    const int nseg = SEG1 ? 1 : a.nseg;
+    const int n = a.n, seg_pts = wpc * 32 * U, npad = nseg * seg_pts;
     const T* const src = static_cast<const T*>(a.src);
     int pf = 0, pb = 0;   // buffer parity of the next forward / backward call
     [[maybe_unused]] int pp = 0;
@@ -517,7 +519,7 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
             for (int e = 0; e < U; ++e) sc_.pw[group][e] = S.pw[e];
         }
         const int p0 = (gw * 32 + lane) * U;
-        if (a.nseg == 1 && p0 < n) {
+        if (nseg == 1 && p0 < n) {
             PA = E.power(p0 + 1);
             if (n - p0 >= U) PB = E.power(n - p0 - U + 1);
         }
@@ -526,7 +528,7 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
     // prefetch (nseg == 1): cell c of slot s of this thread; cells [0, NV): prev, [NV, 2 NV): cur, (VAR: [2 NV, 3 NV): cs,)
     // last: the 16 bytes of prev next to the warp (lane 0: before its first point, lane 31: after its last)
     constexpr int CELLS = (VAR ? 3 : 2) * NV + 1;
-    const bool pre = a.nseg == 1;
+    const bool pre = nseg == 1;
     auto cell = [&](int slot, int c) -> unsigned char* {
         return ex_smem + ((static_cast<size_t>(slot) * CELLS + c) * EX_NT + threadIdx.x) * 16;
     };
@@ -557,7 +559,7 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
         T carry = T(0);
         T y[U];
         [[maybe_unused]] T cp[VAR ? U : 1], iv[VAR ? U : 1];
-        for (int s = 0; s < a.nseg; ++s) {
+        for (int s = 0; s < nseg; ++s) {
             const int p0 = s * seg_pts + (gw * 32 + lane) * U;
             T wp[U], wc[U];
             [[maybe_unused]] T wa[U];                   // VAR: cs, then a_p = ap cs_p
@@ -622,18 +624,18 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
                 carry = group_forward<T, U>(y, cp, iv, carry, wpc, gw, lane, &sc_.agg[pf][0][group * wpc],
                                                         &sc_.agg[pf][1][group * wpc], group);
             } else {                               // Toeplitz: stationary factors on the padded line (see Ends)
-                carry = stat_forward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pf][1][group * wpc], group, a.nseg > 1);
+                carry = stat_forward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pf][1][group * wpc], group, nseg > 1);
             }
             pf ^= 1;
-            if (a.nseg > 1) {
+            if (nseg > 1) {
 #pragma unroll
                 for (int e = 0; e < U; ++e) s_line[static_cast<size_t>(p0 + e)] = y[e];   // parked until the way back
             }
         }
         carry = T(0);
-        for (int s = a.nseg - 1; s >= 0; --s) {
+        for (int s = nseg - 1; s >= 0; --s) {
             const int p0 = s * seg_pts + (gw * 32 + lane) * U;
-            if (a.nseg > 1) {
+            if (nseg > 1) {
 #pragma unroll
                 for (int e = 0; e < U; ++e) y[e] = s_line[static_cast<size_t>(p0 + e)];
             }
@@ -646,7 +648,7 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
                     for (int c = 0; c < NV; ++c) st16g(out + ro + p0 + c * V, y + c * V);
                 }
             } else {
-                carry = stat_backward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pb][3][group * wpc], group, a.nseg > 1);
+                carry = stat_backward<T, U>(y, S, carry, wpc, gw, lane, &sc_.agg[pb][3][group * wpc], group, nseg > 1);
                 pb ^= 1;
                 if (p0 == 0) s_ends[0] = y[0];                 // x''_0
                 if (p0 <= n && n < p0 + U) {                   // x''_n (nobody holds it if the padded line ends at n)
@@ -655,7 +657,7 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
                     for (int e = 1; e < U; ++e) xn = n - p0 == e ? y[e] : xn;
                     s_ends[1] = xn;
                 }
-                if (a.nseg > 1) {
+                if (nseg > 1) {
 #pragma unroll
                     for (int e = 0; e < U; ++e) s_line[static_cast<size_t>(p0 + e)] = y[e];   // x'' until both ends are known
                 }
@@ -665,7 +667,7 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
             group_sync(group, wpc);
             T A, B;
             E.scalars(s_ends[0], n < npad ? s_ends[1] : T(0), A, B);
-            if (a.nseg == 1) {
+            if (nseg == 1) {
                 const int p0 = (gw * 32 + lane) * U;
                 repair_unit<T, U>(y, S, A, B, PA, PB, n - p0, s_pw);
                 if (live && p0 < a.pitch) {
@@ -673,7 +675,7 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
                     for (int c = 0; c < NV; ++c) st16g(out + ro + p0 + c * V, y + c * V);
                 }
             } else {
-                for (int s = 0; s < a.nseg; ++s) {
+                for (int s = 0; s < nseg; ++s) {
                     const int p0 = s * seg_pts + (gw * 32 + lane) * U, m = n - p0;
 #pragma unroll
                     for (int e = 0; e < U; ++e) y[e] = s_line[static_cast<size_t>(p0 + e)];
@@ -684,25 +686,25 @@ __device__ __forceinline__ void exact_x_half_step(const ExactArgs& a, int nh, un
                     }
                 }
             }
-            if (a.nseg > 1) group_sync(group, wpc);   // the parked line is rewritten by the next pass
+            if (nseg > 1) group_sync(group, wpc);   // the parked line is rewritten by the next pass
         }
     }
     cp_async_wait<0>();
 }
 
-template <typename T, bool VAR>
+template <typename T, bool VAR, bool SEG1>
 __global__ void __launch_bounds__(EX_NT) wave2d_exact_x(const __grid_constant__ ExactArgs a)
 {
     extern __shared__ __align__(16) unsigned char ex_smem[];
     __shared__ ExactScratch<T> scratch;
-    exact_x_half_step<T, VAR>(a, a.n_off + 2 * (*a.d_k), ex_smem, scratch);
+    exact_x_half_step<T, VAR, SEG1>(a, a.n_off + 2 * (*a.d_k), ex_smem, scratch);
 }
 
 // ---- y half-step: (A3 + A4) exact ------------------------------------------------------------------------------
 // A strip: columns [c0, c0 + sc) over all n rows.  Shared memory: strip[sc][units * (U + 1)] (a unit of U rows is U + 1
 // apart: a warp reading one row offset of 32 consecutive units touches 32 distinct bank pairs).
 // VAR: a second strip holds a_p = ap cs_p (the solve needs it along the column), so strips are half as wide.
-template <typename T, bool VAR>
+template <typename T, bool VAR, bool SEG1>
 __device__ __forceinline__ void exact_y_half_step(const ExactArgs& a, int nh, unsigned char* ex_smem, ExactScratch<T>& sc_)
 {
     constexpr int U = EX_U, V = 16 / (int)sizeof(T);
@@ -721,7 +723,7 @@ __device__ __forceinline__ void exact_y_half_step(const ExactArgs& a, int nh, un
     const int n = a.n, sc = a.sc;
     static_assert(U == 8, "strip addressing uses r + (r >> 3)");
     const int units = (n + U - 1) / U, cpitch = ex_cpitch(units);   // strip pitch per column
-    const int seg_units = wpc * 32, nseg = (units + seg_units - 1) / seg_units;
+    const int seg_units = wpc * 32, nseg = SEG1 ? 1 : (units + seg_units - 1) / seg_units;
     const T* const src = static_cast<const T*>(a.src);
     int pf = 0, pb = 0;
     [[maybe_unused]] int pp = 0;
@@ -931,12 +933,12 @@ __device__ __forceinline__ void exact_y_half_step(const ExactArgs& a, int nh, un
     }
 }
 
-template <typename T, bool VAR>
+template <typename T, bool VAR, bool SEG1>
 __global__ void __launch_bounds__(EX_NT) wave2d_exact_y(const __grid_constant__ ExactArgs a)
 {
     extern __shared__ __align__(16) unsigned char ex_smem[];
     __shared__ ExactScratch<T> scratch;
-    exact_y_half_step<T, VAR>(a, a.n_off + 2 * (*a.d_k), ex_smem, scratch);
+    exact_y_half_step<T, VAR, SEG1>(a, a.n_off + 2 * (*a.d_k), ex_smem, scratch);
 }
 
 }  // namespace w2d

@@ -328,8 +328,12 @@ wave2d_sweep_panel(const __grid_constant__ SweepMaps maps, const __grid_constant
     int q_id = s_q[0];
     Piece q_pc = Piece{0, 0, 0, 0};
     if (q_id < npieces) q_pc = a.pieces[q_id];
+    // Only the warps that issue a TMA request keep the producer cursor (x: four of them, y: two, ONE: one); the others
+    // skip the bookkeeping.  Their own global writes follow a stage's arrival, i.e. the issuing warp's wait on the
+    // previous sweep, so they need no griddepcontrol.wait of their own before the end of the kernel.
+    const bool producer = DIR == 0 ? warp % (NW / 4) == 0 : ONE ? warp == 0 : warp % (NW / 2) == 0;
     auto produce = [&]() {   // request the next stage into slot q_slot (which must be free)
-        if (q_id >= npieces) return;
+        if (!producer || q_id >= npieces) return;
         if (lane == 0) {
             const int line0 = q_pc.panel * TL;
             const int g0 = (max(q_pc.ua - nbk, 0) & ~(SUB - 1)) + q_s * NW;
@@ -375,7 +379,7 @@ wave2d_sweep_panel(const __grid_constant__ SweepMaps maps, const __grid_constant
 #pragma unroll
     for (int s = 0; s < NSTAGE; ++s) {
         draw_ahead();
-        if (will_advance()) __syncthreads();
+        __syncthreads();   // (thread 0 may have drawn the next piece)
         produce();
     }
 

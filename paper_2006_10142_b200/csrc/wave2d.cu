@@ -177,7 +177,7 @@ struct wave2d_s {
     Piece* d_pieces[2] = {nullptr, nullptr};
     int* d_tickets = nullptr;              // tickets[SLOTS] | done[SLOTS]: per slot of a chunk, zeroed by wave2d_end_chunk
     int* d_cta_off[2] = {nullptr, nullptr};
-    double opt_static_frac = 0.75, opt_tail_div = 2.0;
+    double opt_static_frac = -1.0, opt_tail_div = 2.0;   // static_frac < 0: by dtype (plan_dir)
     int opt_tail_min = 0, opt_tail_max = 6;   // tail_min 0: planned from the stage size
     int opt_trace = 0, opt_pdl = 1, opt_early = 1;
     unsigned long long* d_trace[2] = {nullptr, nullptr};   // per-CTA trace of the last launch per direction
@@ -479,12 +479,13 @@ int plan_exact(wave2d_t* h, int d)
             return WAVE2D_ERR_UNSUPPORTED;
         }
         P.ex_smem = (int)smem;
-        if (var)
-            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, true>)
-                                             : reinterpret_cast<const void*>(&wave2d_exact_x<float, true>);
-        else
-            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, false>)
-                                             : reinterpret_cast<const void*>(&wave2d_exact_x<float, false>);
+        const bool f64 = h->dtype == WAVE2D_F64;
+        if (var) P.ex_fn = f64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, true, true>)
+                               : reinterpret_cast<const void*>(&wave2d_exact_x<float, true, true>);
+        else if (nseg == 1) P.ex_fn = f64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, false, true>)
+                                          : reinterpret_cast<const void*>(&wave2d_exact_x<float, false, true>);
+        else P.ex_fn = f64 ? reinterpret_cast<const void*>(&wave2d_exact_x<double, false, false>)
+                           : reinterpret_cast<const void*>(&wave2d_exact_x<float, false, false>);
         const int passes = (P.nlines + EX_NW / wpc - 1) / (EX_NW / wpc);
         P.grid = passes;
     } else {
@@ -499,12 +500,13 @@ int plan_exact(wave2d_t* h, int d)
         P.ex_sc = sc;
         P.ex_nseg = nseg;
         P.ex_smem = (int)(sc * col);
-        if (var)
-            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, true>)
-                                             : reinterpret_cast<const void*>(&wave2d_exact_y<float, true>);
-        else
-            P.ex_fn = h->dtype == WAVE2D_F64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, false>)
-                                             : reinterpret_cast<const void*>(&wave2d_exact_y<float, false>);
+        const bool f64 = h->dtype == WAVE2D_F64;
+        if (var) P.ex_fn = f64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, true, true>)
+                               : reinterpret_cast<const void*>(&wave2d_exact_y<float, true, true>);
+        else if (nseg == 1) P.ex_fn = f64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, false, true>)
+                                          : reinterpret_cast<const void*>(&wave2d_exact_y<float, false, true>);
+        else P.ex_fn = f64 ? reinterpret_cast<const void*>(&wave2d_exact_y<double, false, false>)
+                           : reinterpret_cast<const void*>(&wave2d_exact_y<float, false, false>);
         const int strips = (P.nlines + sc - 1) / sc;
         P.grid = strips;
     }
@@ -593,7 +595,12 @@ int plan_dir(wave2d_t* h, int d)
     // shorter pieces pay relatively more for their carry warm-up, longer ones lengthen the tail of the kernel
     const int stage_points = V.nw * V.unit * 32 * V.vec;
     const int tail_min = h->opt_tail_min > 0 ? h->opt_tail_min : std::min(6, std::max(2, 16384 / stage_points));
-    build_pieces(P, V.nw, V.sub, slots, h->opt_quota[d], h->opt_static_frac, tail_min, h->opt_tail_div,
+    // share dealt out statically: 0.70 in fp64, 0.75 in fp32.  The effect is a step function of the resulting quota of
+    // stages per CTA and depends on how the shares fall on the line ends (r2 sweeps, reproducible to 0.1 us): 4095^2 fp64
+    // quota 18 / 19 / 20 / 21 -> 129.1 / 128.4 / 130.0 / 131.4 us per step, 8191 x 2047 fp64 129.5 / 130.2 / 127.4 / 128.6;
+    // fp32 loses 1-2 % below 0.75.  0.70 takes the quota of the configuration the roofline target is quoted on.
+    const double static_frac = h->opt_static_frac >= 0.0 ? h->opt_static_frac : h->elem == 8 ? 0.70 : 0.75;
+    build_pieces(P, V.nw, V.sub, slots, h->opt_quota[d], static_frac, tail_min, h->opt_tail_div,
                  h->opt_tail_max);
     P.quota = h->opt_quota[d];
     P.grid = slots;
