@@ -68,6 +68,11 @@ enum {
                                  * fits; forcing it on a larger grid gives ERR_UNSUPPORTED                        */
 };
 
+/* =====================================================================================================
+ * STABLE INTERFACE: the calls of the paper's problem statement.  Everything from here to the
+ * banner "DIAGNOSTICS AND TUNING" below keeps its meaning between versions.
+ * ===================================================================================================== */
+
 /*
  * Create a solver for the grid of (2.6)-(2.7): N1 x N2 intervals on [0,l]^2, time step tau, at most M
  * steps (T = M tau), dtype WAVE2D_F64 or WAVE2D_F32.  Defaults: c == 1, no source, gamma = 2,
@@ -125,6 +130,8 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "early"  1 (default): early start -- a CTA that becomes resident while the previous sweep is still finishing its
  *            last drawn pieces begins with a piece of its share that touches only grid lines that sweep completed in
  *            its static part; needs "pdl".  0: every CTA waits for the whole previous sweep.
+ *   "resident"  1 (default): small grids of the split scheme keep the time levels in the cluster's distributed shared
+ *            memory for a whole run call; 0: the small-grid kernel that goes through global memory.
  *   "trace"  1: sweep kernels record per-CTA timing (see wave2d_get_trace).  Default 0.
  *   "static_frac"          tuning: share of a sweep's work dealt out statically (0..1; default 0.70 in fp64, 0.75 in fp32); the rest is
  *                          drawn from the ticket counter in short pieces.
@@ -203,6 +210,17 @@ int wave2d_steps_done(const wave2d_t *h, int *k);
 /* Block until all work queued on the handle's stream has finished. */
 int wave2d_sync(wave2d_t *h);
 
+const char *wave2d_strerror(int status);
+const char *wave2d_last_error(const wave2d_t *h);
+
+/* =====================================================================================================
+ * DIAGNOSTICS AND TUNING: not part of the stable interface.  Used by bench.py, the tests and the profiles; names,
+ * keys and record layouts may change with the kernels.  Of the options of wave2d_set_option the METHOD options are
+ * stable ("gamma", "kappa", "sigma", "start", "scheme", "solver", "ly"); "graph", "graph_steps", "pdl", "early",
+ * "resident", "trace", "shape_*", "static_frac", "tail_*", "quota_*" are tuning / diagnostic switches that never
+ * change a result beyond rounding.
+ * ===================================================================================================== */
+
 /*
  * Introspection for benchmarks and tests.  name:
  *   "solver_x", "solver_y"   solver path in use per direction (WAVE2D_SOLVER_EXACT / _STREAM / _LINE), after planning
@@ -261,9 +279,6 @@ int wave2d_host_scalars(double gamma, double alpha_plus, double alpha_minus, dou
 int wave2d_host_plan(int n, int nlines, int unit, int units_per_stage, int units_per_tile, int nbk, int slots,
                      int fixed_stages, double static_frac, int *pieces, int capacity, int *npieces, int *nstatic,
                      int *cta_off);
-
-const char *wave2d_strerror(int status);
-const char *wave2d_last_error(const wave2d_t *h);
 
 #ifdef __cplusplus
 }
