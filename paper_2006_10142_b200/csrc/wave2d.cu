@@ -4,6 +4,7 @@
 
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>   // header-only: ranges show up in a timeline profiler, cost nothing without one
 
 #include <algorithm>
 #include <cmath>
@@ -21,6 +22,12 @@
 using namespace w2d;
 
 namespace {
+
+// NVTX range for the duration of a scope ("x_sweep" / "y_sweep" around the sweep launches, the API calls by name)
+struct Range {
+    explicit Range(const char* name) { nvtxRangePushA(name); }
+    ~Range() { nvtxRangePop(); }
+};
 
 // ------------------------------------------------------------------------------------------------
 // Kernel variants: (NW consumer warps = units per stage, NSTAGE) per dtype and direction.
@@ -813,6 +820,7 @@ ExactArgs exact_args(const wave2d_t* h, int d)
 int launch_half_step(wave2d_t* h, cudaStream_t stream, int n_off, bool after_own)
 {
     const int d = n_off & 1;
+    Range range(d == 0 ? "x_sweep" : "y_sweep");   // (launch or capture of the sweep; a graph replay is inside "wave2d_run")
     const DirPlan& P = h->plan[d];
     const int* dk = h->d_k;
     const void* src = h->have_src && !(h->scheme == 1 && d == 1) ? h->src_dev[d] : nullptr;   // scheme 1: f enters in x only
@@ -1145,6 +1153,7 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
 
 int wave2d_set_initial(wave2d_t* h, const void* phi, const void* psi, long ld)
 {
+    Range range("wave2d_set_initial");
     if (!h || !phi || ld < h->n1) return WAVE2D_ERR_ARG;
     if (h->scheme == 1) return set_initial_factored(h, phi, psi, ld);
     // w_0 = phi -> buf[1]; psi staged in buf[2]; w_{-1} = phi - (tau/2) psi -> buf[0]   (roles of half-step 0)
@@ -1282,6 +1291,7 @@ int wave2d_set_source(wave2d_t* h, const void* s, long ld, const double* g_half,
 
 int wave2d_run(wave2d_t* h, int steps)
 {
+    Range range("wave2d_run");
     if (!h || steps < 0) return WAVE2D_ERR_ARG;
     if (!h->have_initial) return WAVE2D_ERR_STATE;
     if ((long long)h->k + steps > h->M) return WAVE2D_ERR_RANGE;
@@ -1325,6 +1335,7 @@ int wave2d_run(wave2d_t* h, int steps)
 
 int wave2d_get(wave2d_t* h, void* u_out, long ld)
 {
+    Range range("wave2d_get");
     if (!h) return WAVE2D_ERR_ARG;
     if (h->scheme == 1) return copy_out(h, u_out, ld, h->buf[(h->k - 1) & 3]);   // U^k
     return copy_out(h, u_out, ld, h->buf[(2 * h->k + 1) % 3]);
