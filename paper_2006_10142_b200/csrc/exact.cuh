@@ -803,27 +803,34 @@ __device__ __forceinline__ void exact_y_half_step(const ExactArgs& a, int nh, un
                     }
                 }
             }
+            // (the item's column range and its strip column are fixed: the source test and the strip addresses per item)
+            const int colb = c0 + kc * ve;
+            const bool src_item = src != nullptr && !one && colb < a.sl0 + a.snl && colb + ve > a.sl0 &&
+                                  r0 < a.sp0 + a.snp && r0 + RB > a.sp0;
+            T* const sp = strip + static_cast<size_t>(kc * ve) * cpitch;
+            [[maybe_unused]] T* const spa = strip_a + static_cast<size_t>(kc * ve) * cpitch;
 #pragma unroll
             for (int k = 0; k < RB; ++k) {
                 const int r = r0 + k;
                 if (r < n) {
-                    const bool src_r = src != nullptr && !one && r >= a.sp0 && r < a.sp0 + a.snp;
                     const int so = r + (r >> 3);
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
                         if (e < ve) {
-                            const int col = c0 + kc * ve + e;
                             T rv;
                             if constexpr (VAR) {   // am_p = am cs_p at the point of the equation
                                 const T amp = am * vs[k][e];
                                 rv = fmaT(g2, vc[k][e], fmaT(amp, vm[k][e] + vm[k + 2][e], -fmaT(T(2), amp, gam) * vm[k + 1][e]));
-                                strip_a[(kc * ve + e) * cpitch + so] = ap * vs[k][e];
+                                spa[e * cpitch + so] = ap * vs[k][e];
                             } else {
                                 rv = one ? vc[k][e] : fmaT(g2, vc[k][e], fmaT(am, vm[k][e] + vm[k + 2][e], c1 * vm[k + 1][e]));
                             }
-                            if (src_r && col >= a.sl0 && col < a.sl0 + a.snl)
-                                rv = fmaT(q, src[static_cast<size_t>(r - a.sp0) * a.snl + (col - a.sl0)], rv);
-                            strip[(kc * ve + e) * cpitch + so] = rv;
+                            if (src_item) {
+                                const int col = colb + e;
+                                if (r >= a.sp0 && r < a.sp0 + a.snp && col >= a.sl0 && col < a.sl0 + a.snl)
+                                    rv = fmaT(q, src[static_cast<size_t>(r - a.sp0) * a.snl + (col - a.sl0)], rv);
+                            }
+                            sp[e * cpitch + so] = rv;
                         }
                     }
                 }
@@ -921,8 +928,9 @@ __device__ __forceinline__ void exact_y_half_step(const ExactArgs& a, int nh, un
                 if (r < n) {
                     const int so = r + (r >> 3);
                     T vo[V];
+                    const T* const sp = strip + static_cast<size_t>(kc * ve) * cpitch + so;
 #pragma unroll
-                    for (int e = 0; e < V; ++e) vo[e] = e < ve ? strip[(kc * ve + e) * cpitch + so] : T(0);
+                    for (int e = 0; e < V; ++e) vo[e] = e < ve ? sp[e * cpitch] : T(0);
                     if (ve == V) st16g(o + k * a.pitch, vo);
                     else
                         for (int e = 0; e < ve; ++e) o[k * a.pitch + e] = vo[e];
