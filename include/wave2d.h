@@ -213,6 +213,49 @@ int wave2d_sync(wave2d_t *h);
 const char *wave2d_strerror(int status);
 const char *wave2d_last_error(const wave2d_t *h);
 
+/*
+ * Small grids without any allocation: `steps` time steps of Algorithm 1 (split scheme (2.11)-(2.12),
+ * PAPER.md:79-85, gamma = 2, kappa = 1/2, constant speed c, no source) in ONE kernel launch and nothing else -- no
+ * handle, no cudaMalloc / cudaFree, no host allocation, no copy, no synchronisation.
+ *
+ * Who needs this.  Everything else in this header works on a wave2d_create handle, and a handle cudaMallocs its time
+ * levels, counters and scalar table.  That is not possible for every caller: code that runs inside a framework whose
+ * caching allocator has already taken the GPU's memory (a raw cudaMalloc from a library then fails while the framework
+ * still reports free space), a service whose device-memory budget is fixed at start-up, or a loop that shares the GPU
+ * with other streams (cudaMalloc and cudaFree synchronise the whole device and stall them).  Here the working memory of
+ * the small-grid kernel -- the ring of three time levels and two scalar rows -- is a fixed array inside the library
+ * image: 1 581 184 bytes (1.5 MiB) on every GPU that loads libwave2d.so, held from module load until the process exits.
+ *
+ * The limit.  Lines of at most 256 unknowns in each direction: N1, N2 <= 257.  Anything larger is refused with
+ * WAVE2D_ERR_UNSUPPORTED and a message in errbuf; use a handle then.
+ *
+ * Arguments.  N1, N2, l, tau, dtype as in wave2d_create; c > 0 the constant speed.  The state of Algorithm 1 is the pair
+ * (u^{k-1/2}, u^k): u_prev_half and u are read, u_out receives u^{k+steps} and u_prev_out (may be NULL)
+ * u^{k+steps-1/2}, so a second call continues where the first stopped.  A start from (2.9) with psi = 0 passes phi as both
+ * inputs.  All four are DEVICE arrays of the current device (host pointers are refused with ERR_ARG: staging them would
+ * need a buffer), interior layout, n2 = N2-1 rows of n1 = N1-1 values of the dtype, one row stride ld >= n1 in elements
+ * for all of them; the caller owns them.  The outputs may be the inputs (the kernel reads both inputs completely before
+ * it writes an output).  cuda_stream: the cudaStream_t to launch into (NULL = the default stream); the call returns as
+ * soon as the kernel is queued.  errbuf / errbuf_len: optional caller-owned buffer for the detail of a failure.
+ *
+ * Shared scratch.  There is ONE array per device for the whole process.  It keeps what the previous call left in it; each
+ * call rewrites every byte it later reads (the pad columns that must be zero included), so calls of any sizes and dtypes
+ * may follow each other.  But two calls whose kernels can overlap on the same GPU -- different streams with no event
+ * between them, or two host threads -- race on it and both results are garbage: order them on one stream or with events.
+ * Handles are not affected (they own their memory).
+ *
+ * First call on a device.  It does the one-time set-up for that device (looks up the array's device address -- every
+ * device has its own copy -- and opts the kernels in to their shared-memory size), with that device current; if the
+ * library's module was not loaded yet, this is also when the driver loads it and the array comes into being.  Make
+ * this first call during start-up, before any stream capture.
+ *
+ * Errors: ERR_ARG (bad size / NULL / host pointer / ld < n1), ERR_UNSUPPORTED (beyond the limit; device ordinal >= 64),
+ * ERR_CUDA (no sm_100 device, set-up or launch failed).
+ */
+int wave2d_small_steps_static(int N1, int N2, double l, double tau, double c, int steps, int dtype,
+                              const void *u_prev_half, const void *u, void *u_out, void *u_prev_out, long ld,
+                              void *cuda_stream, char *errbuf, int errbuf_len);
+
 /* =====================================================================================================
  * DIAGNOSTICS AND TUNING: not part of the stable interface.  Used by bench.py, the tests and the profiles; names,
  * keys and record layouts may change with the kernels.  Of the options of wave2d_set_option the METHOD options are

@@ -23,6 +23,7 @@ EXPORTS = [
     "wave2d_set_speed", "wave2d_set_speed_field", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
     "wave2d_get_rows", "wave2d_set_rows", "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
     "wave2d_host_scalars", "wave2d_host_plan", "wave2d_strerror", "wave2d_last_error",
+    "wave2d_small_steps_static",
 ]
 
 
@@ -74,6 +75,8 @@ def load_library() -> C.CDLL:
     L.wave2d_strerror.restype = C.c_char_p
     L.wave2d_last_error.argtypes = [vp]
     L.wave2d_last_error.restype = C.c_char_p
+    L.wave2d_small_steps_static.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int,
+                                            vp, vp, vp, vp, C.c_long, vp, C.c_char_p, C.c_int]
     _lib = L
     return L
 
@@ -274,6 +277,46 @@ def from_workload(w, dtype=None, solver=None, graph=None) -> "Wave2D":
         h.set_source(w.s.astype(npdt, copy=False), w.g_half)
     h.set_initial(w.phi.astype(npdt, copy=False), None if w.psi is None else w.psi.astype(npdt, copy=False))
     return h
+
+
+def small_steps_static(N1: int, N2: int, l: float, tau: float, c: float, steps: int, u_prev_half, u, u_out,
+                       u_prev_out=None, stream=None):
+    """wave2d_small_steps_static: `steps` time steps on a small grid (N1, N2 <= 257) with no allocation anywhere in
+    the library -- for callers that cannot cudaMalloc (a framework's allocator owns the GPU's memory, a fixed memory
+    budget, or other streams that a device-wide synchronisation would stall); the kernel's working memory is a 1.5 MiB
+    array inside libwave2d.so, shared by all calls in the process (see include/wave2d.h for what that implies).
+
+    u_prev_half, u (inputs: u^{k-1/2}, u^k) and u_out, u_prev_out (outputs: u^{k+steps}, u^{k+steps-1/2}; the second is
+    optional) are torch CUDA tensors of shape (N2-1, N1-1), float64 or float32, unit inner stride and one common row
+    stride; the caller creates them, this function only passes their pointers on.  Asynchronous on `stream` (default:
+    torch's current stream).  Nothing is returned: the result is in u_out / u_prev_out."""
+    import torch
+    L = load_library()
+    n1, n2 = N1 - 1, N2 - 1
+    fields = [u_prev_half, u, u_out] + ([] if u_prev_out is None else [u_prev_out])
+    for t in fields:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dim() == 2 and tuple(t.shape) == (n2, n1) and
+                t.stride(1) == 1 and t.dtype == u.dtype and t.stride(0) == u.stride(0)):
+            raise ValueError(f"expected CUDA tensors of shape {(n2, n1)}, one dtype, unit inner stride, one row stride")
+    if u.dtype not in (torch.float64, torch.float32):
+        raise ValueError("dtype must be float64 or float32")
+    ld = int(u.stride(0)) if n2 > 1 else n1
+    if stream is None:
+        stream = torch.cuda.current_stream(u.device)
+    sp = getattr(stream, "cuda_stream", stream)
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(u.device):
+        st = L.wave2d_small_steps_static(int(N1), int(N2), float(l), float(tau), float(c), int(steps),
+                                         F64 if u.dtype == torch.float64 else F32,
+                                         C.c_void_p(u_prev_half.data_ptr()), C.c_void_p(u.data_ptr()),
+                                         C.c_void_p(u_out.data_ptr()),
+                                         C.c_void_p(0 if u_prev_out is None else u_prev_out.data_ptr()), ld,
+                                         C.c_void_p(sp or 0), err, len(err))
+    if st != 0:
+        detail = L.wave2d_strerror(st).decode()
+        if err.value:
+            detail += "; " + err.value.decode()
+        raise Wave2DError(st, "wave2d_small_steps_static", detail)
 
 
 def host_scalars(gamma: float, alpha_plus: float, alpha_minus: float, q: float = 0.0) -> np.ndarray:

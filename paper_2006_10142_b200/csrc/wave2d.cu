@@ -1581,3 +1581,333 @@ const char* wave2d_strerror(int status)
 const char* wave2d_last_error(const wave2d_t* h) { return h ? h->err.c_str() : ""; }
 
 }  // extern "C"
+
+// =====================================================================================================
+// wave2d_small_steps_static (include/wave2d.h): the small-grid step loop for callers that must not allocate.
+//
+// The handle path above cudaMallocs its working memory (wave2d_create: three time levels and the counters; the first
+// run: the scalar table).  Some users of a small-grid solver cannot afford that: a plug-in inside a framework whose
+// caching allocator has already reserved the GPU's memory (a raw cudaMalloc then fails although the framework shows
+// free space), a service with a device-memory budget fixed at start-up, a control loop that other streams share the
+// GPU with (cudaMalloc / cudaFree synchronise the whole device and stall them).  For these the working memory of ONE
+// kernel -- the small-grid kernel of line.cuh, whose scratch is the ring of three time levels plus the two scalar rows
+// -- is the file-scope array below: it is part of the library image, so every GPU that loads libwave2d.so holds its
+// 1.5 MiB from module load until the process exits, and no call ever allocates or frees anything.
+//
+// The price: ONE array per device, shared by every call in the process.  It keeps whatever the last call left in it
+// (each call rewrites everything it later reads, see the kernel's prologue), and two calls whose kernels overlap on the
+// GPU (different streams without an event between them, or two host threads) overwrite each other's time levels.
+// =====================================================================================================
+#include <cstdarg>
+#include <mutex>
+
+namespace w2d_static {
+constexpr int NMAX = 32 * 8;                                                   // unknowns per line, either direction
+constexpr size_t FIELD_BYTES = (size_t)NMAX * NMAX * sizeof(double);           // one time level at the largest size
+constexpr size_t TABLE_BYTES = (size_t)2 * w2d::ROW_DOUBLES * sizeof(double);  // scalar rows of the x and y half-step
+constexpr size_t SCRATCH_BYTES = 3 * FIELD_BYTES + TABLE_BYTES;                // 1 581 184 bytes
+static_assert(NMAX <= w2d::KMAX, "every pivot of a line is tabulated");
+}  // namespace w2d_static
+
+// In HOST code this name is only a handle for cudaGetSymbolAddress: its host-side address is not device memory, and a
+// kernel handed `wave2d_static_scratch` directly would fault (or, where the GPU can reach host memory, quietly work on
+// the wrong bytes).  static_device() below asks the runtime for the device address, per device.
+static __device__ __align__(256) unsigned char wave2d_static_scratch[w2d_static::SCRATCH_BYTES];
+
+namespace {
+
+struct StaticArgs {
+    unsigned char* scratch;   // DEVICE address of wave2d_static_scratch on the device that runs the kernel
+    const void* in_prev;      // caller: u^{k-1/2}      } n2 rows of n1 values, row stride ld (elements)
+    const void* in_cur;       // caller: u^k            }
+    void* out_cur;            // caller: u^{k+nsteps}
+    void* out_prev;           // caller: u^{k+nsteps-1/2}, or NULL
+    long long ld, pitch;      // elements; pitch = row stride inside the scratch, a multiple of 16
+    int n1, n2, nsteps;
+    double g2;                // 2 gamma
+    double rows[2][ROW_DOUBLES];   // [0]: x half-steps, [1]: y half-steps (constant speed: two rows serve every step)
+};
+
+// wave2d_line_steps (line.cuh) with its global working memory inside `a.scratch` instead of cudaMalloc'd buffers:
+//   scratch + b * FIELD_BYTES, b = 0..2   the ring of time levels, roles by roles_of(nh, 3), rows a.pitch apart
+//   scratch + 3 * FIELD_BYTES             the two scalar rows (copied from the kernel parameters by CTA 0)
+// Prologue: the caller's two levels are copied into ring buffers 0 and 1 with the pad columns [n1, pitch) written as
+// zeros -- the only part of the scratch that must start at zero (a row's right-hand ghost value, (2.10)); ring buffer 2
+// is written by the first x half-step over the full pitch before anything reads it, so nothing a previous call left
+// behind is ever read.  Epilogue: the last two levels go to the caller's arrays.  Constant speed, no source, split
+// scheme (2.11)-(2.12) with gamma = 2, kappa = 1/2; the line solve is solve_line_warp, as in the handle path.
+// grid = one cluster; block = 32 * W threads; dynamic shared memory: two strips [16][32 U + 1] of T.
+template <typename T, int U, int W>
+__global__ void __launch_bounds__(32 * W, 1) wave2d_line_steps_static(const __grid_constant__ StaticArgs a)
+{
+    constexpr int V = 16 / (int)sizeof(T), NV = U / V, SC = 16, KC = SC / V, RP = 32 * U + 1;
+    extern __shared__ __align__(16) unsigned char static_smem[];
+    T* const s_prev = reinterpret_cast<T*>(static_smem);
+    T* const s_cur = s_prev + SC * RP;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int cta = (int)cluster_ctarank(), ncta = (int)cluster_nctarank();
+    const int p0 = U * lane;
+    const T g2 = static_cast<T>(a.g2);
+    auto level = [&](int b) { return reinterpret_cast<T*>(a.scratch + (size_t)b * w2d_static::FIELD_BYTES); };
+    double* const tab = reinterpret_cast<double*>(a.scratch + 3 * w2d_static::FIELD_BYTES);
+
+    // ---- prologue: scalar rows and the caller's two time levels into the scratch
+    if (cta == 0)
+        for (int i = threadIdx.x; i < 2 * ROW_DOUBLES; i += 32 * W) tab[i] = a.rows[i / ROW_DOUBLES][i % ROW_DOUBLES];
+    {
+        const T* const ip = static_cast<const T*>(a.in_prev);
+        const T* const ic = static_cast<const T*>(a.in_cur);
+        T* const b0 = level(0);   // roles_of(0, 3): w_{-1} = ring 0, w_0 = ring 1
+        T* const b1 = level(1);
+        for (int j = cta * W + warp; j < a.n2; j += ncta * W)
+            for (int i = lane; i < a.pitch; i += 32) {
+                const bool in = i < a.n1;
+                b0[j * a.pitch + i] = in ? ip[j * a.ld + i] : T(0);
+                b1[j * a.pitch + i] = in ? ic[j * a.ld + i] : T(0);
+            }
+    }
+    cluster_barrier();
+
+    for (int nh = 0; nh < 2 * a.nsteps; ++nh) {
+        const int d = nh & 1;
+        const double* row = tab + d * ROW_DOUBLES;
+        const Roles R = roles_of(nh, 3);
+        const T* const prev = level(R.prev);
+        const T* const cur = level(R.cur);
+        T* const out = level(R.out);
+        const int n = d == 0 ? a.n1 : a.n2, nlines = d == 0 ? a.n2 : a.n1;
+        const T am = static_cast<T>(a.rows[d][ROW_AM]), c1 = static_cast<T>(a.rows[d][ROW_C1]);
+        T cp[U], iv[U], qs[U];
+#pragma unroll
+        for (int e = 0; e < U; ++e) {            // beyond the line: cp = inv = 0 decouples the padding (x = 0 there)
+            const bool in = p0 + e < n;
+            cp[e] = in ? static_cast<T>(__ldcg(row + ROW_CP + p0 + e)) : T(0);
+            iv[e] = in ? static_cast<T>(__ldcg(row + ROW_INVP + p0 + e)) : T(0);
+            qs[e] = T(0);                        // no source
+        }
+        if (d == 0) {
+            // ---- x half-step: one warp per grid row, lanes along the row
+            const bool inrow = p0 < a.pitch;
+            for (int j = cta * W + warp; j < nlines; j += ncta * W) {
+                T wp[U], wc[U];
+#pragma unroll
+                for (int e = 0; e < U; ++e) wp[e] = wc[e] = T(0);
+                const long long o = static_cast<long long>(j) * a.pitch + p0;
+                if (inrow) {
+#pragma unroll
+                    for (int c = 0; c < NV; ++c) {
+                        ldcg16(prev + o + c * V, wp + c * V);
+                        ldcg16(cur + o + c * V, wc + c * V);
+                    }
+                }
+                solve_line_warp<T, U>(wp, wc, qs, cp, iv, am, c1, g2, false, lane);
+                if (inrow) {
+#pragma unroll
+                    for (int c = 0; c < NV; ++c) st16(out + o + c * V, wc + c * V);
+                }
+            }
+        } else {
+            // ---- y half-step: strips of 16 grid columns per CTA, transposed through shared memory
+            for (int c0 = SC * cta; c0 < nlines; c0 += SC * ncta) {
+                const int kc = threadIdx.x % KC, r0 = threadIdx.x / KC;
+                for (int r = r0; r < n; r += (32 * W) / KC) {
+                    T vp[V], vc[V];
+                    const long long o = static_cast<long long>(r) * a.pitch + c0 + kc * V;   // c0 + 16 <= pitch
+                    ldcg16(prev + o, vp);
+                    ldcg16(cur + o, vc);
+#pragma unroll
+                    for (int e = 0; e < V; ++e) {
+                        s_prev[(kc * V + e) * RP + r] = vp[e];
+                        s_cur[(kc * V + e) * RP + r] = vc[e];
+                    }
+                }
+                __syncthreads();
+                for (int w = warp; w < SC; w += W) {            // warp = grid column c0 + w (pad columns solve zeros)
+                    T wp[U], wc[U];
+#pragma unroll
+                    for (int e = 0; e < U; ++e) {
+                        const bool in = p0 + e < n;
+                        wp[e] = in ? s_prev[w * RP + p0 + e] : T(0);
+                        wc[e] = in ? s_cur[w * RP + p0 + e] : T(0);
+                    }
+                    solve_line_warp<T, U>(wp, wc, qs, cp, iv, am, c1, g2, false, lane);
+#pragma unroll
+                    for (int e = 0; e < U; ++e)
+                        if (p0 + e < n) s_cur[w * RP + p0 + e] = wc[e];
+                }
+                __syncthreads();
+                for (int r = r0; r < n; r += (32 * W) / KC) {
+                    T vo[V];
+#pragma unroll
+                    for (int e = 0; e < V; ++e) vo[e] = s_cur[(kc * V + e) * RP + r];
+                    st16(out + static_cast<long long>(r) * a.pitch + c0 + kc * V, vo);
+                }
+                __syncthreads();
+            }
+        }
+        cluster_barrier();   // the half-step's stores are visible to every CTA of the cluster
+    }
+
+    // ---- epilogue: roles_of(2 nsteps, 3): "cur" = u^{k+nsteps}, "prev" = u^{k+nsteps-1/2}
+    {
+        const Roles R = roles_of(2 * a.nsteps, 3);
+        const T* const fc = level(R.cur);
+        const T* const fp = level(R.prev);
+        T* const oc = static_cast<T*>(a.out_cur);
+        T* const op = static_cast<T*>(a.out_prev);
+        for (int j = cta * W + warp; j < a.n2; j += ncta * W)
+            for (int i = lane; i < a.n1; i += 32) {
+                oc[j * a.ld + i] = __ldcg(fc + j * a.pitch + i);
+                if (op != nullptr) op[j * a.ld + i] = __ldcg(fp + j * a.pitch + i);
+            }
+    }
+}
+
+template <typename T, int U>
+const void* static_kernel() { return reinterpret_cast<const void*>(&wave2d_line_steps_static<T, U, LINE_WARPS>); }
+
+const void* static_kernel_of(int dtype, int U)
+{
+    if (dtype == WAVE2D_F64) return U == 4 ? static_kernel<double, 4>() : static_kernel<double, 8>();
+    return U == 4 ? static_kernel<float, 4>() : static_kernel<float, 8>();
+}
+
+int static_smem_bytes(int dtype, int U) { return 2 * 16 * (32 * U + 1) * (dtype == WAVE2D_F64 ? 8 : 4); }
+
+// Per-device set-up, done by the first call on a device with that device current: the DEVICE address of the scratch
+// array (every device has its own copy of a __device__ variable, so the address is asked for per device) and the
+// opt-in to more than 48 KB of dynamic shared memory for the four instantiations.  Fixed-size table, no heap.
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDevice {
+    bool ready = false;
+    unsigned char* scratch = nullptr;
+};
+StaticDevice g_static_device[STATIC_MAX_DEVICES];
+std::mutex g_static_mutex;
+
+void static_msg(char* errbuf, int errbuf_len, const char* fmt, ...)
+{
+    if (!errbuf || errbuf_len <= 0) return;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(errbuf, (size_t)errbuf_len, fmt, ap);
+    va_end(ap);
+}
+
+int static_device(int dev, unsigned char** scratch, char* errbuf, int errbuf_len)
+{
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) {
+        static_msg(errbuf, errbuf_len, "device ordinal %d: the static path serves devices 0..%d", dev, STATIC_MAX_DEVICES - 1);
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& D = g_static_device[dev];
+    if (!D.ready) {
+        int major = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e == cudaSuccess && major != 10) {
+            static_msg(errbuf, errbuf_len, "device %d is not an sm_100 device: there is no other code path", dev);
+            return WAVE2D_ERR_CUDA;
+        }
+        unsigned char* ptr = nullptr;
+        if (e == cudaSuccess) e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), wave2d_static_scratch);
+        for (int dt = 0; dt < 2 && e == cudaSuccess; ++dt)
+            for (int U = 4; U <= 8 && e == cudaSuccess; U += 4)
+                e = cudaFuncSetAttribute(static_kernel_of(dt, U), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_smem_bytes(dt, U));
+        if (e != cudaSuccess || ptr == nullptr) {
+            static_msg(errbuf, errbuf_len, "set-up on device %d: %s", dev, cudaGetErrorString(e));
+            (void)cudaGetLastError();
+            return WAVE2D_ERR_CUDA;
+        }
+        D.scratch = ptr;
+        D.ready = true;
+    }
+    *scratch = D.scratch;
+    return WAVE2D_OK;
+}
+
+// a pointer the kernel can dereference on device `dev`?  (cudaPointerGetAttributes allocates nothing)
+bool static_on_device(const void* p, int dev)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeManaged || (at.type == cudaMemoryTypeDevice && at.device == dev);
+}
+
+}  // namespace
+
+extern "C" int wave2d_small_steps_static(int N1, int N2, double l, double tau, double c, int steps, int dtype,
+                                         const void* u_prev_half, const void* u, void* u_out, void* u_prev_out, long ld,
+                                         void* cuda_stream, char* errbuf, int errbuf_len)
+{
+    if (errbuf && errbuf_len > 0) errbuf[0] = '\0';
+    if (N1 < 2 || N2 < 2 || !(l > 0.0) || !(tau > 0.0) || !(c > 0.0) || steps < 1 ||
+        (dtype != WAVE2D_F64 && dtype != WAVE2D_F32) || !u_prev_half || !u || !u_out || ld < N1 - 1) {
+        static_msg(errbuf, errbuf_len, "wave2d_small_steps_static: need N1, N2 >= 2, l, tau, c > 0, steps >= 1, a valid dtype, "
+                   "non-NULL u_prev_half, u, u_out and ld >= N1 - 1");
+        return WAVE2D_ERR_ARG;
+    }
+    const int n1 = N1 - 1, n2 = N2 - 1;
+    if (n1 > w2d_static::NMAX || n2 > w2d_static::NMAX) {
+        static_msg(errbuf, errbuf_len, "wave2d_small_steps_static: %d x %d unknowns, but the static scratch holds lines of at most "
+                   "%d unknowns in each direction (N1, N2 <= %d); larger grids need a wave2d_create handle", n1, n2,
+                   w2d_static::NMAX, w2d_static::NMAX + 1);
+        return WAVE2D_ERR_UNSUPPORTED;
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        static_msg(errbuf, errbuf_len, "wave2d_small_steps_static: no CUDA device (there is no CPU fallback)");
+        (void)cudaGetLastError();
+        return WAVE2D_ERR_CUDA;
+    }
+    unsigned char* scratch = nullptr;
+    int st = static_device(dev, &scratch, errbuf, errbuf_len);
+    if (st) return st;
+    if (!static_on_device(u_prev_half, dev) || !static_on_device(u, dev) || !static_on_device(u_out, dev) ||
+        (u_prev_out && !static_on_device(u_prev_out, dev))) {
+        static_msg(errbuf, errbuf_len, "wave2d_small_steps_static: every field must be DEVICE memory of the current device %d "
+                   "(a host array would need a staging buffer, which this call may not allocate)", dev);
+        return WAVE2D_ERR_ARG;
+    }
+
+    StaticArgs a;   // 8.4 KB of kernel parameters, on the stack
+    a.scratch = scratch;
+    a.in_prev = u_prev_half; a.in_cur = u; a.out_cur = u_out; a.out_prev = u_prev_out;
+    a.ld = ld;
+    a.pitch = (n1 + 15) / 16 * 16;
+    a.n1 = n1; a.n2 = n2; a.nsteps = steps;
+    const double gamma = 2.0, sigma = 0.5, t2 = tau * tau;
+    a.g2 = 2.0 * gamma;
+    for (int d = 0; d < 2; ++d) {   // as build_table for scheme 0 with a constant speed and no source
+        const double hd = d == 0 ? l / N1 : l / N2;
+        fill_row(a.rows[d], gamma, sigma * t2 * c / (hd * hd), (1.0 - sigma) * t2 * c / (hd * hd), 0.0);
+    }
+    const int nmax = std::max(n1, n2);
+    const int U = nmax <= 32 * 4 ? 4 : 8;
+    const int ctas = std::max(1, std::min(8, std::max((n2 + LINE_WARPS - 1) / LINE_WARPS, (n1 + 15) / 16)));
+    void* args[1] = {&a};
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(ctas);
+    cfg.blockDim = dim3(32 * LINE_WARPS);
+    cfg.dynamicSmemBytes = static_smem_bytes(dtype, U);
+    cfg.stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = ctas;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    const cudaError_t e = cudaLaunchKernelExC(&cfg, static_kernel_of(dtype, U), args);
+    if (e != cudaSuccess) {
+        static_msg(errbuf, errbuf_len, "wave2d_small_steps_static: launch: %s", cudaGetErrorString(e));
+        (void)cudaGetLastError();
+        return WAVE2D_ERR_CUDA;
+    }
+    return WAVE2D_OK;
+}
