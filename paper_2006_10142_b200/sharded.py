@@ -123,6 +123,11 @@ class DistExchange:
                 recv.append((b.top + own, got))
         for w in dist.batch_isend_irecv(ops) if ops else []:
             w.wait()
+        if self.device is not None and self.torch.device(self.device).type == "cuda":
+            # On NCCL, wait() only makes torch's current stream wait for the transfer; the host goes on.  The engine copies
+            # the halo rows on a non-blocking stream of its own, which is ordered after neither: block the host until the
+            # rows have arrived (and the send buffers are no longer read) before set_rows touches them.
+            self.torch.cuda.current_stream(self.device).synchronize()
         for j0, got in recv:
             s.engine.set_rows(0, j0, got if got.is_cuda else got.numpy())
 

@@ -191,3 +191,57 @@ def test_three_blocks_on_one_gpu_match_the_oracle_and_the_single_handle(dtype, t
     finally:
         h.close()
     assert np.abs(got - one).max() <= (1e-12 if dtype == "f64" else 2e-5) * np.abs(want).max()
+
+
+NCCL_WORKER = r'''
+import os, sys
+sys.path.insert(0, os.environ["W2D_ROOT"])
+import numpy as np
+import torch
+import torch.distributed as dist
+from paper_2006_10142_b200 import sharded as S
+from tests.test_sharded import problem
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+torch.cuda.set_device(rank)
+dev = torch.device("cuda", rank)
+dist.init_process_group("nccl", device_id=dev)
+p = problem(N1=700, N2=1500, M=10, seed=11)
+shards, G = S.make_shards(p["N1"], p["N2"], p["l"], p["tau"], p["M"], "f64", world, p["phi"], p["psi"], p["c"], p["s"], p["g"],
+                          ranks=[rank])
+sh = shards[0]
+ex = S.DistExchange(sh, rank, world, dev)
+for _ in range(p["M"]):
+    sh.step(1)
+    ex.refresh()
+np.save(os.path.join(os.environ["W2D_OUT"], f"owned{rank}.npy"), sh.owned())
+sh.engine.close()
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+'''
+
+
+@pytest.mark.gpu
+def test_two_ranks_over_nccl_match_the_oracle(tmp_path):
+    """DistExchange on the CUDA library, one rank per GPU: the halo rows arrive on NCCL's stream and are written by the
+    engine's own stream, so the refresh has to order the two (it blocks the host on torch's current stream after the
+    waits).  A stale halo shows up as an error far above the tolerance.  Needs two GPUs; skipped on a one-GPU box."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), W2D_ROOT=ROOT, W2D_OUT=str(tmp_path), PYTHONPATH=ROOT)
+        procs.append(subprocess.Popen([sys.executable, "-c", NCCL_WORKER], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True, cwd=ROOT))
+    outs = [q.communicate(timeout=600)[0] for q in procs]
+    for q, out in zip(procs, outs):
+        assert q.returncode == 0, out
+    p = problem(N1=700, N2=1500, M=10, seed=11)
+    want = oracle.solve(p["N1"], p["N2"], p["l"], p["tau"], p["M"], p["phi"], p["psi"], c_half=p["c"], s=p["s"], g_half=p["g"])
+    got = np.concatenate([np.load(tmp_path / f"owned{r}.npy") for r in range(2)], axis=0)
+    assert np.abs(got - want).max() <= 1e-10 * np.abs(want).max()
