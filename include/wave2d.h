@@ -60,7 +60,9 @@ enum {
 enum {
     WAVE2D_SOLVER_AUTO = 0,     /* LINE on small grids; else streamed kernels where the decay bound
                                  * rho^H <= tol allows, else EXACT                                        */
-    WAVE2D_SOLVER_EXACT = 1,    /* whole lines on chip, nothing truncated (any tau/h; lines up to 16384 unknowns) */
+    WAVE2D_SOLVER_EXACT = 1,    /* whole lines on chip, nothing truncated (any tau/h); a line must fit one CTA's shared
+                                 * memory: x lines up to 24576 unknowns in fp64 (49152 in fp32), y lines up to 22752
+                                 * (45504); longer ones give ERR_UNSUPPORTED at the first plan, with the limit in the text */
     WAVE2D_SOLVER_STREAM = 2,   /* force the streamed kernels; ERR_UNSUPPORTED if the bound fails        */
     WAVE2D_SOLVER_LINE = 3      /* small grids (at most 256 unknowns per line in both directions): the whole step
                                  * loop in one launch of one thread-block cluster, every line solved whole and
@@ -78,7 +80,9 @@ enum {
  * steps (T = M tau), dtype WAVE2D_F64 or WAVE2D_F32.  Defaults: c == 1, no source, gamma = 2,
  * kappa = 1/2 (see wave2d_set_option).  Uses the current CUDA device and a non-blocking stream of its own.
  * Errors: ERR_ARG (N < 2, l <= 0, tau <= 0, M < 0, bad dtype, out == NULL), ERR_ALLOC, ERR_CUDA
- * (no device, or not an sm_100 device), ERR_UNSUPPORTED (a line too long for every solver path).
+ * (no device, or not an sm_100 device).  Whether a solver path can take the grid depends on options and speed samples
+ * that are set later, so a line too long for every path is reported by the first plan instead: wave2d_run or
+ * wave2d_get_info return ERR_UNSUPPORTED, never this call.
  */
 int wave2d_create(wave2d_t **out, int N1, int N2, double l, double tau, int M, int dtype);
 
@@ -104,8 +108,9 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
  *   "start"  scheme 1 only.  1 (default): (2.9) as printed, u^1 = phi + tau psi (first order).
  *            2: u^1 = phi + tau psi + (tau^2 / 2) (c^0 Lap_h phi + g^0 s), the Taylor value with u_tt from (2.1): the
  *            three-level scheme (2.8) is then second order in tau also for psi != 0 or f != 0.  The extra term needs
- *            the final speed and source samples, so it is added at the first wave2d_run (wave2d_get before that
- *            returns phi + tau psi).  With scheme 0, wave2d_run returns ERR_UNSUPPORTED.
+ *            the final speed and source samples, so it is added by the first wave2d_run with steps > 0: until then
+ *            -- after wave2d_run(h, 0) too, and always when M = 1, where no step can be run -- wave2d_get returns
+ *            the first-order phi + tau psi.  With scheme 0, wave2d_run returns ERR_UNSUPPORTED.
  *   "scheme" 0 (default): the split scheme (2.11)-(2.12) driven by Algorithm 1.
  *            1: the factorised form of the unsplit three-level scheme (2.8),
  *                 (I - ax+ Dx)(I - ay+ Dy) u^{k+1} = 2 u^k - (I - ax- Dx)(I - ay- Dy) u^{k-1} + tau^2 f^k,
@@ -173,6 +178,8 @@ int wave2d_set_speed(wave2d_t *h, const double *c_half, int count);
  * elimination pivots (a scan of linear-fractional maps, csrc/exact.cuh) inside the whole-line solvers, which read one
  * more field per sweep (32 instead of 24 bytes per point in fp64).  Split scheme only (scheme 1: ERR_UNSUPPORTED), lines
  * of at most 4096 unknowns (ERR_UNSUPPORTED at the first run otherwise), solver AUTO or EXACT.  Before the first run.
+ * The field is checked before anything changes: a call that fails with ERR_ARG leaves a previously accepted field (or
+ * c = c(t)) in force.
  */
 int wave2d_set_speed_field(wave2d_t *h, const void *cs, long ld);
 

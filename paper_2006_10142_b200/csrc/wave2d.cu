@@ -482,7 +482,11 @@ int plan_exact(wave2d_t* h, int d)
         const size_t smem = nseg > 1 ? (size_t)nseg * wpc * 32 * EX_U * h->elem
                                      : (size_t)2 * ((var ? 3 : 2) * (EX_U * h->elem / 16) + 1) * EX_NT * 16;
         if (smem > budget) {
-            h->err = "exact solver: an x line of more than 25600 fp64 unknowns does not fit shared memory";
+            const int seg = wpc * 32 * EX_U;   // a line is parked in whole segments
+            char msg[160];
+            snprintf(msg, sizeof msg, "exact solver: an x line of more than %d %s unknowns does not fit shared memory",
+                     (int)(budget / ((size_t)seg * h->elem)) * seg, h->elem == 8 ? "fp64" : "fp32");
+            h->err = msg;
             return WAVE2D_ERR_UNSUPPORTED;
         }
         P.ex_smem = (int)smem;
@@ -500,7 +504,12 @@ int plan_exact(wave2d_t* h, int d)
         int sc = 16;
         while (sc > 1 && sc * col > budget) sc /= 2;
         if (sc * col > budget) {
-            h->err = "exact solver: a y line of more than 22700 fp64 unknowns does not fit shared memory";
+            int mu = (int)(budget / h->elem / (EX_U + 1));   // most units whose one-column strip still fits
+            while (mu > 0 && (size_t)ex_cpitch(mu) * h->elem > budget) --mu;
+            char msg[160];
+            snprintf(msg, sizeof msg, "exact solver: a y line of more than %d %s unknowns does not fit shared memory",
+                     mu * EX_U, h->elem == 8 ? "fp64" : "fp32");
+            h->err = msg;
             return WAVE2D_ERR_UNSUPPORTED;
         }
         while (sc > 1 && (P.nlines + sc - 1) / sc < h->num_sms) sc /= 2;   // small grids: more, narrower strips
@@ -1214,28 +1223,32 @@ int wave2d_set_speed_field(wave2d_t* h, const void* cs, long ld)
     if (!h) return WAVE2D_ERR_ARG;
     if (h->ran) return WAVE2D_ERR_STATE;
     if (cs && (ld < h->n1 || h->scheme == 1)) return h->scheme == 1 ? WAVE2D_ERR_UNSUPPORTED : WAVE2D_ERR_ARG;
-    invalidate_plan(h);
-    h->have_cs = false;
-    if (!cs) return WAVE2D_OK;
-    const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
-    if (!h->d_cs) {
-        int st = dev_alloc(h, &h->d_cs, fbytes);
-        if (st) return st;
+    if (!cs) {
+        invalidate_plan(h);
+        h->have_cs = false;
+        return WAVE2D_OK;
     }
-    W2D_CUDA(h, cudaMemsetAsync(h->d_cs, 0, fbytes, h->stream));
-    int st = copy_in(h, h->d_cs, cs, ld);
-    if (st) return st;
-    // every value must be positive: checked on a host copy
+    // every value must be positive: checked on a host copy BEFORE the handle is touched, so that a
+    // rejected field leaves a previously accepted one in place
     const size_t e = h->elem, n1 = h->n1, n2 = h->n2;
     std::vector<unsigned char> host(n1 * n2 * e);
-    W2D_CUDA(h, cudaMemcpy2DAsync(host.data(), n1 * e, h->d_cs, (size_t)h->pitch * e, n1 * e, n2, cudaMemcpyDeviceToHost,
-                                  h->stream));
-    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    W2D_CUDA(h, cudaMemcpy2D(host.data(), n1 * e, cs, (size_t)ld * e, n1 * e, n2, cudaMemcpyDefault));
     for (size_t i = 0; i < n1 * n2; ++i) {
         const double v = h->dtype == WAVE2D_F64 ? reinterpret_cast<const double*>(host.data())[i]
                                                 : (double)reinterpret_cast<const float*>(host.data())[i];
         if (!(v > 0.0)) return WAVE2D_ERR_ARG;
     }
+    const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
+    if (!h->d_cs) {
+        int st = dev_alloc(h, &h->d_cs, fbytes);
+        if (st) return st;
+    }
+    invalidate_plan(h);
+    h->have_cs = false;   // until the new field is on the device
+    W2D_CUDA(h, cudaMemsetAsync(h->d_cs, 0, fbytes, h->stream));
+    W2D_CUDA(h, cudaMemcpy2DAsync(h->d_cs, (size_t)h->pitch * e, host.data(), n1 * e, n1 * e, n2, cudaMemcpyHostToDevice,
+                                  h->stream));
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     h->have_cs = true;
     return WAVE2D_OK;
 }

@@ -80,7 +80,7 @@ def test_random_cases_match_the_oracle(seed):
         finally:
             h.close()
         err = float(np.abs(u - r).max() / max(np.abs(r).max(), 1e-300))
-        tol = 3e-4 * max(1.0, p["tf"]) if f32 else 1e-10
+        tol = 1e-4 * max(1.0, p["tf"]) if f32 else 1e-10   # observed: <= 1.7e-5 over the 38 fp32 cases of these seeds
         assert np.isfinite(u).all() and err <= tol, (what, err)
         ran += 1
     assert ran >= 30

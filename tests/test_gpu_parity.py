@@ -1034,3 +1034,72 @@ def test_sigma_and_start_are_refused_where_they_do_not_apply():
             h.set_option("sigma", 0.0)
     finally:
         h.close()
+
+
+# ---- header = code: what a failed call leaves behind, the limits the error texts quote, start = 2 at M = 1 ----
+def test_a_rejected_speed_field_leaves_the_accepted_one_in_force():
+    """wave2d_set_speed_field checks the new field before it touches the handle: after ERR_ARG the run still uses the
+    field that was accepted before (it used to fall back to c = c(t) silently)."""
+    w = W.cfg2(N=200, M=6)
+    cs = _speed_field(np.random.default_rng(77), w.phi.shape)
+    r = oracle.solve(w.N1, w.N2, w.l, w.tau, w.M, w.phi, None, c_half=w.c_half, cs=cs)
+    h = B.from_workload(w)
+    try:
+        h.set_speed_field(cs)
+        bad = cs.copy()
+        bad[17, 23] = 0.0
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_speed_field(bad)
+        assert e.value.status == -1
+        h.run(w.M)
+        u = h.get()
+        assert h.info("solver_x") == B.SOLVER_EXACT      # the variable-speed path, not the Toeplitz one
+    finally:
+        h.close()
+    assert relerr(u, r) <= 1e-10
+    assert relerr(u, ref(w)) > 1e-3                      # and it differs from c = c(t)
+
+
+@pytest.mark.parametrize("dtype,N1,N2,text", [("f64", 24578, 3, "24576 fp64"), ("f32", 49154, 3, "49152 fp32"),
+                                              ("f64", 3, 22754, "22752 fp64"), ("f32", 3, 45506, "45504 fp32")])
+def test_exact_solver_limits_are_the_ones_the_header_states(dtype, N1, N2, text):
+    """One unknown more than include/wave2d.h's limit for WAVE2D_SOLVER_EXACT is refused at the first plan, with the limit
+    of THIS dtype in the message; the limit itself is accepted."""
+    for extra, ok in ((0, False), (-1, True)):
+        n1, n2 = (N1 + extra, N2) if N1 > N2 else (N1, N2 + extra)
+        h = B.Wave2D(n1, n2, 1.0, 1e-3, 2, dtype)
+        try:
+            h.set_option("solver", B.SOLVER_EXACT)
+            h.set_initial(np.ones((n2 - 1, n1 - 1), dtype=np.float64 if dtype == "f64" else np.float32))
+            if ok:
+                h.run(1)
+                assert np.isfinite(h.get()).all()
+            else:
+                with pytest.raises(B.Wave2DError) as e:
+                    h.run(0)
+                assert e.value.status == -5 and text in str(e.value), str(e.value)
+        finally:
+            h.close()
+
+
+def test_second_order_start_is_not_applied_before_a_step_is_run():
+    """include/wave2d.h, option "start": the tau^2/2 term is added by the first wave2d_run with steps > 0.  With M = 1 no
+    step can be run, so wave2d_get is the first-order phi + tau psi -- on both sides (the oracle adds it at the same place)."""
+    N, tau = 48, 0.02
+    rng = np.random.default_rng(5)
+    phi, psi = rng.uniform(-1, 1, (N - 1, N - 1)), rng.uniform(-1, 1, (N - 1, N - 1))
+    r = oracle.solve(N, N, 1.0, tau, 1, phi, psi, scheme=1, start=2)
+    np.testing.assert_allclose(r, phi + tau * psi, rtol=0, atol=1e-15)
+    h = B.Wave2D(N, N, 1.0, tau, 1, "f64")
+    try:
+        h.set_option("scheme", 1)
+        h.set_option("start", 2)
+        h.set_initial(phi, psi)
+        h.run(0)
+        assert h.steps_done() == 1
+        np.testing.assert_allclose(h.get(), r, rtol=0, atol=1e-15)
+        with pytest.raises(B.Wave2DError) as e:
+            h.run(1)
+        assert e.value.status == -6
+    finally:
+        h.close()
