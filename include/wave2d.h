@@ -326,6 +326,15 @@ int wave2d_get_trace(wave2d_t *h, int dir, unsigned long long *out, int capacity
  */
 int wave2d_host_scalars(double gamma, double alpha_plus, double alpha_minus, double q, double *out, int capacity,
                         int *count);
+/*
+ * wave2d_host_decay: the decay ratio rho of a sweep's systems tridiag(-alpha+, gamma + 2 alpha+, -alpha+) for lines of mesh
+ * width extent / N at the speed sample c: alpha+ = sigma tau^2 c / (extent / N)^2 ((2.11)-(2.12) times tau^2,
+ * PAPER.md:79-85), rho = the small root of alpha+ z^2 - (gamma + 2 alpha+) z + alpha+ -- the number the handle reports as
+ * "rho_x" / "rho_y" once it exists.  A line may be cut where G further points are available with rho^G below the rounding
+ * unit: the row-block driver (paper_2006_10142_b200/sharded.py) sizes its halo with it before any handle is created, so
+ * that no arithmetic of the method lives outside the library.  Errors: ERR_ARG.
+ */
+int wave2d_host_decay(int N, double extent, double tau, double c, double gamma, double sigma, double *rho);
 int wave2d_host_plan(int n, int nlines, int unit, int units_per_stage, int units_per_tile, int nbk, int slots,
                      int fixed_stages, double static_frac, int *pieces, int capacity, int *npieces, int *nstatic,
                      int *cta_off);

@@ -23,7 +23,7 @@ EXPORTS = [
     "wave2d_set_speed", "wave2d_set_speed_field", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
     "wave2d_get_rows", "wave2d_set_rows", "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
     "wave2d_host_scalars", "wave2d_host_plan", "wave2d_strerror", "wave2d_last_error",
-    "wave2d_small_steps_static",
+    "wave2d_small_steps_static", "wave2d_host_decay",
 ]
 
 
@@ -70,6 +70,7 @@ def load_library() -> C.CDLL:
     L.wave2d_get_trace.argtypes = [vp, C.c_int, vp, C.c_int, C.POINTER(C.c_int)]
     ip = C.POINTER(C.c_int)
     L.wave2d_host_scalars.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, dp, C.c_int, ip]
+    L.wave2d_host_decay.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, dp]
     L.wave2d_host_plan.argtypes = [C.c_int] * 8 + [C.c_double, ip, C.c_int, ip, ip, ip]
     L.wave2d_strerror.argtypes = [C.c_int]
     L.wave2d_strerror.restype = C.c_char_p
@@ -329,6 +330,16 @@ def host_scalars(gamma: float, alpha_plus: float, alpha_minus: float, q: float =
     if st != 0:
         raise Wave2DError(st, "wave2d_host_scalars", L.wave2d_strerror(st).decode())
     return out[:cnt.value].copy()
+
+
+def host_decay(N: int, extent: float, tau: float, c: float, gamma: float = 2.0, sigma: float = 0.5) -> float:
+    """wave2d_host_decay: rho of a sweep over lines of mesh width extent / N at speed c (host only, no device)."""
+    L = load_library()
+    rho = C.c_double()
+    st = L.wave2d_host_decay(int(N), float(extent), float(tau), float(c), float(gamma), float(sigma), C.byref(rho))
+    if st != 0:
+        raise Wave2DError(st, "wave2d_host_decay", L.wave2d_strerror(st).decode())
+    return rho.value
 
 
 def host_plan(n: int, nlines: int, unit: int, units_per_stage: int, units_per_tile: int, nbk: int, slots: int,

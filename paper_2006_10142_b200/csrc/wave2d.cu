@@ -1552,6 +1552,17 @@ int wave2d_host_scalars(double gamma, double alpha_plus, double alpha_minus, dou
     return WAVE2D_OK;
 }
 
+int wave2d_host_decay(int N, double extent, double tau, double c, double gamma, double sigma, double* rho)
+{
+    if (N < 2 || !(extent > 0.0) || !(tau > 0.0) || !(c > 0.0) || !(gamma > 0.0) || !(sigma > 0.0 && sigma <= 1.0) || !rho)
+        return WAVE2D_ERR_ARG;
+    const double hd = extent / N;
+    double row[ROW_DOUBLES];
+    fill_row(row, gamma, sigma * tau * tau * c / (hd * hd), 0.0, 0.0);   // alpha+ as in build_table; alpha-, q do not enter rho
+    *rho = row[ROW_RHO];
+    return WAVE2D_OK;
+}
+
 int wave2d_host_plan(int n, int nlines, int unit, int units_per_stage, int units_per_tile, int nbk, int slots,
                      int fixed_stages, double static_frac, int* pieces, int capacity, int* npieces, int* nstatic,
                      int* cta_off)

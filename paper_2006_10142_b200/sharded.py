@@ -15,15 +15,13 @@ u^{k+1/2} needs no exchange: the next x half-step recomputes its halo rows from 
 physical boundary has no halo there (the true Dirichlet condition).  The exchange is point-to-point between neighbours
 (`torch.distributed` isend / irecv: NCCL over NVLink on GPUs, gloo in the CPU test); `LocalExchange` moves the rows
 inside one process, which is how the path is tested on one GPU.  No arithmetic of the method lives here: the engine is
-the C ABI (binding.Wave2D), the halo width comes from the library's own scalars (wave2d_host_scalars).
+the C ABI (binding.Wave2D), the halo width comes from the library's own decay ratio (wave2d_host_decay).
 """
 from __future__ import annotations
 
 import math
 
 import numpy as np
-
-ROW_RHO = 2   # include/wave2d.h, wave2d_host_scalars: out[2] = rho
 
 
 def halo_rows(rho: float, tol: float) -> int:
@@ -147,11 +145,9 @@ class Shard:
 
 
 def y_decay(N2: int, l: float, tau: float, c_half, gamma: float = 2.0, sigma: float = 0.5) -> float:
-    """rho of the y systems at the largest speed sample (the library's own scalar row)."""
+    """rho of the y systems at the largest speed sample: computed by the library (wave2d_host_decay), not here."""
     from . import binding
-    h2 = l / N2
-    ap = sigma * tau * tau * float(np.max(c_half)) / (h2 * h2)
-    return float(binding.host_scalars(gamma, ap, ap, 0.0)[ROW_RHO])
+    return binding.host_decay(N2, l, tau, float(np.max(c_half)), gamma, sigma)
 
 
 def make_shards(N1: int, N2: int, l: float, tau: float, M: int, dtype: str, world: int, phi, psi=None, c_half=None,

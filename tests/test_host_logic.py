@@ -84,3 +84,23 @@ def test_host_entry_points_reject_bad_arguments():
         B.host_plan(100, 100, 8, 16, 2, 17, 148)     # carry series longer than a stage
     with pytest.raises(B.Wave2DError):
         B.host_plan(0, 100, 8, 16, 2, 3, 148)
+
+
+@pytest.mark.parametrize("N,extent,tau,c,gamma,sigma", [(1024, 1.0, 1.0 / 1024, 1.5, 2.0, 0.5), (2048, 1.0, 1.0 / 8192, 1.3, 2.0, 0.5),
+                                                        (150, 1.0, 1.0 / 150, 1.3, 2.0, 1.0), (4096, 1.0, 16.0 / 4096, 1.0, 1.0, 0.75)])
+def test_decay_ratio_of_a_sweep(N, extent, tau, c, gamma, sigma):
+    """wave2d_host_decay (what the row-block driver sizes its halo with): alpha+ = sigma tau^2 c / h^2, rho the small root of
+    alpha+ z^2 - (gamma + 2 alpha+) z + alpha+ -- against the root written in its cancellation-free form, against the
+    decay of a dense solve with a unit right-hand side at one end, and against the scalar row of the same alpha+."""
+    rho = B.host_decay(N, extent, tau, c, gamma, sigma)
+    h = extent / N
+    ap = sigma * tau * tau * c / (h * h)
+    beta = gamma + 2 * ap
+    assert abs(rho - 2 * ap / (beta + np.sqrt(beta * beta - 4 * ap * ap))) <= 4e-16
+    assert rho == B.host_scalars(gamma, ap, 0.3, 0.0)[2]
+    n = 800                                    # long enough that the far end's reflection (rho^(2 (n - j))) is below rounding
+    T = np.diag(np.full(n, beta)) + np.diag(np.full(n - 1, -ap), 1) + np.diag(np.full(n - 1, -ap), -1)
+    x = np.linalg.solve(T, np.eye(n)[0])
+    np.testing.assert_allclose(x[11:21] / x[10:20], rho, rtol=1e-9)     # the influence of an end decays like rho per point
+    with pytest.raises(B.Wave2DError):
+        B.host_decay(N, extent, tau, -1.0)
