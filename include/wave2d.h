@@ -150,6 +150,21 @@ int wave2d_set_stream(wave2d_t *h, void *cuda_stream);
 int wave2d_set_option(wave2d_t *h, const char *name, double value);
 
 /*
+ * Caller-owned memory for the time levels (SURVEY.md 8b "Memory"; optional).  By default the handle cudaMallocs its
+ * ring of time levels (three fields, four with scheme 1: all but a few KB of what it owns).  A caller that manages
+ * device memory itself -- PyTorch's caching allocator, an arena -- can hand the library a block instead:
+ * wave2d_workspace_bytes gives the size for the handle's current scheme, wave2d_set_workspace attaches a DEVICE block of
+ * at least that size, 256-byte aligned (ERR_ARG otherwise; a torch allocation is).  The handle frees its own fields,
+ * zeroes the block and keeps every time level in it; the caller must keep the block alive and untouched until
+ * wave2d_destroy or wave2d_set_workspace(h, NULL, 0) (back to memory of its own).  The small tables and counters stay
+ * handle-owned.  Allowed before wave2d_set_initial only (ERR_STATE afterwards), and after the scheme is chosen:
+ * wave2d_set_option(h, "scheme", 1) on a handle with a three-field workspace gives ERR_STATE.
+ * For a step loop that allocates nothing at all on small grids see wave2d_small_steps_static.
+ */
+int wave2d_workspace_bytes(const wave2d_t *h, unsigned long long *bytes);
+int wave2d_set_workspace(wave2d_t *h, void *workspace, unsigned long long bytes);
+
+/*
  * Initial data (2.2)-(2.3), discretised as in (2.9) adapted to half-levels:
  *   u^0 = phi,  u^{-1/2} = phi - (tau/2) psi     (psi == NULL means psi = 0, i.e. Algorithm 1's "u = U0").
  * Resets the step count to 0.  Synchronous for host pointers.

@@ -23,7 +23,7 @@ EXPORTS = [
     "wave2d_set_speed", "wave2d_set_speed_field", "wave2d_set_source", "wave2d_run", "wave2d_get", "wave2d_get_prev",
     "wave2d_get_rows", "wave2d_set_rows", "wave2d_steps_done", "wave2d_sync", "wave2d_get_info", "wave2d_profile_sweeps", "wave2d_get_trace",
     "wave2d_host_scalars", "wave2d_host_plan", "wave2d_strerror", "wave2d_last_error",
-    "wave2d_small_steps_static", "wave2d_host_decay",
+    "wave2d_small_steps_static", "wave2d_host_decay", "wave2d_workspace_bytes", "wave2d_set_workspace",
 ]
 
 
@@ -70,6 +70,8 @@ def load_library() -> C.CDLL:
     L.wave2d_get_trace.argtypes = [vp, C.c_int, vp, C.c_int, C.POINTER(C.c_int)]
     ip = C.POINTER(C.c_int)
     L.wave2d_host_scalars.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, dp, C.c_int, ip]
+    L.wave2d_workspace_bytes.argtypes = [vp, C.POINTER(C.c_ulonglong)]
+    L.wave2d_set_workspace.argtypes = [vp, vp, C.c_ulonglong]
     L.wave2d_host_decay.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, dp]
     L.wave2d_host_plan.argtypes = [C.c_int] * 8 + [C.c_double, ip, C.c_int, ip, ip, ip]
     L.wave2d_strerror.argtypes = [C.c_int]
@@ -157,6 +159,22 @@ class Wave2D:
 
     def set_option(self, name: str, value: float):
         self._check(self._L.wave2d_set_option(self._h, name.encode(), float(value)), "wave2d_set_option")
+
+    def workspace_bytes(self) -> int:
+        n = C.c_ulonglong()
+        self._check(self._L.wave2d_workspace_bytes(self._h, C.byref(n)), "wave2d_workspace_bytes")
+        return int(n.value)
+
+    def set_workspace(self, block):
+        """Keep the time levels in `block` (a torch CUDA tensor of at least workspace_bytes() bytes, or None to return
+        to handle-owned memory).  The handle holds a reference, so the block outlives it."""
+        if block is None:
+            self._check(self._L.wave2d_set_workspace(self._h, None, 0), "wave2d_set_workspace")
+            self._workspace = None
+            return
+        nbytes = block.numel() * block.element_size()
+        self._check(self._L.wave2d_set_workspace(self._h, C.c_void_p(block.data_ptr()), nbytes), "wave2d_set_workspace")
+        self._workspace = block
 
     def set_initial(self, phi, psi=None):
         keep = []

@@ -8,6 +8,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -161,6 +162,7 @@ struct wave2d_s {
     int scheme = 0;                      // 0: split scheme (2.11)-(2.12); 1: factorised unsplit scheme (2.8)
     bool v_ready = false;                // scheme 1: V^0, V^1 computed from U^0, U^1 (needs the final c samples)
     void* buf[4] = {nullptr, nullptr, nullptr, nullptr};   // scheme 0 uses 3
+    bool ext_fields = false;             // the ring lives in caller memory (wave2d_set_workspace): never freed here
     std::vector<double> c_half, g_half;  // g_half empty: g == 1
     bool have_cs = false;                // spatial speed factor set (wave2d_set_speed_field): variable-coefficient solvers
     void* d_cs = nullptr;                // pitched like a field, pad 0
@@ -1084,7 +1086,8 @@ void wave2d_destroy(wave2d_t* h)
     if (!h) return;
     if (h->stream) cudaStreamSynchronize(h->stream);
     drop_graph(h);
-    for (int b = 0; b < 4; ++b) cudaFree(h->buf[b]);
+    if (!h->ext_fields)
+        for (int b = 0; b < 4; ++b) cudaFree(h->buf[b]);
     cudaFree(h->src_dev[0]);
     cudaFree(h->src_dev[1]);
     cudaFree(h->d_cs);
@@ -1130,6 +1133,10 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
         if ((iv != 0 && iv != 1) || h->have_initial) return WAVE2D_ERR_ARG;
         if (iv == 1 && (h->have_cs || h->sigma != 0.5)) return WAVE2D_ERR_UNSUPPORTED;   // variable speed, sigma: split scheme only
         if (iv == 1 && !h->buf[3]) {
+            if (h->ext_fields) {   // a three-field workspace is attached: the scheme has to be chosen before it
+                h->err = "scheme 1 needs a fourth field: set the scheme before wave2d_set_workspace";
+                return WAVE2D_ERR_STATE;
+            }
             const size_t fbytes = (size_t)h->pitch * h->n2 * h->elem;
             int st = dev_alloc(h, &h->buf[3], fbytes);
             if (st) return st;
@@ -1157,6 +1164,60 @@ int wave2d_set_option(wave2d_t* h, const char* name, double value)
     else if (!strcmp(name, "quota_y")) { if (iv < 0) return WAVE2D_ERR_ARG; h->opt_quota[1] = iv; }
     else return WAVE2D_ERR_ARG;
     invalidate_plan(h);
+    return WAVE2D_OK;
+}
+
+// bytes of one time level inside a caller's workspace (a multiple of 256, so that every level starts 256-byte aligned)
+static size_t workspace_slice(const wave2d_t* h)
+{
+    return ((size_t)h->pitch * h->n2 * h->elem + 255) / 256 * 256;
+}
+
+int wave2d_workspace_bytes(const wave2d_t* h, unsigned long long* bytes)
+{
+    if (!h || !bytes) return WAVE2D_ERR_ARG;
+    *bytes = (unsigned long long)(h->scheme == 1 ? 4 : 3) * workspace_slice(h);
+    return WAVE2D_OK;
+}
+
+int wave2d_set_workspace(wave2d_t* h, void* workspace, unsigned long long bytes)
+{
+    if (!h) return WAVE2D_ERR_ARG;
+    if (h->have_initial || h->ran) return WAVE2D_ERR_STATE;   // the ring would lose its contents
+    const int nf = h->scheme == 1 ? 4 : 3;
+    const size_t slice = workspace_slice(h), fbytes = (size_t)h->pitch * h->n2 * h->elem;
+    if (workspace) {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, workspace) != cudaSuccess ||
+            (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)) {
+            (void)cudaGetLastError();
+            h->err = "wave2d_set_workspace: not device memory";
+            return WAVE2D_ERR_ARG;
+        }
+        if (reinterpret_cast<uintptr_t>(workspace) % 256 != 0 || bytes < (unsigned long long)nf * slice) {
+            h->err = "wave2d_set_workspace: needs a 256-byte aligned block of at least wave2d_workspace_bytes() bytes";
+            return WAVE2D_ERR_ARG;
+        }
+    } else if (!h->ext_fields) {
+        return WAVE2D_OK;   // already on its own memory
+    }
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
+    invalidate_plan(h);   // the TMA descriptors and the graphs name the field addresses
+    if (!h->ext_fields)
+        for (int b = 0; b < 4; ++b) dev_free(h, h->buf[b], h->buf[b] ? fbytes : 0);
+    for (int b = 0; b < 4; ++b) h->buf[b] = nullptr;
+    h->ext_fields = false;
+    if (workspace) {
+        for (int b = 0; b < nf; ++b) h->buf[b] = static_cast<unsigned char*>(workspace) + (size_t)b * slice;
+        h->ext_fields = true;
+    } else {
+        for (int b = 0; b < nf; ++b) {
+            int st = dev_alloc(h, &h->buf[b], fbytes);
+            if (st) return st;
+        }
+    }
+    for (int b = 0; b < nf; ++b) W2D_CUDA(h, cudaMemsetAsync(h->buf[b], 0, fbytes, h->stream));   // pad columns stay zero
+    W2D_CUDA(h, cudaStreamSynchronize(h->stream));
     return WAVE2D_OK;
 }
 

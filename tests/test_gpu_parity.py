@@ -1103,3 +1103,73 @@ def test_second_order_start_is_not_applied_before_a_step_is_run():
         assert e.value.status == -6
     finally:
         h.close()
+
+
+# ---- SURVEY.md 8b "Memory": the ring of time levels in a block the caller allocated (wave2d_set_workspace) ---------------------
+@pytest.mark.parametrize("name,w,scheme", [("cfg2_N700", W.cfg2(N=700, M=20), 0), ("cfg3_N300", W.cfg3(N=300, M=30), 0),
+                                           ("cfg1", W.cfg1(), 0), ("cfg2_N700_scheme1", W.cfg2(N=700, M=20), 1),
+                                           ("cfg4_f32", W.cfg4(N1=1030, N2=270, M=12, dtype="f32"), 0)],
+                         ids=["cfg2_N700", "cfg3_N300", "cfg1", "cfg2_N700_scheme1", "cfg4_f32"])
+def test_workspace_owned_by_the_caller(name, w, scheme):
+    """A torch allocation backs the time levels: same result, bit for bit, as the handle that allocates its own; the
+    handle then owns less than one field of device memory; the block can be dropped only after the handle."""
+    import torch
+    npdt = np.float64 if w.dtype == "f64" else np.float32
+
+    def run(with_block):
+        h = B.Wave2D(w.N1, w.N2, w.l, w.tau, w.M, w.dtype)
+        try:
+            if scheme:
+                h.set_option("scheme", 1)
+            own = h.info("device_bytes")
+            if with_block:
+                need = h.workspace_bytes()
+                field = h.info("pitch") * w.n2 * (8 if w.dtype == "f64" else 4)
+                assert (4 if scheme else 3) * field <= need <= (4 if scheme else 3) * (field + 255)
+                block = torch.full((need,), 0x7f, dtype=torch.uint8, device="cuda")     # garbage: the library clears it
+                h.set_workspace(block)
+                assert h.info("device_bytes") < min(field, own - 2 * field)
+            h.set_speed(w.c_half)
+            if w.s is not None:
+                h.set_source(w.s.astype(npdt), w.g_half)
+            h.set_initial(w.phi.astype(npdt), None if w.psi is None else w.psi.astype(npdt))
+            h.run(w.M - h.steps_done())
+            return h.get()
+        finally:
+            h.close()
+
+    u_own, u_ws = run(False), run(True)
+    assert np.array_equal(u_own, u_ws)
+    r = oracle.solve(w.N1, w.N2, w.l, w.tau, w.M, w.phi, w.psi, c_half=w.c_half, s=w.s, g_half=w.g_half, scheme=scheme)
+    assert relerr(u_ws, r) <= TOL[w.dtype]
+
+
+def test_workspace_state_machine():
+    import torch
+    h = B.Wave2D(200, 120, 1.0, 0.004, 6)
+    try:
+        need = h.workspace_bytes()
+        block = torch.empty((need + 256,), dtype=torch.uint8, device="cuda")
+        for bad in (block[:need - 1], block[1:need + 1], torch.empty((need,), dtype=torch.uint8)):
+            with pytest.raises(B.Wave2DError) as e:      # too small; not 256-byte aligned; host memory
+                h.set_workspace(bad)
+            assert e.value.status == -1
+        h.set_workspace(block)
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_option("scheme", 1)                    # the fourth field is not there: choose the scheme first
+        assert e.value.status == -2
+        h.set_workspace(None)                            # back to memory of its own ...
+        h.set_option("scheme", 1)                        # ... where the fourth field can be allocated
+        assert h.workspace_bytes() == need // 3 * 4
+        h.set_option("scheme", 0)
+        h.set_workspace(block)
+        phi = np.random.default_rng(1).uniform(-1, 1, (119, 199))
+        h.set_initial(phi)
+        with pytest.raises(B.Wave2DError) as e:
+            h.set_workspace(None)                        # not once the ring holds data
+        assert e.value.status == -2
+        h.run(6)
+        u = h.get()
+    finally:
+        h.close()
+    assert relerr(u, oracle.solve(200, 120, 1.0, 0.004, 6, phi)) <= 1e-10
