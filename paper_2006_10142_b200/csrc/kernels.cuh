@@ -39,15 +39,43 @@ struct __align__(8) vec2f {
     __device__ __forceinline__ vec2f(float a, float b) : x(a), y(b) {}
     __device__ __forceinline__ vec2f(int a) : x(static_cast<float>(a)), y(static_cast<float>(a)) {}
     __device__ __forceinline__ explicit vec2f(double a) : x(static_cast<float>(a)), y(static_cast<float>(a)) {}
-    __device__ __forceinline__ vec2f& operator+=(const vec2f& b) { x += b.x; y += b.y; return *this; }
-    __device__ __forceinline__ vec2f& operator*=(const vec2f& b) { x *= b.x; y *= b.y; return *this; }
+    __device__ __forceinline__ vec2f& operator+=(const vec2f& b);
+    __device__ __forceinline__ vec2f& operator*=(const vec2f& b);
 };
-__device__ __forceinline__ vec2f operator+(const vec2f& a, const vec2f& b) { return vec2f(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ vec2f operator*(const vec2f& a, const vec2f& b) { return vec2f(a.x * b.x, a.y * b.y); }
+// Blackwell's packed fp32 pipe: one FFMA2 / FMUL2 / FADD2 works on both elements of a 64-bit register pair
+// (fma.rn.f32x2 etc., sm_100+), rounding each element exactly like the scalar instruction.
+__device__ __forceinline__ unsigned long long pack2(const vec2f& a)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+    return r;
+}
+__device__ __forceinline__ vec2f unpack2(unsigned long long r)
+{
+    vec2f a;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+    return a;
+}
+__device__ __forceinline__ vec2f operator+(const vec2f& a, const vec2f& b)
+{
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)));
+    return unpack2(r);
+}
+__device__ __forceinline__ vec2f operator*(const vec2f& a, const vec2f& b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)));
+    return unpack2(r);
+}
 __device__ __forceinline__ vec2f fmaT(const vec2f& a, const vec2f& b, const vec2f& c)
 {
-    return vec2f(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y));
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)), "l"(pack2(c)));
+    return unpack2(r);
 }
+__device__ __forceinline__ vec2f& vec2f::operator+=(const vec2f& b) { *this = *this + b; return *this; }
+__device__ __forceinline__ vec2f& vec2f::operator*=(const vec2f& b) { *this = *this * b; return *this; }
 __device__ __forceinline__ double fmaT(double a, double b, double c) { return ::fma(a, b, c); }
 __device__ __forceinline__ float fmaT(float a, float b, float c) { return ::fmaf(a, b, c); }
 
